@@ -1,0 +1,129 @@
+/* nnp.h -- C-ABI boundary of the B200-native NNP energy+force evaluator.
+ *
+ * One call of nnp_eval = one evaluation of the ML potential behind the paper's ML/MM interface:
+ *   inputs  = atomic numbers, positions, simulation box, PBC type, ML index group (PAPER.md line 77,
+ *             "multiple inputs to the model can be specified, such as atomic numbers, positions, the
+ *             simulation box and type of periodic boundary conditions ... ML subsystem ... index group");
+ *   outputs = E_ML and F_i = -grad_i E_ML (eq. 2), the forces being
+ *             "supplied directly by the model".
+ * The model is the ANI / Behler-Parrinello descriptor network fixed by BASELINE.json (north_star stages
+ * 1-4) and restated in SURVEY.md Appendix A; DESIGN.md lists every reading taken.
+ *
+ * Conventions
+ *   - every function returns an int status: NNP_OK (0) or a negative NNP_ERR_* code; no exceptions/aborts.
+ *   - "host" / "device" is stated for every pointer.  Device pointers are owned by the caller.
+ *   - units are nominal: Angstrom in, "eV" and "eV/Angstrom" out (weights are synthetic).
+ *   - nnp_eval is asynchronous on the workspace stream, allocates nothing and never synchronises, so a
+ *     sequence of calls can be captured into a CUDA graph.  Device-side faults (unknown species,
+ *     neighbour overflow, coincident atoms) are recorded in a sticky flag read by nnp_status().
+ *   - there is NO CPU fallback: without a CUDA device every compute entry point returns NNP_ERR_CUDA.
+ */
+#ifndef NNP_H_
+#define NNP_H_
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NNP_OK 0
+#define NNP_ERR_INVALID_ARG (-1)     /* null/negative/unsorted/out-of-range argument, dims[0] != AEV length */
+#define NNP_ERR_UNKNOWN_SPECIES (-2) /* an ML atom's Z has no species slot or no network (MM atoms' Z unread) */
+#define NNP_ERR_BOX_UNSUPPORTED (-3) /* non-zero off-diagonal or non-positive length (orthorhombic only)      */
+#define NNP_ERR_CAPACITY (-4)        /* a neighbour row overflowed the workspace's row capacity                */
+#define NNP_ERR_COINCIDENT (-5)      /* two ML atoms at distance exactly 0                                     */
+#define NNP_ERR_CUDA (-6)            /* CUDA runtime error or no device                                        */
+#define NNP_ERR_UNSUPPORTED (-7)     /* descriptor shape outside the kernels' range (see nnp_model_create)     */
+
+typedef struct nnp_model nnp_model;         /* opaque, immutable after create, shareable between workspaces */
+typedef struct nnp_workspace nnp_workspace; /* opaque scratch, one per stream, not thread-safe              */
+
+/* Descriptor hyper-parameters (BASELINE.json configs[0]). All arrays are HOST
+ * arrays and are copied.  AEV length = n_species*nShfR + n_species*(n_species+1)/2 * nShfA*nShfZ;
+ * element order: radial s*nShfR+m, angular n_species*nShfR + p(s1,s2)*nShfA*nShfZ + a*nShfZ + z with
+ * p = s1*S - s1*(s1-1)/2 + (s2-s1), s1 <= s2 (reading #11). */
+typedef struct {
+  double Rcr, Rca, EtaR, EtaA, Zeta;
+  int32_t nShfR, nShfA, nShfZ;
+  const double *ShfR, *ShfA, *ShfZ;
+  double radial_prefactor;  /* c_R, 0.25 (reading #2)                                 */
+  double cos_scale;         /* c_theta, 0.95: theta = acos(c_theta cos) (reading #3)  */
+  int32_t n_species;
+  const int32_t* species_Z; /* [n_species] slot -> atomic number, e.g. {1,6,7,8}      */
+} nnp_aev_params;
+
+/* One per species slot; n_layers = 0 => the slot has no network (an ML atom of it is an error). */
+typedef struct {
+  int32_t n_layers;        /* 1..4 layers; hidden layers CELU(alpha), last layer linear (reading #14)   */
+  const int32_t* dims;     /* HOST [n_layers+1]; dims[0] = AEV length, dims[n_layers] = 1               */
+  const float* const* W;   /* HOST W[l]: dims[l+1] x dims[l], row-major [out][in]                       */
+  const float* const* b;   /* HOST b[l]: dims[l+1]                                                      */
+  double celu_alpha;       /* 0.1                                                                       */
+} nnp_mlp_desc;
+
+/* MLP arithmetic (nnp_workspace_set_mlp_mode):
+ *   NNP_MLP_FP32_SIMT  fp32 FMA on CUDA cores (reference rung of the precision ladder, slow)
+ *   NNP_MLP_BF16X3     tcgen05 tensor cores, operands split x = hi + lo in bf16, three products
+ *                      hi*hi + hi*lo + lo*hi accumulated in fp32 TMEM (default)
+ *   NNP_MLP_BF16X1     tcgen05, one bf16 product (fails the force tolerance; for the ladder only) */
+#define NNP_MLP_FP32_SIMT 0
+#define NNP_MLP_BF16X3 1
+#define NNP_MLP_BF16X1 2
+
+/* Creates the immutable model: copies parameters, uploads weights (and the derived bf16 hi/lo tile
+ * images) to the current CUDA device.  Limits: n_species <= 8, nShfR <= 16, nShfA*nShfZ == 32,
+ * hidden widths multiples of 16 and <= 256, n_layers <= 4  -> otherwise NNP_ERR_UNSUPPORTED. */
+int nnp_model_create(const nnp_aev_params* aev, const nnp_mlp_desc* nets /* HOST [n_species] */, nnp_model** out);
+int nnp_model_destroy(nnp_model*);
+int nnp_model_aev_length(const nnp_model*);
+
+/* Allocates all device scratch for up to max_ml_atoms ML atoms out of up to max_atoms atoms.
+ * cuda_stream: a cudaStream_t (0 = legacy default stream).  Neighbour-row capacities default to
+ * 128 radial / 48 angular (observed maxima on liquid water: 71 / 26). */
+int nnp_workspace_create(const nnp_model*, int64_t max_atoms, int64_t max_ml_atoms, void* cuda_stream,
+                         nnp_workspace** out);
+int nnp_workspace_destroy(nnp_workspace*);
+int nnp_workspace_set_mlp_mode(nnp_workspace*, int32_t mode);
+
+/* One energy+force evaluation.  Asynchronous on the workspace stream.
+ *   d_pos      DEVICE [n_atoms][3] fp32, Angstrom, any periodic image
+ *   d_Z        DEVICE [n_atoms] int32 atomic numbers (only ML atoms' entries are read)
+ *   box        HOST   [9] row vectors a,b,c in Angstrom; orthorhombic only (read during the call)
+ *   pbc        1 = xyz periodic (minimum image), 0 = open boundaries (box ignored)
+ *   d_ml_index DEVICE [n_ml] int32 strictly ascending atom indices, or NULL => all atoms are ML (n_ml ignored)
+ *   d_energy   DEVICE [1] fp64
+ *   d_forces   DEVICE [n_atoms][3] fp32; rows of non-ML atoms are set to +0.0f
+ * Returns NNP_ERR_INVALID_ARG for sizes beyond the workspace, NNP_ERR_BOX_UNSUPPORTED for a bad box.
+ * Content errors found on the device (unsorted ml_index, unknown species, overflow, coincident atoms)
+ * surface through nnp_status(); outputs are then unspecified. */
+int nnp_eval(nnp_workspace*, int64_t n_atoms, const float* d_pos, const int32_t* d_Z, const float box[9],
+             int32_t pbc, const int32_t* d_ml_index, int64_t n_ml, double* d_energy, float* d_forces);
+
+/* Same evaluation with HOST buffers: copies inputs to workspace-owned device buffers, runs nnp_eval,
+ * copies energy and forces back and synchronises the stream.  h_ml_index may be NULL.  This is the
+ * end-to-end entry point a host MD engine (GROMACS nnpot) would call. */
+int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int32_t* h_Z, const float box[9],
+                  int32_t pbc, const int32_t* h_ml_index, int64_t n_ml, double* h_energy, float* h_forces);
+
+/* Synchronises the stream and returns the sticky device status (NNP_OK or the first NNP_ERR_* seen),
+ * then clears it. */
+int nnp_status(nnp_workspace*);
+const char* nnp_strerror(int);
+
+/* Debug / parity exports of the LAST evaluation (synchronising; HOST output buffers).
+ *   nnp_debug_neighbors: which = 0 radial (R <= Rcr), 1 angular (R <= Rca).  CSR over ML rows in
+ *     ml_index order; h_col = GLOBAL atom indices, ascending within a row.  Pass h_col = NULL (or a too
+ *     small cap) to query *n_pairs only.
+ *   nnp_debug_aev: fp32 AEV rows [n_ml][aev_length] in ml_index order.
+ *   nnp_debug_atomic_energies: [n_ml] in ml_index order.
+ *   nnp_debug_counters: launches[0] = number of kernels launched by the last nnp_eval. */
+int nnp_debug_neighbors(nnp_workspace*, int which, int64_t* n_pairs, int32_t* h_row_start, int32_t* h_col,
+                        int64_t col_cap);
+int nnp_debug_aev(nnp_workspace*, float* h_aev);
+int nnp_debug_atomic_energies(nnp_workspace*, float* h_e);
+int nnp_debug_counters(nnp_workspace*, int64_t* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NNP_H_ */

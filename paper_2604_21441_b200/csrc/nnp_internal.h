@@ -1,0 +1,152 @@
+// nnp_internal.h -- shared declarations of the CUDA path (not part of the C-ABI; never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/nnp.h"
+
+namespace nnp {
+
+constexpr int MAX_S = 8;          // species slots
+constexpr int MAX_LAYERS = 4;
+constexpr int TILE_M = 128;       // MLP row tile (tcgen05 M)
+constexpr int HP = 256;           // pitch of the hidden-activation / delta scratch rows (max hidden width)
+constexpr int NSHFR = 16;         // radial shifts (fixed by the kernels)
+constexpr int NSHFA = 4;          // angular radial shifts
+constexpr int NSHFZ = 8;          // angular theta shifts
+constexpr int BLK = 32;           // AEV column block: one angular pair (4x8) or two radial species (2x16)
+constexpr int MAX_BLK = 40;       // ceil(8/2) + 8*9/2
+constexpr int RCAP_MAX = 128;     // radial neighbour row capacity (positions fit a uint8 with room to spare)
+constexpr int ACAP_MAX = 48;      // angular neighbour row capacity
+constexpr int JBITS = 26;         // neighbour entry: sorted index in the low 26 bits, 3x2-bit cell offset above
+constexpr uint32_t JMASK = (1u << JBITS) - 1u;
+constexpr int FIX_SHIFT = 40;     // fixed-point scale 2^40 for the int64 force accumulators (K8)
+
+// device-side sticky status bits
+enum : int { FLAG_ARG = 1, FLAG_SPECIES = 2, FLAG_CAP = 4, FLAG_COINCIDENT = 8 };
+
+// Descriptor constants, passed to kernels by value.
+struct AevConst {
+  float Rcr, Rca, Rcr2, Rca2;
+  double Rcr2_d, Rca2_d;      // exact fp64 thresholds of the pinned neighbour predicate (reading #6)
+  float etaR, etaA;
+  float etaR_l2e, etaA_l2e;   // eta * log2(e): exp(-eta x^2) = exp2(-eta_l2e x^2)
+  float cR, cTheta, zeta;
+  int zeta_is_32;
+  float inv_Rcr, inv_Rca;     // 1 / Rc
+  int S;                      // species slots
+  int nRB;                    // radial column blocks = ceil(S/2)
+  int nblk_full;              // nRB + S(S+1)/2
+  int L;                      // AEV length in the public (BASELINE.json) order
+  float ShfR[NSHFR];
+  float ShfA[NSHFA];
+  float cosZ[NSHFZ], sinZ[NSHFZ];  // cos / sin of ShfZ
+  int8_t zlut[128];           // atomic number -> slot (-1: none / no network)
+};
+
+// Cell grid of one evaluation (device resident; written by k_grid_setup).
+struct GridInfo {
+  int nc[3];
+  int ncell;
+  int pbc;
+  float edge[3];       // cell edge per dimension
+  double edge_d[3];
+  double inv_edge_d[3];
+  double origin_d[3];  // 0 for pbc; bounding-box minimum for open boundaries
+  double L_d[3];       // box lengths (fp32 inputs promoted), for the exact predicate
+  float L[3];
+};
+
+// Species groups, MLP tiles and the compacted AEV column map of one evaluation (device resident; k_scan).
+// Internal AEV column order: radial species s at s*16 (padded to nRB*32 columns), angular pair p at
+// (nRB + p)*32.  Only column blocks that can be non-zero for the species present are materialised
+// ("structural-zero compaction"): compact column = cpos[block]*32 + (col % 32).
+struct GroupInfo {
+  int count[MAX_S];      // atoms per slot
+  int start[MAX_S + 1];  // first sorted index of the slot (sorted order is slot-major)
+  int pad_shift[MAX_S];  // row = sorted index + pad_shift[slot]; group rows padded to TILE_M
+  int n_tiles;
+  int n_rows;            // padded row count
+  int nblk;              // materialised column blocks
+  int Kc;                // 32 * nblk = row pitch of aev / daev
+  int blkmap[MAX_BLK];   // compact block -> internal block
+  int cpos[MAX_BLK];     // internal block -> compact block, or -1
+};
+
+struct TileInfo { int slot, row0, nvalid, pad; };
+
+struct Net {             // device pointers, one per slot
+  int n_layers;
+  int dims[MAX_LAYERS + 1];
+  const float* W[MAX_LAYERS];   // [out][in] fp32; layer 0 in the internal padded column order [out][Kfull]
+  const float* WT[MAX_LAYERS];  // [in][out] fp32; layer 0 [Kfull][out]
+  const float* b[MAX_LAYERS];
+  float alpha;
+};
+
+struct NetTable { Net net[MAX_S]; };
+
+}  // namespace nnp
+
+struct nnp_model {
+  nnp::AevConst aev;
+  nnp::NetTable nets;        // device pointers
+  int n_layers;              // common to all networks
+  int Kfull;                 // 32 * nblk_full
+  void* dev_blob;            // single allocation holding all fp32 weights
+  size_t blob_bytes;
+  void* tc;                  // tensor-core weight images (mlp_tc.cu), or nullptr
+};
+
+struct nnp_workspace {
+  const nnp_model* model;
+  cudaStream_t stream;
+  int64_t max_atoms, max_ml;
+  int rcap, acap;            // neighbour row capacities
+  int max_cells;
+  int mlp_mode;
+  int dense_k;               // 1: materialise every column block (no structural-zero compaction)
+  int64_t max_rows;          // padded AEV rows
+  int max_tiles;
+  // last evaluation
+  int64_t n_atoms, n_ml;
+  const int32_t* d_ml_index;
+  int64_t launches;
+  // device buffers
+  nnp::GridInfo* grid;
+  nnp::GroupInfo* groups;
+  nnp::TileInfo* tiles;
+  int* flags;
+  int* cell_count;           // [MAX_S*max_cells + 1]
+  int* bstart;               // [MAX_S*max_cells + 1]
+  float4* tmp4;              // [max_ml] local coords + key
+  int* rank;                 // [max_ml]
+  float4* spos;              // [max_ml] sorted: cell-local xyz, w = ml-local index | slot << 28
+  int* scell;                // [max_ml]
+  uint32_t* nbrR;            // [max_ml][rcap]
+  uint8_t* nbrA;             // [max_ml][acap] positions into the radial row
+  int* cntR; int* cntA;      // [max_ml]
+  float* aev;                // [max_rows][Kc] fp32
+  float* daev;               // [max_rows][Kc] fp32
+  float* hbuf[3];            // hidden activations [max_rows][HP]
+  float* dbuf[2];            // deltas [max_rows][HP]
+  float* e_atom;             // [max_rows]
+  unsigned long long* facc;  // [max_ml][3] int64 fixed point, indexed by sorted position
+  void* tc_ws;               // tensor-core path scratch
+  // host-buffer entry point
+  float* hd_pos; int32_t* hd_Z; int32_t* hd_ml; double* hd_energy; float* hd_forces;
+};
+
+namespace nnp {
+// stage launchers (each returns the number of kernels it launched)
+int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
+                          const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
+int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);
+int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
+int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
+int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
+                       float* d_forces);
+int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets);
+void tc_model_destroy(nnp_model* m);
+int tc_workspace_create(nnp_workspace* ws);
+void tc_workspace_destroy(nnp_workspace* ws);
+}  // namespace nnp
