@@ -84,6 +84,10 @@ int nnp_workspace_create(const nnp_model*, int64_t max_atoms, int64_t max_ml_ato
                          nnp_workspace** out);
 int nnp_workspace_destroy(nnp_workspace*);
 int nnp_workspace_set_mlp_mode(nnp_workspace*, int32_t mode);
+/* dense != 0: materialise every AEV column block (K = full padded AEV length, "as ANI would run it");
+ * 0 (default): only the column blocks that can be non-zero for the species present in the evaluation
+ * (exact structural-zero compaction).  Results are identical up to summation order. */
+int nnp_workspace_set_dense_k(nnp_workspace*, int32_t dense);
 
 /* One energy+force evaluation.  Asynchronous on the workspace stream.
  *   d_pos      DEVICE [n_atoms][3] fp32, Angstrom, any periodic image

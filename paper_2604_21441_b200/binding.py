@@ -1,0 +1,296 @@
+"""ctypes binding of include/nnp.h -- argument marshalling only (same names as the C entry points).
+
+Low level: nnp_* functions take/return raw pointers (ints) exactly like the C-ABI.
+Convenience: Model / Workspace own the opaque handles; Workspace.eval takes torch CUDA tensors (device memory
+and streams are torch's; nothing else of torch is used) and Workspace.eval_host takes numpy arrays.
+"""
+import ctypes as C
+import os
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
+
+NNP_OK = 0
+NNP_MLP_FP32_SIMT, NNP_MLP_BF16X3, NNP_MLP_BF16X1 = 0, 1, 2
+
+EXPORTS = [
+    "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
+    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
+    "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev",
+    "nnp_debug_atomic_energies", "nnp_debug_counters",
+]
+
+
+class NNPError(RuntimeError):
+    def __init__(self, code, where=""):
+        self.code = code
+        super().__init__(f"{where}: nnp error {code}: {nnp_strerror(code)}")
+
+
+class _AevParams(C.Structure):
+    _fields_ = [("Rcr", C.c_double), ("Rca", C.c_double), ("EtaR", C.c_double), ("EtaA", C.c_double),
+                ("Zeta", C.c_double), ("nShfR", C.c_int32), ("nShfA", C.c_int32), ("nShfZ", C.c_int32),
+                ("ShfR", C.POINTER(C.c_double)), ("ShfA", C.POINTER(C.c_double)), ("ShfZ", C.POINTER(C.c_double)),
+                ("radial_prefactor", C.c_double), ("cos_scale", C.c_double), ("n_species", C.c_int32),
+                ("species_Z", C.POINTER(C.c_int32))]
+
+
+class _MlpDesc(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("dims", C.POINTER(C.c_int32)),
+                ("W", C.POINTER(C.POINTER(C.c_float))), ("b", C.POINTER(C.POINTER(C.c_float))),
+                ("celu_alpha", C.c_double)]
+
+
+_lib = None
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def lib():
+    """Loads libnnp_b200.so (built in-tree by paper_2604_21441_b200/build.py).  No fallback of any kind."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2604_21441_b200.build` "
+                              "(there is no CPU or PyTorch fallback for the NNP path)")
+        L = C.CDLL(_LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.nnp_model_create.argtypes = [vp, vp, C.POINTER(vp)]
+        L.nnp_model_destroy.argtypes = [vp]
+        L.nnp_model_aev_length.argtypes = [vp]
+        L.nnp_workspace_create.argtypes = [vp, i64, i64, vp, C.POINTER(vp)]
+        L.nnp_workspace_destroy.argtypes = [vp]
+        L.nnp_workspace_set_mlp_mode.argtypes = [vp, i32]
+        L.nnp_workspace_set_dense_k.argtypes = [vp, i32]
+        L.nnp_eval.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
+        L.nnp_eval_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
+        L.nnp_status.argtypes = [vp]
+        L.nnp_strerror.argtypes = [C.c_int]
+        L.nnp_strerror.restype = C.c_char_p
+        L.nnp_debug_neighbors.argtypes = [vp, C.c_int, C.POINTER(i64), vp, vp, i64]
+        L.nnp_debug_aev.argtypes = [vp, vp]
+        L.nnp_debug_atomic_energies.argtypes = [vp, vp]
+        L.nnp_debug_counters.argtypes = [vp, C.POINTER(i64)]
+        _lib = L
+    return _lib
+
+
+# ---------------------------------------------------------------- low level: one function per C entry point
+def nnp_strerror(code):
+    return lib().nnp_strerror(int(code)).decode()
+
+
+def nnp_model_create(aev_struct, nets_array):
+    out = C.c_void_p()
+    rc = lib().nnp_model_create(C.addressof(aev_struct), C.addressof(nets_array), C.byref(out))
+    return rc, out.value
+
+
+def nnp_model_destroy(model):
+    return lib().nnp_model_destroy(model)
+
+
+def nnp_model_aev_length(model):
+    return lib().nnp_model_aev_length(model)
+
+
+def nnp_workspace_create(model, max_atoms, max_ml_atoms, cuda_stream):
+    out = C.c_void_p()
+    rc = lib().nnp_workspace_create(model, int(max_atoms), int(max_ml_atoms), cuda_stream, C.byref(out))
+    return rc, out.value
+
+
+def nnp_workspace_destroy(ws):
+    return lib().nnp_workspace_destroy(ws)
+
+
+def nnp_workspace_set_mlp_mode(ws, mode):
+    return lib().nnp_workspace_set_mlp_mode(ws, int(mode))
+
+
+def nnp_workspace_set_dense_k(ws, dense):
+    return lib().nnp_workspace_set_dense_k(ws, int(dense))
+
+
+def nnp_eval(ws, n_atoms, d_pos, d_Z, box_ptr, pbc, d_ml_index, n_ml, d_energy, d_forces):
+    return lib().nnp_eval(ws, int(n_atoms), d_pos, d_Z, box_ptr, int(pbc), d_ml_index, int(n_ml), d_energy, d_forces)
+
+
+def nnp_eval_host(ws, n_atoms, h_pos, h_Z, box_ptr, pbc, h_ml_index, n_ml, h_energy, h_forces):
+    return lib().nnp_eval_host(ws, int(n_atoms), h_pos, h_Z, box_ptr, int(pbc), h_ml_index, int(n_ml), h_energy,
+                               h_forces)
+
+
+def nnp_status(ws):
+    return lib().nnp_status(ws)
+
+
+def nnp_debug_neighbors(ws, which, h_row_start, h_col, col_cap):
+    n = C.c_int64(0)
+    rc = lib().nnp_debug_neighbors(ws, int(which), C.byref(n), h_row_start, h_col, int(col_cap))
+    return rc, n.value
+
+
+def nnp_debug_aev(ws, h_aev):
+    return lib().nnp_debug_aev(ws, h_aev)
+
+
+def nnp_debug_atomic_energies(ws, h_e):
+    return lib().nnp_debug_atomic_energies(ws, h_e)
+
+
+def nnp_debug_counters(ws):
+    n = C.c_int64(0)
+    rc = lib().nnp_debug_counters(ws, C.byref(n))
+    return rc, n.value
+
+
+# ---------------------------------------------------------------- convenience owners
+def _check(rc, where):
+    if rc != NNP_OK:
+        raise NNPError(rc, where)
+
+
+class Model:
+    """aev: dict with Rcr, Rca, EtaR, EtaA, Zeta, ShfR, ShfA, ShfZ, radial_prefactor, cos_scale, species_Z;
+    nets: {Z: (dims, [W_l], [b_l])}; species without an entry have no network."""
+
+    def __init__(self, aev, nets, celu_alpha=0.1):
+        keep = []
+        k = lambda a: (keep.append(a), a)[1]
+        dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        ShfR = k(np.ascontiguousarray(aev["ShfR"], dtype=np.float64))
+        ShfA = k(np.ascontiguousarray(aev["ShfA"], dtype=np.float64))
+        ShfZ = k(np.ascontiguousarray(aev["ShfZ"], dtype=np.float64))
+        sZ = k(np.ascontiguousarray(aev["species_Z"], dtype=np.int32))
+        S = len(sZ)
+        p = _AevParams(aev["Rcr"], aev["Rca"], aev["EtaR"], aev["EtaA"], aev["Zeta"], len(ShfR), len(ShfA),
+                       len(ShfZ), dp(ShfR), dp(ShfA), dp(ShfZ), aev["radial_prefactor"], aev["cos_scale"], S,
+                       sZ.ctypes.data_as(C.POINTER(C.c_int32)))
+        arr = (_MlpDesc * S)()
+        for s, Z in enumerate(sZ):
+            if int(Z) not in nets:
+                arr[s] = _MlpDesc(0, None, None, None, celu_alpha)
+                continue
+            dims, W, b = nets[int(Z)]
+            d = k(np.ascontiguousarray(dims, dtype=np.int32))
+            nl = len(d) - 1
+            Wp = k((C.POINTER(C.c_float) * nl)())
+            bp = k((C.POINTER(C.c_float) * nl)())
+            for l in range(nl):
+                w = k(np.ascontiguousarray(W[l], dtype=np.float32))
+                bb = k(np.ascontiguousarray(b[l], dtype=np.float32))
+                if w.shape != (d[l + 1], d[l]) or bb.shape != (d[l + 1],):
+                    raise ValueError("weight/bias shape mismatch")
+                Wp[l] = w.ctypes.data_as(C.POINTER(C.c_float))
+                bp[l] = bb.ctypes.data_as(C.POINTER(C.c_float))
+            arr[s] = _MlpDesc(nl, d.ctypes.data_as(C.POINTER(C.c_int32)), Wp, bp, celu_alpha)
+        rc, h = nnp_model_create(p, arr)
+        _check(rc, "nnp_model_create")
+        self.handle = h
+        self.aev_length = nnp_model_aev_length(h)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            nnp_model_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        self.close()
+
+
+class Workspace:
+    def __init__(self, model, max_atoms, max_ml_atoms=None, stream=None):
+        import torch
+        self.model = model
+        self.max_atoms = int(max_atoms)
+        self.max_ml = int(max_atoms if max_ml_atoms is None else max_ml_atoms)
+        self.stream = torch.cuda.current_stream() if stream is None else stream
+        rc, h = nnp_workspace_create(model.handle, self.max_atoms, self.max_ml, self.stream.cuda_stream)
+        _check(rc, "nnp_workspace_create")
+        self.handle = h
+
+    def set_mlp_mode(self, mode):
+        _check(nnp_workspace_set_mlp_mode(self.handle, mode), "nnp_workspace_set_mlp_mode")
+
+    def set_dense_k(self, dense):
+        _check(nnp_workspace_set_dense_k(self.handle, dense), "nnp_workspace_set_dense_k")
+
+    def eval(self, pos, Z, box, pbc=1, ml_index=None, energy=None, forces=None, check=False):
+        """pos (N,3) float32 cuda, Z (N,) int32 cuda, box: 9 floats on the HOST, ml_index (n_ml,) int32 cuda
+        or None.  Asynchronous on the workspace stream; returns (energy (1,) float64 cuda, forces (N,3))."""
+        import torch
+        n = pos.shape[0]
+        assert pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous()
+        assert Z.is_cuda and Z.dtype == torch.int32 and Z.is_contiguous()
+        if energy is None:
+            energy = torch.empty(1, dtype=torch.float64, device=pos.device)
+        if forces is None:
+            forces = torch.empty((n, 3), dtype=torch.float32, device=pos.device)
+        b = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+        ml_ptr, n_ml = None, n
+        if ml_index is not None:
+            assert ml_index.is_cuda and ml_index.dtype == torch.int32 and ml_index.is_contiguous()
+            ml_ptr, n_ml = ml_index.data_ptr(), ml_index.shape[0]
+        rc = nnp_eval(self.handle, n, pos.data_ptr(), Z.data_ptr(), b.ctypes.data, pbc, ml_ptr, n_ml,
+                      energy.data_ptr(), forces.data_ptr())
+        _check(rc, "nnp_eval")
+        self._last = (pos, Z, ml_index)  # keep the device buffers of the last evaluation alive for debug exports
+        if check:
+            _check(nnp_status(self.handle), "nnp_status")
+        return energy, forces
+
+    def eval_host(self, pos, Z, box, pbc=1, ml_index=None, forces_out=None):
+        """numpy in / numpy out through nnp_eval_host (copies + synchronisation inside the library)."""
+        pos = np.ascontiguousarray(pos, dtype=np.float32)
+        Z = np.ascontiguousarray(Z, dtype=np.int32)
+        b = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+        n = pos.shape[0]
+        ml = None if ml_index is None else np.ascontiguousarray(ml_index, dtype=np.int32)
+        E = np.zeros(1, dtype=np.float64)
+        F = np.empty((n, 3), dtype=np.float32) if forces_out is None else forces_out
+        rc = nnp_eval_host(self.handle, n, pos.ctypes.data, Z.ctypes.data, b.ctypes.data, pbc,
+                           None if ml is None else ml.ctypes.data, 0 if ml is None else len(ml), E.ctypes.data,
+                           F.ctypes.data)
+        _check(rc, "nnp_eval_host")
+        self._last = None
+        self._n_ml = n if ml is None else len(ml)
+        return float(E[0]), F
+
+    def status(self):
+        return nnp_status(self.handle)
+
+    def neighbors(self, which, n_ml):
+        start = np.zeros(n_ml + 1, dtype=np.int32)
+        rc, n = nnp_debug_neighbors(self.handle, which, None, None, 0)
+        _check(rc, "nnp_debug_neighbors")
+        col = np.zeros(max(n, 1), dtype=np.int32)
+        rc, n = nnp_debug_neighbors(self.handle, which, start.ctypes.data, col.ctypes.data, len(col))
+        _check(rc, "nnp_debug_neighbors")
+        return start, col[:n]
+
+    def aev(self, n_ml):
+        a = np.zeros((n_ml, self.model.aev_length), dtype=np.float32)
+        _check(nnp_debug_aev(self.handle, a.ctypes.data), "nnp_debug_aev")
+        return a
+
+    def atomic_energies(self, n_ml):
+        e = np.zeros(n_ml, dtype=np.float32)
+        _check(nnp_debug_atomic_energies(self.handle, e.ctypes.data), "nnp_debug_atomic_energies")
+        return e
+
+    def launches(self):
+        rc, n = nnp_debug_counters(self.handle)
+        _check(rc, "nnp_debug_counters")
+        return n
+
+    def close(self):
+        if getattr(self, "handle", None):
+            nnp_workspace_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        self.close()

@@ -1,0 +1,378 @@
+// api.cu -- the C-ABI boundary of include/nnp.h: model / workspace lifetime, nnp_eval (K0-K8 on one stream, no
+// host synchronisation, no allocation), the host-buffer entry point, status and the debug exports.
+// Interface: PAPER.md line 77 (inputs), lines 49-51 and 86 (outputs); SURVEY.md section 8.b.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <algorithm>
+#include <new>
+#include <vector>
+#include "nnp_internal.h"
+
+using namespace nnp;
+
+#define CU_OK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return NNP_ERR_CUDA; } } while (0)
+
+extern "C" const char* nnp_strerror(int code) {
+  switch (code) {
+    case NNP_OK: return "ok";
+    case NNP_ERR_INVALID_ARG: return "invalid argument";
+    case NNP_ERR_UNKNOWN_SPECIES: return "ML atom with an atomic number that has no species slot or no network";
+    case NNP_ERR_BOX_UNSUPPORTED: return "box must be orthorhombic with positive lengths";
+    case NNP_ERR_CAPACITY: return "neighbour row or tile capacity exceeded";
+    case NNP_ERR_COINCIDENT: return "two ML atoms coincide";
+    case NNP_ERR_CUDA: return "CUDA error or no CUDA device";
+    case NNP_ERR_UNSUPPORTED: return "descriptor or network shape outside the kernels' range";
+    default: return "unknown error";
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ model
+extern "C" int nnp_model_create(const nnp_aev_params* p, const nnp_mlp_desc* nets, nnp_model** out) {
+  if (!p || !nets || !out) return NNP_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (p->n_species < 1 || !p->species_Z || !p->ShfR || !p->ShfA || !p->ShfZ) return NNP_ERR_INVALID_ARG;
+  if (!(p->Rcr > 0) || !(p->Rca > 0) || p->Rca > p->Rcr) return NNP_ERR_INVALID_ARG;
+  if (p->n_species > MAX_S || p->nShfR != NSHFR || p->nShfA != NSHFA || p->nShfZ != NSHFZ) return NNP_ERR_UNSUPPORTED;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return NNP_ERR_CUDA; }
+  const int S = p->n_species;
+  const int L = S * NSHFR + S * (S + 1) / 2 * NSHFA * NSHFZ;
+  nnp_model* m = new (std::nothrow) nnp_model();
+  if (!m) return NNP_ERR_CUDA;
+  memset(m, 0, sizeof(*m));
+  AevConst& c = m->aev;
+  c.Rcr = (float)p->Rcr; c.Rca = (float)p->Rca;
+  c.Rcr2_d = p->Rcr * p->Rcr; c.Rca2_d = p->Rca * p->Rca;
+  c.Rcr2 = (float)c.Rcr2_d; c.Rca2 = (float)c.Rca2_d;
+  c.etaR = (float)p->EtaR; c.etaA = (float)p->EtaA;
+  c.etaR_l2e = (float)(p->EtaR * 1.4426950408889634); c.etaA_l2e = (float)(p->EtaA * 1.4426950408889634);
+  c.cR = (float)p->radial_prefactor; c.cTheta = (float)p->cos_scale; c.zeta = (float)p->Zeta;
+  c.zeta_is_32 = (p->Zeta == 32.0);
+  c.inv_Rcr = (float)(1.0 / p->Rcr); c.inv_Rca = (float)(1.0 / p->Rca);
+  c.S = S; c.nRB = (S + 1) / 2; c.nblk_full = c.nRB + S * (S + 1) / 2; c.L = L;
+  for (int i = 0; i < NSHFR; ++i) c.ShfR[i] = (float)p->ShfR[i];
+  for (int i = 0; i < NSHFA; ++i) c.ShfA[i] = (float)p->ShfA[i];
+  for (int i = 0; i < NSHFZ; ++i) { c.cosZ[i] = (float)cos(p->ShfZ[i]); c.sinZ[i] = (float)sin(p->ShfZ[i]); }
+  for (int z = 0; z < 128; ++z) c.zlut[z] = -1;
+  m->Kfull = c.nblk_full * BLK;
+
+  // networks: validate, then pack all fp32 weights into one blob (layer 0 permuted to the internal column order)
+  int nl_common = 0;
+  size_t total = 0;
+  for (int s = 0; s < S; ++s) {
+    const nnp_mlp_desc& d = nets[s];
+    if (d.n_layers == 0) continue;
+    bool ok = d.n_layers >= 1 && d.n_layers <= MAX_LAYERS && d.dims && d.W && d.b && d.dims[d.n_layers] == 1;
+    if (!ok) { delete m; return NNP_ERR_INVALID_ARG; }
+    if (d.dims[0] != L) { delete m; return NNP_ERR_INVALID_ARG; }
+    for (int l = 1; l < d.n_layers; ++l)
+      if (d.dims[l] < 16 || d.dims[l] > HP || d.dims[l] % 16) { delete m; return NNP_ERR_UNSUPPORTED; }
+    if (nl_common == 0) nl_common = d.n_layers;
+    if (d.n_layers != nl_common) { delete m; return NNP_ERR_UNSUPPORTED; }
+    const int z = p->species_Z[s];
+    if (z < 0 || z >= 128) { delete m; return NNP_ERR_INVALID_ARG; }
+    c.zlut[z] = (int8_t)s;
+    for (int l = 0; l < d.n_layers; ++l) {
+      const size_t in = (l == 0) ? (size_t)m->Kfull : (size_t)d.dims[l];
+      total += in * d.dims[l + 1] + (size_t)d.dims[l + 1];
+      total = (total + 3) & ~(size_t)3;
+    }
+  }
+  if (nl_common == 0) { delete m; return NNP_ERR_INVALID_ARG; }
+  m->n_layers = nl_common;
+  std::vector<float> blob(total, 0.f);
+  float* dbase = nullptr;
+  if (cudaMalloc(&dbase, std::max<size_t>(total, 4) * sizeof(float)) != cudaSuccess) { cudaGetLastError(); delete m; return NNP_ERR_CUDA; }
+  size_t off = 0;
+  for (int s = 0; s < S; ++s) {
+    const nnp_mlp_desc& d = nets[s];
+    Net& n = m->nets.net[s];
+    n.n_layers = d.n_layers;
+    if (d.n_layers == 0) continue;
+    n.alpha = (float)d.celu_alpha;
+    for (int l = 0; l <= d.n_layers; ++l) n.dims[l] = d.dims[l];
+    n.dims[0] = m->Kfull;  // device-side input width = internal padded column count
+    for (int l = 0; l < d.n_layers; ++l) {
+      const int in = d.dims[l], outw = d.dims[l + 1];
+      const size_t ldw = (l == 0) ? (size_t)m->Kfull : (size_t)in;
+      n.W[l] = dbase + off;
+      for (int o = 0; o < outw; ++o)
+        for (int i = 0; i < in; ++i) {
+          size_t col = (size_t)i;
+          if (l == 0 && i >= S * NSHFR) col = (size_t)c.nRB * BLK + (size_t)(i - S * NSHFR);
+          blob[off + (size_t)o * ldw + col] = d.W[l][(size_t)o * in + i];
+        }
+      off += ldw * outw;
+      n.b[l] = dbase + off;
+      for (int o = 0; o < outw; ++o) blob[off + o] = d.b[l][o];
+      off += outw;
+      off = (off + 3) & ~(size_t)3;
+      n.WT[l] = nullptr;
+    }
+  }
+  if (cudaMemcpy(dbase, blob.data(), total * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError(); cudaFree(dbase); delete m; return NNP_ERR_CUDA;
+  }
+  m->dev_blob = dbase; m->blob_bytes = total * sizeof(float);
+  m->tc = nullptr;
+  int rc = tc_model_create(m, nets);
+  if (rc != NNP_OK) { cudaFree(dbase); delete m; return rc; }
+  *out = m;
+  return NNP_OK;
+}
+
+extern "C" int nnp_model_destroy(nnp_model* m) {
+  if (!m) return NNP_OK;
+  tc_model_destroy(m);
+  if (m->dev_blob) cudaFree(m->dev_blob);
+  delete m;
+  return NNP_OK;
+}
+
+extern "C" int nnp_model_aev_length(const nnp_model* m) { return m ? m->aev.L : NNP_ERR_INVALID_ARG; }
+
+// ------------------------------------------------------------------------------------------------ workspace
+template <class T>
+static bool dmalloc(T** p, size_t n) {
+  *p = nullptr;
+  if (cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return false; }
+  return cudaMemset(*p, 0, std::max<size_t>(n, 1) * sizeof(T)) == cudaSuccess;
+}
+
+extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
+  if (!ws) return NNP_OK;
+  cudaStreamSynchronize(ws->stream);
+  tc_workspace_destroy(ws);
+  void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
+                  ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
+                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->hd_pos, ws->hd_Z, ws->hd_ml,
+                  ws->hd_energy, ws->hd_forces};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  cudaGetLastError();
+  delete ws;
+  return NNP_OK;
+}
+
+extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64_t max_ml, void* stream,
+                                    nnp_workspace** out) {
+  if (!m || !out || max_atoms < 0 || max_ml < 0 || max_ml > max_atoms) return NNP_ERR_INVALID_ARG;
+  if (max_ml >= (1ll << JBITS)) return NNP_ERR_UNSUPPORTED;
+  *out = nullptr;
+  nnp_workspace* ws = new (std::nothrow) nnp_workspace();
+  if (!ws) return NNP_ERR_CUDA;
+  memset(ws, 0, sizeof(*ws));
+  ws->model = m; ws->stream = (cudaStream_t)stream; ws->max_atoms = max_atoms; ws->max_ml = max_ml;
+  ws->rcap = RCAP_MAX; ws->acap = ACAP_MAX;
+  ws->max_cells = (int)std::min<int64_t>(std::max<int64_t>(512, max_ml / 4), 1 << 21);
+  ws->mlp_mode = m->tc ? NNP_MLP_BF16X3 : NNP_MLP_FP32_SIMT;
+  ws->dense_k = 0;
+  ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
+  ws->max_rows = (int64_t)ws->max_tiles * TILE_M;
+  const size_t nm = (size_t)max_ml, nr = (size_t)ws->max_rows, K = (size_t)m->Kfull;
+  bool ok = dmalloc(&ws->grid, 1) && dmalloc(&ws->groups, 1) && dmalloc(&ws->tiles, (size_t)ws->max_tiles) &&
+            dmalloc(&ws->flags, 1) && dmalloc(&ws->cell_count, (size_t)MAX_S * ws->max_cells + 1) &&
+            dmalloc(&ws->bstart, (size_t)MAX_S * ws->max_cells + 1) && dmalloc(&ws->tmp4, nm) &&
+            dmalloc(&ws->rank, nm) && dmalloc(&ws->spos, nm) && dmalloc(&ws->scell, nm) &&
+            dmalloc(&ws->nbrR, nm * ws->rcap) && dmalloc(&ws->nbrA, nm * ws->acap) && dmalloc(&ws->cntR, nm) &&
+            dmalloc(&ws->cntA, nm) && dmalloc(&ws->aev, nr * K) && dmalloc(&ws->daev, nr * K) &&
+            dmalloc(&ws->hbuf[0], nr * HP) && dmalloc(&ws->hbuf[1], nr * HP) && dmalloc(&ws->hbuf[2], nr * HP) &&
+            dmalloc(&ws->dbuf[0], nr * HP) && dmalloc(&ws->dbuf[1], nr * HP) && dmalloc(&ws->e_atom, nr) &&
+            dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
+            dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) && dmalloc(&ws->hd_energy, 1) &&
+            dmalloc(&ws->hd_forces, 3 * (size_t)max_atoms);
+  if (ok) ok = (tc_workspace_create(ws) == NNP_OK);
+  if (!ok || cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); nnp_workspace_destroy(ws); return NNP_ERR_CUDA; }
+  *out = ws;
+  return NNP_OK;
+}
+
+extern "C" int nnp_workspace_set_mlp_mode(nnp_workspace* ws, int32_t mode) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  if (mode == NNP_MLP_FP32_SIMT) { ws->mlp_mode = mode; return NNP_OK; }
+  if (mode == NNP_MLP_BF16X3 || mode == NNP_MLP_BF16X1) {
+    if (!ws->model->tc) return NNP_ERR_UNSUPPORTED;
+    ws->mlp_mode = mode;
+    return NNP_OK;
+  }
+  return NNP_ERR_INVALID_ARG;
+}
+
+extern "C" int nnp_workspace_set_dense_k(nnp_workspace* ws, int32_t dense) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  ws->dense_k = dense ? 1 : 0;
+  return NNP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ evaluation
+static int check_box(const float* box, int pbc) {
+  if (!pbc) return NNP_OK;
+  if (!box) return NNP_ERR_INVALID_ARG;
+  for (int r = 0; r < 3; ++r)
+    for (int c = 0; c < 3; ++c) {
+      const float v = box[3 * r + c];
+      if (r == c) { if (!(v > 0.f) || !isfinite(v)) return NNP_ERR_BOX_UNSUPPORTED; }
+      else if (v != 0.f) return NNP_ERR_BOX_UNSUPPORTED;
+    }
+  return NNP_OK;
+}
+
+extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, const int32_t* d_Z, const float box[9],
+                        int32_t pbc, const int32_t* d_ml, int64_t n_ml, double* d_energy, float* d_forces) {
+  if (!ws || n_atoms < 0 || !d_energy || (n_atoms > 0 && (!d_pos || !d_Z || !d_forces))) return NNP_ERR_INVALID_ARG;
+  if (!d_ml) n_ml = n_atoms;
+  if (n_ml < 0 || n_ml > n_atoms || n_atoms > ws->max_atoms || n_ml > ws->max_ml) return NNP_ERR_INVALID_ARG;
+  int rc = check_box(box, pbc);
+  if (rc) return rc;
+  const float unit[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+  ws->n_atoms = n_atoms; ws->n_ml = n_ml; ws->d_ml_index = d_ml;
+  int nl = launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
+  nl += launch_aev_forward(ws, n_ml);
+  nl += (ws->mlp_mode == NNP_MLP_FP32_SIMT) ? launch_mlp_simt(ws, n_ml) : launch_mlp_tc(ws, n_ml);
+  nl += launch_force_stage(ws, n_atoms, n_ml, d_ml, d_energy, d_forces);
+  ws->launches = nl;
+  if (cudaGetLastError() != cudaSuccess) return NNP_ERR_CUDA;
+  return NNP_OK;
+}
+
+extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_pos, const int32_t* h_Z,
+                             const float box[9], int32_t pbc, const int32_t* h_ml, int64_t n_ml, double* h_energy,
+                             float* h_forces) {
+  if (!ws || n_atoms < 0 || n_atoms > ws->max_atoms || !h_energy || (n_atoms > 0 && (!h_pos || !h_Z || !h_forces)))
+    return NNP_ERR_INVALID_ARG;
+  if (h_ml && (n_ml < 0 || n_ml > ws->max_ml)) return NNP_ERR_INVALID_ARG;
+  cudaStream_t st = ws->stream;
+  CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
+  CU_OK(cudaMemcpyAsync(ws->hd_Z, h_Z, sizeof(int32_t) * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
+  if (h_ml) CU_OK(cudaMemcpyAsync(ws->hd_ml, h_ml, sizeof(int32_t) * (size_t)n_ml, cudaMemcpyHostToDevice, st));
+  int rc = nnp_eval(ws, n_atoms, ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml, ws->hd_energy,
+                    ws->hd_forces);
+  if (rc) return rc;
+  CU_OK(cudaMemcpyAsync(h_energy, ws->hd_energy, sizeof(double), cudaMemcpyDeviceToHost, st));
+  CU_OK(cudaMemcpyAsync(h_forces, ws->hd_forces, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyDeviceToHost, st));
+  CU_OK(cudaStreamSynchronize(st));
+  return NNP_OK;
+}
+
+extern "C" int nnp_status(nnp_workspace* ws) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  if (cudaStreamSynchronize(ws->stream) != cudaSuccess) { cudaGetLastError(); return NNP_ERR_CUDA; }
+  int f = 0;
+  CU_OK(cudaMemcpy(&f, ws->flags, sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemset(ws->flags, 0, sizeof(int)));
+  if (f & FLAG_ARG) return NNP_ERR_INVALID_ARG;
+  if (f & FLAG_SPECIES) return NNP_ERR_UNKNOWN_SPECIES;
+  if (f & FLAG_CAP) return NNP_ERR_CAPACITY;
+  if (f & FLAG_COINCIDENT) return NNP_ERR_COINCIDENT;
+  return NNP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ debug exports
+namespace {
+struct Snapshot {
+  std::vector<float4> spos;
+  std::vector<int32_t> ml;
+  GroupInfo grp;
+};
+int take_snapshot(nnp_workspace* ws, Snapshot& s) {
+  if (cudaStreamSynchronize(ws->stream) != cudaSuccess) { cudaGetLastError(); return NNP_ERR_CUDA; }
+  const size_t n = (size_t)ws->n_ml;
+  s.spos.resize(n);
+  if (n) CU_OK(cudaMemcpy(s.spos.data(), ws->spos, n * sizeof(float4), cudaMemcpyDeviceToHost));
+  s.ml.clear();
+  if (ws->d_ml_index && n) {
+    s.ml.resize(n);
+    CU_OK(cudaMemcpy(s.ml.data(), ws->d_ml_index, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  }
+  CU_OK(cudaMemcpy(&s.grp, ws->groups, sizeof(GroupInfo), cudaMemcpyDeviceToHost));
+  return NNP_OK;
+}
+inline int ml_local(const float4& v) { int w; memcpy(&w, &v.w, 4); return w & 0x0fffffff; }
+inline int slot_of(const float4& v) { int w; memcpy(&w, &v.w, 4); return (w >> 28) & 7; }
+}  // namespace
+
+extern "C" int nnp_debug_neighbors(nnp_workspace* ws, int which, int64_t* n_pairs, int32_t* h_row_start,
+                                   int32_t* h_col, int64_t col_cap) {
+  if (!ws || !n_pairs || (which != 0 && which != 1)) return NNP_ERR_INVALID_ARG;
+  Snapshot s;
+  int rc = take_snapshot(ws, s);
+  if (rc) return rc;
+  const size_t n = (size_t)ws->n_ml;
+  std::vector<int> cntR(n), cntA(n);
+  std::vector<uint32_t> nbrR(n * ws->rcap);
+  std::vector<uint8_t> nbrA(n * ws->acap);
+  if (n) {
+    CU_OK(cudaMemcpy(cntR.data(), ws->cntR, n * sizeof(int), cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(cntA.data(), ws->cntA, n * sizeof(int), cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(nbrR.data(), ws->nbrR, nbrR.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    CU_OK(cudaMemcpy(nbrA.data(), ws->nbrA, nbrA.size(), cudaMemcpyDeviceToHost));
+  }
+  std::vector<int> sorted_of(n);  // ml-local index -> sorted position
+  for (size_t ip = 0; ip < n; ++ip) sorted_of[ml_local(s.spos[ip])] = (int)ip;
+  int64_t tot = 0;
+  for (size_t a = 0; a < n; ++a) tot += which ? cntA[sorted_of[a]] : cntR[sorted_of[a]];
+  *n_pairs = tot;
+  if (!h_col || !h_row_start || col_cap < tot) return NNP_OK;
+  int64_t pos = 0;
+  for (size_t a = 0; a < n; ++a) {
+    const int ip = sorted_of[a];
+    h_row_start[a] = (int32_t)pos;
+    const int cnt = which ? cntA[ip] : cntR[ip];
+    for (int q = 0; q < cnt; ++q) {
+      const int pr = which ? nbrA[(size_t)ip * ws->acap + q] : q;
+      const int jp = (int)(nbrR[(size_t)ip * ws->rcap + pr] & JMASK);
+      const int aj = ml_local(s.spos[jp]);
+      h_col[pos + q] = s.ml.empty() ? aj : s.ml[aj];
+    }
+    std::sort(h_col + pos, h_col + pos + cnt);
+    pos += cnt;
+  }
+  h_row_start[n] = (int32_t)pos;
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_aev(nnp_workspace* ws, float* h_aev) {
+  if (!ws || !h_aev) return NNP_ERR_INVALID_ARG;
+  Snapshot s;
+  int rc = take_snapshot(ws, s);
+  if (rc) return rc;
+  const AevConst& c = ws->model->aev;
+  const size_t n = (size_t)ws->n_ml, Kc = (size_t)s.grp.Kc;
+  std::vector<float> buf((size_t)s.grp.n_rows * Kc);
+  if (!buf.empty()) CU_OK(cudaMemcpy(buf.data(), ws->aev, buf.size() * sizeof(float), cudaMemcpyDeviceToHost));
+  memset(h_aev, 0, n * (size_t)c.L * sizeof(float));
+  for (size_t ip = 0; ip < n; ++ip) {
+    const int a = ml_local(s.spos[ip]), sl = slot_of(s.spos[ip]);
+    const float* row = buf.data() + (ip + s.grp.pad_shift[sl]) * Kc;
+    float* dst = h_aev + (size_t)a * c.L;
+    for (int b = 0; b < s.grp.nblk; ++b) {
+      const int ib = s.grp.blkmap[b];
+      for (int q = 0; q < BLK; ++q) {
+        const int icol = ib * BLK + q;  // internal column -> public column
+        int pub;
+        if (ib < c.nRB) { if (icol >= c.S * NSHFR) continue; pub = icol; }
+        else pub = c.S * NSHFR + (icol - c.nRB * BLK);
+        dst[pub] = row[(size_t)b * BLK + q];
+      }
+    }
+  }
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_atomic_energies(nnp_workspace* ws, float* h_e) {
+  if (!ws || !h_e) return NNP_ERR_INVALID_ARG;
+  Snapshot s;
+  int rc = take_snapshot(ws, s);
+  if (rc) return rc;
+  std::vector<float> buf((size_t)s.grp.n_rows);
+  if (!buf.empty()) CU_OK(cudaMemcpy(buf.data(), ws->e_atom, buf.size() * sizeof(float), cudaMemcpyDeviceToHost));
+  for (size_t ip = 0; ip < (size_t)ws->n_ml; ++ip)
+    h_e[ml_local(s.spos[ip])] = buf[ip + s.grp.pad_shift[slot_of(s.spos[ip])]];
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_counters(nnp_workspace* ws, int64_t* launches) {
+  if (!ws || !launches) return NNP_ERR_INVALID_ARG;
+  launches[0] = ws->launches;
+  return NNP_OK;
+}

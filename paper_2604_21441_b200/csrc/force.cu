@@ -1,0 +1,202 @@
+// force.cu -- K7 + K8 of SURVEY.md section 8.a: chain rule dE/dAEV -> pair partials p_ij = dE_i/dr_j, and the
+// deterministic force assembly F_a = sum_j (p_aj - p_ja)  (eq. 2 F = -grad E;
+// BASELINE.json north_star stage (4); formulas SURVEY.md Appendix A "Forces").
+//
+// K7: one warp per centre.  Radial: lane <-> neighbour.  Angular: lane <-> neighbour j (P = 1, 2 or 4 lanes
+// per j share the partner loop), each lane accumulating ONLY its own p_ij over all partners k, so no
+// cross-lane scatter is needed; every unordered triplet is therefore visited from both ends.
+// K8: p_ij is converted to 2^-40 fixed point and accumulated with 64-bit integer atomics (integer addition
+// is associative, so the result does not depend on the arrival order): forces are bitwise reproducible.
+#include "aev_common.cuh"
+
+namespace nnp {
+
+__device__ __forceinline__ long long to_fix(float v) { return __float2ll_rn(v * 1099511627776.0f); }  // 2^40
+__device__ __forceinline__ long long shfl_xor_ll(long long v, int o) {
+  int lo = __shfl_xor_sync(0xffffffffu, (int)(v & 0xffffffffll), o);
+  int hi = __shfl_xor_sync(0xffffffffu, (int)(v >> 32), o);
+  return ((long long)hi << 32) | (unsigned int)lo;
+}
+
+__global__ void __launch_bounds__(AEV_WARPS * 32)
+k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
+               const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
+               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
+               const float* __restrict__ daev, unsigned long long* __restrict__ facc) {
+  __shared__ WarpEnv env[AEV_WARPS];
+  __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int ip = blockIdx.x * AEV_WARPS + w;
+  if (ip >= n_ml) return;
+  WarpEnv& e = env[w];
+  const float4 ci = spos[ip];
+  const int si = (__float_as_int(ci.w) >> 28) & 7;
+  const int nR = cntR[ip], nA = cntA[ip];
+  const uint32_t* __restrict__ rowR = nbrR + (size_t)ip * rcap;
+  load_env(c, g, spos, rowR, nbrA + (size_t)ip * acap, nR, nA, ci, lane, e);
+  const int Kc = grp->Kc;
+  const float* __restrict__ gi = daev + (size_t)(ip + grp->pad_shift[si]) * Kc;
+
+  // ---- angular: p_ij for the angular neighbours, staged in Pacc
+  const int P = (nA <= 8) ? 4 : (nA <= 16) ? 2 : 1;   // lanes per neighbour
+  const int JW = 32 / P;                               // neighbours per pass
+  const int h = lane % P;
+  for (int j0 = 0; j0 < nA; j0 += JW) {
+    const int j = j0 + lane / P;
+    float px = 0.f, py = 0.f, pz = 0.f;
+    if (j < nA) {
+      const float4 uj = e.ua[j];
+      const float fj = e.fA[j], dfj = e.dfA[j];
+      const int sj = e.slotA[j];
+      for (int k = h; k < nA; k += P) {
+        if (k == j) continue;
+        const float4 uk = e.ua[k];
+        const float fk = e.fA[k];
+        const int sk = e.slotA[k];
+        const int s1 = min(sj, sk), s2 = max(sj, sk);
+        const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
+        const float4* __restrict__ gb = reinterpret_cast<const float4*>(gi + grp->cpos[c.nRB + pidx] * BLK);
+        const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
+        const float cc = c.cTheta * u;
+        const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
+        const float dth_du = -c.cTheta / ss;
+        float F1[NSHFZ], dF1[NSHFZ];
+#pragma unroll
+        for (int z = 0; z < NSHFZ; ++z) {
+          const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
+          const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
+          const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 0.f);
+          float Bz, Bm;
+          bpow(c, B, Bz, Bm);
+          F1[z] = Bz;
+          dF1[z] = (-0.5f * c.zeta * dth_du) * Bm * sind;   // dF1/du
+        }
+        const float Rbar = 0.5f * (uj.w + uk.w);
+        float sW = 0.f, sV = 0.f;
+#pragma unroll
+        for (int a = 0; a < NSHFA; ++a) {
+          const float4 g0 = gb[2 * a], g1 = gb[2 * a + 1];
+          float W = g0.x * F1[0], V = g0.x * dF1[0];
+          W = fmaf(g0.y, F1[1], W); V = fmaf(g0.y, dF1[1], V);
+          W = fmaf(g0.z, F1[2], W); V = fmaf(g0.z, dF1[2], V);
+          W = fmaf(g0.w, F1[3], W); V = fmaf(g0.w, dF1[3], V);
+          W = fmaf(g1.x, F1[4], W); V = fmaf(g1.x, dF1[4], V);
+          W = fmaf(g1.y, F1[5], W); V = fmaf(g1.y, dF1[5], V);
+          W = fmaf(g1.z, F1[6], W); V = fmaf(g1.z, dF1[6], V);
+          W = fmaf(g1.w, F1[7], W); V = fmaf(g1.w, dF1[7], V);
+          const float x = Rbar - c.ShfA[a];
+          const float F2 = ex2f(-c.etaA_l2e * x * x);
+          sW = fmaf(W * F2, fmaf(-c.etaA * x, fj, dfj), sW);   // dt/dR_ij / (2 F1 fk)
+          sV = fmaf(V, F2, sV);
+        }
+        const float Aj = 2.0f * fk * sW;
+        const float Au = 2.0f * fj * fk * sV;
+        const float q = Au / uj.w;
+        const float r = Aj - q * u;
+        px = fmaf(r, uj.x, fmaf(q, uk.x, px));
+        py = fmaf(r, uj.y, fmaf(q, uk.y, py));
+        pz = fmaf(r, uj.z, fmaf(q, uk.z, pz));
+      }
+    }
+    for (int o = 1; o < P; o <<= 1) {
+      px += __shfl_xor_sync(0xffffffffu, px, o);
+      py += __shfl_xor_sync(0xffffffffu, py, o);
+      pz += __shfl_xor_sync(0xffffffffu, pz, o);
+    }
+    if (j < nA && h == 0) { Pacc[w][j][0] = px; Pacc[w][j][1] = py; Pacc[w][j][2] = pz; }
+  }
+  __syncwarp();
+
+  // ---- radial + assembly: lane <-> radial neighbour
+  long long ox = 0, oy = 0, oz = 0;   // sum_j p_ij in fixed point
+  for (int q0 = 0; q0 < nR; q0 += 32) {
+    const int q = q0 + lane;
+    if (q < nR) {
+      const float4 uq = e.u[q];
+      const int s = e.slotR[q];
+      const float4* __restrict__ gr = reinterpret_cast<const float4*>(gi + grp->cpos[s >> 1] * BLK + (s & 1) * 16);
+      const float f = e.wR[q];   // c_R f_C
+      float fc, dfc;
+      cutoff(fminf(uq.w, c.Rcr), c.inv_Rcr, fc, dfc);
+      const float df = c.cR * dfc;
+      float coef = 0.f;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float4 gv = gr[v];
+        const float gg[4] = {gv.x, gv.y, gv.z, gv.w};
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          const float x = uq.w - c.ShfR[4 * v + t];
+          const float ex = ex2f(-c.etaR_l2e * x * x);
+          coef = fmaf(gg[t] * ex, fmaf(-2.0f * c.etaR * x, f, df), coef);
+        }
+      }
+      float px = coef * uq.x, py = coef * uq.y, pz = coef * uq.z;
+      // angular share of this neighbour, if it is one: binary search of q in posA
+      int lo = 0, hi = nA;
+      while (lo < hi) { int mid = (lo + hi) >> 1; if (e.posA[mid] < q) lo = mid + 1; else hi = mid; }
+      if (lo < nA && e.posA[lo] == q) { px += Pacc[w][lo][0]; py += Pacc[w][lo][1]; pz += Pacc[w][lo][2]; }
+      const long long fx = to_fix(px), fy = to_fix(py), fz = to_fix(pz);
+      ox += fx; oy += fy; oz += fz;
+      const int jp = (int)(rowR[q] & JMASK);
+      atomicAdd(&facc[3 * (size_t)jp + 0], (unsigned long long)(-fx));
+      atomicAdd(&facc[3 * (size_t)jp + 1], (unsigned long long)(-fy));
+      atomicAdd(&facc[3 * (size_t)jp + 2], (unsigned long long)(-fz));
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) { ox += shfl_xor_ll(ox, o); oy += shfl_xor_ll(oy, o); oz += shfl_xor_ll(oz, o); }
+  if (lane == 0) {
+    atomicAdd(&facc[3 * (size_t)ip + 0], (unsigned long long)ox);
+    atomicAdd(&facc[3 * (size_t)ip + 1], (unsigned long long)oy);
+    atomicAdd(&facc[3 * (size_t)ip + 2], (unsigned long long)oz);
+  }
+}
+
+// K8b: facc (sorted order, fixed point; = sum_j (p_aj - p_ja) = +F) -> forces in the caller's atom order.
+__global__ void k_force_out(const float4* __restrict__ spos, const unsigned long long* __restrict__ facc,
+                            const int32_t* __restrict__ ml, int n_ml, float* __restrict__ forces) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ip >= n_ml) return;
+  const int a = __float_as_int(spos[ip].w) & 0x0fffffff;
+  const size_t o = ml ? (size_t)ml[a] : (size_t)a;
+  const double sc = 1.0 / 1099511627776.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) forces[3 * o + d] = (float)((double)(long long)facc[3 * (size_t)ip + d] * sc);
+}
+
+// E = sum_i E_i over the valid rows, fixed order (thread-strided partial sums in fp64, then a fixed tree).
+__global__ void __launch_bounds__(1024) k_energy(const GroupInfo* __restrict__ grp, const float* __restrict__ e_atom,
+                                                 int S, double* __restrict__ energy) {
+  __shared__ double part[1024];
+  double s = 0.0;
+  for (int q = 0; q < S; ++q) {
+    const int r0 = grp->start[q] + grp->pad_shift[q], n = grp->count[q];
+    for (int r = threadIdx.x; r < n; r += 1024) s += (double)e_atom[r0 + r];
+  }
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *energy = part[0];
+}
+
+int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
+                       float* d_forces) {
+  const nnp_model* m = ws->model;
+  int nl = 0;
+  cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
+  if (n_ml > 0) {
+    const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
+    k_aev_backward<<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR, ws->nbrA,
+                                                          ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
+                                                          ws->facc);
+    k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces);
+    nl += 2;
+  }
+  k_energy<<<1, 1024, 0, ws->stream>>>(ws->groups, ws->e_atom, m->aev.S, d_energy);
+  return nl + 1;
+}
+
+}  // namespace nnp
