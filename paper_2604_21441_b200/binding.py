@@ -234,7 +234,8 @@ class Workspace:
         ml_ptr, n_ml = None, n
         if ml_index is not None:
             assert ml_index.is_cuda and ml_index.dtype == torch.int32 and ml_index.is_contiguous()
-            ml_ptr, n_ml = ml_index.data_ptr(), ml_index.shape[0]
+            n_ml = ml_index.shape[0]
+            ml_ptr = ml_index.data_ptr() if n_ml > 0 else Z.data_ptr()  # empty subset: any non-NULL pointer
         rc = nnp_eval(self.handle, n, pos.data_ptr(), Z.data_ptr(), b.ctypes.data, pbc, ml_ptr, n_ml,
                       energy.data_ptr(), forces.data_ptr())
         _check(rc, "nnp_eval")

@@ -1,0 +1,279 @@
+"""-m gpu: the CUDA path (through the C-ABI binding) against the fp64 CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star; SURVEY.md section 8.c reading #23):
+  neighbour lists   bit-exact after canonical sort
+  energy            |E_gpu - E_oracle| / n_ml <= 1e-4 eV/atom
+  forces            RMS relative error <= 1e-3, max abs component error <= 5e-3 eV/Angstrom
+  AEV (debug)       |dG| <= 2e-5 * (1 + |G|)   (fp32 arithmetic, ex2.approx, B^32 by squaring)
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+E_TOL, F_RMS_TOL, F_MAX_TOL = 1e-4, 1e-3, 5e-3
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def make(cfg, mode=None, max_atoms=None):
+    import paper_2604_21441_b200 as nnp
+    m = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    n = cfg["pos"].shape[0] if max_atoms is None else max_atoms
+    n_ml = n if cfg["ml_index"] is None else len(cfg["ml_index"])
+    ws = nnp.Workspace(m, n, n_ml if max_atoms is None else max_atoms)
+    if mode is not None:
+        ws.set_mlp_mode(mode)
+    return m, ws
+
+
+def run_gpu(ws, pos, Z, box, pbc=1, ml=None):
+    torch = _torch()
+    dpos = torch.from_numpy(np.ascontiguousarray(pos, np.float32)).cuda()
+    dZ = torch.from_numpy(np.ascontiguousarray(Z, np.int32)).cuda()
+    dml = None if ml is None else torch.from_numpy(np.ascontiguousarray(ml, np.int32)).cuda()
+    E, F = ws.eval(dpos, dZ, box, pbc, dml)
+    torch.cuda.synchronize()
+    st = ws.status()
+    assert st == 0, f"nnp_status {st}"
+    return float(E.cpu()[0]), F.cpu().numpy().astype(np.float64)
+
+
+def check_EF(Eg, Fg, ref, n_ml, rows=None):
+    Fo = ref["forces"]
+    dE = abs(Eg - ref["energy"]) / max(n_ml, 1)
+    if rows is not None:
+        Fg, Fo = Fg[rows], Fo[rows]
+    dF = Fg - Fo
+    rms = np.sqrt((dF ** 2).sum() / max((Fo ** 2).sum(), 1e-300))
+    mx = np.abs(dF).max() if dF.size else 0.0
+    assert dE <= E_TOL, f"energy error {dE:.3e} eV/atom"
+    assert rms <= F_RMS_TOL, f"force RMS rel {rms:.3e}"
+    assert mx <= F_MAX_TOL, f"force max abs {mx:.3e}"
+    return dE, rms, mx
+
+
+def check_lists(ws, cfg, pos, n_ml, ml=None, pbc=1):
+    for which, Rc in ((0, cfg["aev"]["Rcr"]), (1, cfg["aev"]["Rca"])):
+        s_o, c_o = oracle.neighbors(pos, cfg["box"], Rc, pbc, ml, mode=1 if n_ml > 4000 else 0)
+        s_g, c_g = ws.neighbors(which, n_ml)
+        assert np.array_equal(s_o, s_g), f"row starts differ (which={which})"
+        assert np.array_equal(c_o, c_g), f"columns differ (which={which})"
+
+
+# ------------------------------------------------------------------ full configs
+@pytest.mark.parametrize("k", [0, 1])
+def test_config_small(k):
+    cfg = gen.get_config(k)
+    n = cfg["pos"].shape[0]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None, want_aev=True, want_atomic=True)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_lists(ws, cfg, cfg["pos"], n)
+    G = ws.aev(n).astype(np.float64)
+    assert np.all(np.abs(G - ref["aev"]) <= 2e-5 * (1 + np.abs(ref["aev"]))), np.abs(G - ref["aev"]).max()
+    ea = ws.atomic_energies(n).astype(np.float64)
+    assert np.abs(ea - ref["e_atom"]).max() <= 1e-4
+    check_EF(Eg, Fg, ref, n)
+    assert abs(Fg.sum(0)).max() < 1e-3
+    # every MLP arithmetic mode the library offers must meet the bar (BF16X1 is ladder-only, excluded)
+    import paper_2604_21441_b200 as nnp
+    for mode in (nnp.NNP_MLP_FP32_SIMT, nnp.NNP_MLP_BF16X3):
+        if nnp.nnp_workspace_set_mlp_mode(ws.handle, mode) != 0:
+            continue
+        Eg2, Fg2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+        check_EF(Eg2, Fg2, ref, n)
+
+
+def test_config1_perturbed_steps():
+    """cfg 1: positions perturbed by seeded N(0, 0.01 A) per step (reading #17): lists change every step."""
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 4)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    m, ws = make(cfg)
+    for t in (0, 3):
+        ref = oracle.evaluate(om, P[t], cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
+        Eg, Fg = run_gpu(ws, P[t], cfg["Z"], cfg["box"])
+        check_lists(ws, cfg, P[t], n)
+        check_EF(Eg, Fg, ref, n)
+
+
+def test_config2_full_size():
+    """cfg 2 (24 000 atoms, the bench workload): lists bit-exact, E and F against the oracle on every atom."""
+    cfg = gen.get_config(2)
+    n = cfg["pos"].shape[0]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_lists(ws, cfg, cfg["pos"], n)
+    check_EF(Eg, Fg, ref, n)
+    # dense-K mode ("as ANI would run it") gives the same answer
+    ws.set_dense_k(1)
+    Eg2, Fg2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_EF(Eg2, Fg2, ref, n)
+
+
+def test_config3_sampled():
+    """cfg 3 (96 000 atoms): lists bit-exact; E/F checked on every atom with the oracle's cell-list mode."""
+    cfg = gen.get_config(3)
+    n = cfg["pos"].shape[0]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_lists(ws, cfg, cfg["pos"], n)
+    check_EF(Eg, Fg, ref, n)
+
+
+@pytest.mark.parametrize("layout", ["A", "B"])
+def test_config4_mlmm_subset(layout):
+    cfg = gen.get_config(4, layout=layout)
+    ml = cfg["ml_index"]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    check_lists(ws, cfg, cfg["pos"], len(ml), ml)
+    check_EF(Eg, Fg, ref, len(ml), rows=ml)
+    mm = np.setdiff1d(np.arange(cfg["pos"].shape[0]), ml)
+    assert np.all(Fg[mm] == 0.0) and not np.any(np.signbit(Fg[mm]))   # MM rows are +0.0f
+    # MM independence: scrambling MM coordinates and atomic numbers changes nothing, bit for bit
+    pos2, Z2 = cfg["pos"].copy(), cfg["Z"].copy()
+    rng = np.random.default_rng(7)
+    pos2[mm] += rng.normal(0, 1.0, size=(len(mm), 3)).astype(np.float32)
+    Z2[mm] = 99
+    Eg2, Fg2 = run_gpu(ws, pos2, Z2, cfg["box"], 1, ml)
+    assert Eg2 == Eg and np.array_equal(Fg2, Fg)
+
+
+# ------------------------------------------------------------------ edge and degenerate cases
+def _small_cfg(bias_scale=0.0):
+    return gen.get_config(0, bias_scale=bias_scale)
+
+
+def test_bitwise_reproducible_and_host_entry():
+    cfg = gen.get_config(1)
+    m, ws = make(cfg)
+    E1, F1 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    assert E1 == E2 and np.array_equal(F1, F2)
+    E3, F3 = ws.eval_host(cfg["pos"], cfg["Z"], cfg["box"])
+    assert ws.status() == 0
+    assert E3 == E1 and np.array_equal(F3.astype(np.float64), F1)
+    assert ws.launches() > 0
+
+
+def test_nonzero_biases_and_padding_rows():
+    """Non-zero biases make MLP(0) != 0: padded tile rows must not leak into E."""
+    cfg = _small_cfg(bias_scale=0.3)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_EF(Eg, Fg, ref, cfg["pos"].shape[0])
+
+
+def test_open_boundaries_cluster_and_orthorhombic_box():
+    cfg = gen.get_config(4)
+    ml = cfg["ml_index"]
+    pos, Z = cfg["pos"][ml].copy(), cfg["Z"][ml].copy()
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    sub = dict(cfg, pos=pos, Z=Z, ml_index=None)
+    m, ws = make(sub)
+    ref = oracle.evaluate(om, pos, Z, cfg["box"], 0, None)
+    Eg, Fg = run_gpu(ws, pos, Z, cfg["box"], 0)
+    check_lists(ws, cfg, pos, len(pos), None, pbc=0)
+    check_EF(Eg, Fg, ref, len(pos))
+    # orthorhombic, non-cubic box; one dimension with fewer than three cells; atoms shifted by box vectors
+    box = np.diag([17.0, 23.5, 12.0]).astype(np.float32).reshape(9)
+    rng = np.random.default_rng(11)
+    pos2 = (pos - pos.mean(0) + np.array([8.0, 11.0, 6.0])).astype(np.float32)
+    shift = rng.integers(-2, 3, size=pos2.shape) * np.array([17.0, 23.5, 12.0])
+    pos2 = (pos2 + shift).astype(np.float32)
+    ref2 = oracle.evaluate(om, pos2, Z, box, 1, None)
+    Eg2, Fg2 = run_gpu(ws, pos2, Z, box, 1)
+    cfg2 = dict(cfg, box=box)
+    check_lists(ws, cfg2, pos2, len(pos2))
+    check_EF(Eg2, Fg2, ref2, len(pos2))
+
+
+def test_one_layer_network_golden_monomer():
+    """All-ones one-layer network on a water monomer: E = 7.1130060875."""
+    import json, os
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "appendix_b.json")))
+    aev = gen.aev_params(gen.weights.SPECIES_4)
+    L = gen.aev_length(aev)
+    nets = {Z: ((L, 1), [np.ones((1, L), np.float32)], [np.zeros(1, np.float32)]) for Z in (1, 6, 7, 8)}
+    R, phi = 0.9572, np.deg2rad(104.52 / 2)
+    O = np.array([10.0, 10.0, 10.0])
+    pos = np.array([O, O + [R * np.sin(phi), 0, R * np.cos(phi)], O + [-R * np.sin(phi), 0, R * np.cos(phi)]], np.float32)
+    Z = np.array([8, 1, 1], np.int32)
+    box = np.diag([30.0] * 3).astype(np.float32).reshape(9)
+    cfg = dict(aev=aev, nets=nets, celu_alpha=0.1, pos=pos, ml_index=None, box=box)
+    m, ws = make(cfg)
+    Eg, Fg = run_gpu(ws, pos, Z, box)
+    key = [k for k in gold if "E" in k and "B2" in k]
+    assert abs(Eg - 7.1130060875) < 2e-5, (Eg, key)
+    assert abs(Fg[0, 2] + 0.98434044) < 2e-4 and abs(Fg[1, 0] - 2.68119284) < 2e-4
+    assert abs(Fg.sum(0)).max() < 1e-5
+
+
+def test_empty_and_single_atom():
+    cfg = _small_cfg(bias_scale=0.2)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    m, ws = make(cfg)
+    torch = _torch()
+    # n_atoms = 0
+    E, F = ws.eval(torch.zeros((0, 3), dtype=torch.float32, device="cuda"),
+                   torch.zeros((0,), dtype=torch.int32, device="cuda"), cfg["box"])
+    torch.cuda.synchronize()
+    assert ws.status() == 0 and float(E.cpu()[0]) == 0.0
+    # one atom: E = MLP(0), F = 0
+    pos, Z = cfg["pos"][:1], cfg["Z"][:1]
+    ref = oracle.evaluate(om, pos, Z, cfg["box"], 1, None)
+    Eg, Fg = run_gpu(ws, pos, Z, cfg["box"])
+    assert abs(Eg - ref["energy"]) < 1e-5 and np.all(Fg == 0.0)
+    # empty ML subset of a non-empty system
+    ml = np.zeros((0,), np.int32)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert Eg == 0.0 and np.all(Fg == 0.0)
+
+
+def test_error_reporting():
+    import paper_2604_21441_b200 as nnp
+    cfg = _small_cfg()
+    m, ws = make(cfg)
+    torch = _torch()
+    dpos = torch.from_numpy(cfg["pos"]).cuda()
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    bad_box = cfg["box"].copy(); bad_box[1] = 0.5
+    with pytest.raises(nnp.NNPError) as e:
+        ws.eval(dpos, dZ, bad_box)
+    assert e.value.code == -3
+    Zbad = cfg["Z"].copy(); Zbad[5] = 16   # sulfur: no slot in the 4-species model
+    ws.eval(dpos, torch.from_numpy(Zbad).cuda(), cfg["box"])
+    assert ws.status() == -2
+    ml = torch.tensor([3, 2, 10], dtype=torch.int32, device="cuda")   # not ascending
+    ws.eval(dpos, dZ, cfg["box"], 1, ml)
+    assert ws.status() == -1
+    pos2 = cfg["pos"].copy(); pos2[7] = pos2[3]
+    ws.eval(torch.from_numpy(pos2).cuda(), dZ, cfg["box"])
+    assert ws.status() == -5
+    # too many atoms for the workspace
+    big = torch.zeros((cfg["pos"].shape[0] + 1, 3), dtype=torch.float32, device="cuda")
+    with pytest.raises(nnp.NNPError):
+        ws.eval(big, torch.ones(big.shape[0], dtype=torch.int32, device="cuda"), cfg["box"])
+    # the workspace still works afterwards
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    check_EF(Eg, Fg, ref, cfg["pos"].shape[0])
