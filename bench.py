@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py -- NNP energy+force throughput on seeded synthetic water boxes (BASELINE.json metric).
+
+One "step" = one full nnp_eval (K0-K8, neighbour list rebuilt) of the cfg-2 water box (8000 H2O, 24 000 atoms,
+1008-length AEV, ANI-2x-shaped H/O networks), cycling over 16 seeded perturbed position sets so that the lists
+really change.  value = atom-steps/s with inputs resident in HBM; e2e = the same through
+nnp_eval_host with pinned HOST buffers (H2D + D2H inside the timed region).  L2 is flushed between timed steps.
+N > 1 (torchrun): independent replicas, one box per GPU, no data-path collective ("scaling": "weak").
+--impl reference: the fp64 CPU oracle as it stands, on the host cores, rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+import gen  # noqa: E402
+
+METRIC = "nnp_energy_force_atom_steps_per_s"
+UNIT = "atom-steps/s"
+WORKLOAD = "cfg2_water_8000 (24000 atoms, AEV 1008, H 1008-256-192-160-1 / O 1008-224-192-160-1)"
+N_POS_SETS = 16
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x FMA x max SM clock
+# algorithmic FP32 work of the AEV kernels: per directed radial pair / per unordered triplet
+FLOP_FWD_PAIR, FLOP_FWD_TRIPLET = 16 * 6, 170
+FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sustained=d.get("bf16_tflops_sustained"),
+                    src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, src="fallback")
+
+
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, dev):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(dev), f"--query-gpu={self.Q}", "--format=csv,noheader",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.count(",") >= 8]
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        mhz = [float(r[1].split()[0]) for r in rows]
+        reasons = set()
+        for r in rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if "Active" in v and "Not" not in v:
+                    reasons.add(name)
+        out.update(sm_mhz=float(np.median(mhz)), sm_max_mhz=float(rows[0][2].split()[0]), reasons=sorted(reasons),
+                   samples=len(rows))
+        return out
+
+
+def mlp_flops_per_atom(dims, K0):
+    """4 x MACs (forward + backward, no weight gradients) with first-layer width K0."""
+    d = (K0,) + tuple(dims[1:])
+    return 4 * sum(d[i] * d[i + 1] for i in range(len(d) - 1))
+
+
+def run_reference(args, rank):
+    """The oracle as it stands on the host cores; each step = one evaluation of a sub-box of the same generator,
+    density and model, sized so that the whole run ends within a few minutes."""
+    if rank != 0:
+        return
+    import oracle
+    cfg = gen.get_config(2)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    budget_s = 150.0 / max(args.steps + args.warmup, 1)
+    n = int(min(20, max(4, (budget_s * 4000.0 / 3.0) ** (1.0 / 3.0))))
+    if n == 20:
+        pos, Z, box = cfg["pos"], cfg["Z"], cfg["box"]
+    else:
+        pos, Z, box, _ = gen.water_box(n, n, n, 62.1 * n / 20.0, 102)
+    for _ in range(args.warmup):
+        oracle.evaluate(om, pos, Z, box, 1, None, nbr_mode=1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.evaluate(om, pos, Z, box, 1, None, nbr_mode=1)
+    dt = time.perf_counter() - t0
+    v = pos.shape[0] * args.steps / dt
+    sample = f"{n}x{n}x{n} H2O sub-box ({pos.shape[0]} atoms) of the cfg-2 generator/model, one evaluation per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "ns_per_day_2fs": 0.1728 * args.steps / dt}))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import paper_2604_21441_b200 as nnp
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    cfg = gen.get_config(2)
+    n = cfg["pos"].shape[0]
+    # replicas: rank r perturbs with its own seed, so every GPU runs an independent box of the same shape
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"] + 1000 * rank, N_POS_SETS)
+    model = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ws = nnp.Workspace(model, n)
+    if args.mlp_mode != "default":
+        ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "bf16x3": nnp.NNP_MLP_BF16X3}[args.mlp_mode])
+    dpos = [torch.from_numpy(P[t]).cuda() for t in range(N_POS_SETS)]
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    E = torch.zeros(1, dtype=torch.float64, device="cuda")
+    F = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    box = cfg["box"]
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up (also collects the workload statistics used for the algorithmic work)
+    for t in range(max(args.warmup, 3)):
+        ws.eval(dpos[t % N_POS_SETS], dZ, box, 1, None, E, F)
+    torch.cuda.synchronize()
+    assert ws.status() == 0
+    launches_per_step = ws.launches()
+    sR, _ = ws.neighbors(0, n)
+    sA, _ = ws.neighbors(1, n)
+    nA = np.diff(sA).astype(np.int64)
+    pairs_R, triplets = int(sR[-1]), int((nA * (nA - 1) // 2).sum())
+
+    # ---- device-resident timing: per-step CUDA events, L2 flushed between steps, stage events inside
+    ws.set_profiling(1)
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    stage = np.zeros(5)
+    clocks = ClockSampler(local_rank)
+    barrier()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.zero_()
+        ev0[k].record()
+        ws.eval(dpos[k % N_POS_SETS], dZ, box, 1, None, E, F)
+        ev1[k].record()
+        stage += ws.stage_times()     # waits for this step's last event (outside the timed events)
+    barrier()
+    wall = time.perf_counter() - wall0
+    clk = clocks.stop()
+    assert ws.status() == 0
+    ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
+    total_s = float(ms.sum()) * 1e-3
+    ws.set_profiling(0)
+
+    # ---- end to end: nnp_eval_host with pinned host buffers (H2D of pos/Z, D2H of E/F, sync inside the call)
+    hpos = [torch.from_numpy(P[t]).pin_memory() for t in range(N_POS_SETS)]
+    hZ = torch.from_numpy(cfg["Z"]).pin_memory()
+    hF = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    for t in range(3):
+        ws.eval_host(hpos[t].numpy(), hZ.numpy(), box, 1, None, hF.numpy())
+    e2e_s = 0.0
+    barrier()
+    for k in range(args.steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ws.eval_host(hpos[k % N_POS_SETS].numpy(), hZ.numpy(), box, 1, None, hF.numpy())
+        e2e_s += time.perf_counter() - t0
+    barrier()
+
+    if dist is not None:
+        tt = torch.tensor([total_s, e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_s, e2e_s = float(tt[0]), float(tt[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    value = world * n * args.steps / total_s
+    e2e = world * n * args.steps / e2e_s
+    stage_ms = stage / args.steps
+    names = ["neighbour", "aev_forward", "mlp", "aev_backward", "output"]
+    nH, nO = int((cfg["Z"] == 1).sum()), int((cfg["Z"] == 8).sum())
+    Kc = 160   # compacted AEV width for an H/O-only system: 2 radial + 3 angular 32-column blocks
+    mlp_flops = nH * mlp_flops_per_atom(cfg["nets"][1][0], Kc) + nO * mlp_flops_per_atom(cfg["nets"][8][0], Kc)
+    work = {
+        "neighbour": ("hbm", n * (16 + 32 + 8) + 4 * pairs_R + pairs_R // 4, pk["hbm"], "GB/s", 1e9),
+        "aev_forward": ("alu", pairs_R * FLOP_FWD_PAIR + triplets * FLOP_FWD_TRIPLET, FP32_PEAK_TFLOPS, "TFLOP/s", 1e12),
+        "mlp": ("tensor", mlp_flops, pk["bf16"], "TFLOP/s", 1e12),
+        "aev_backward": ("alu", pairs_R * FLOP_BWD_PAIR + triplets * FLOP_BWD_TRIPLET, FP32_PEAK_TFLOPS, "TFLOP/s", 1e12),
+        "output": ("hbm", n * (24 + 16 + 12), pk["hbm"], "GB/s", 1e9),
+    }
+    stages = {}
+    for i, nm in enumerate(names):
+        bound, w, peak, unit, sc = work[nm]
+        ach = w / (stage_ms[i] * 1e-3) / sc if stage_ms[i] > 0 else 0.0
+        stages[nm] = {"ms": float(stage_ms[i]), "bound": bound, "achieved": ach, "peak": peak, "unit": unit,
+                      "frac": ach / peak}
+    dom = names[int(np.argmax(stage_ms))]
+    roof = dict(stages[dom])
+    roof.pop("ms")
+    roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md)", traffic=None)
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+        t0 = time.perf_counter()
+        reps = 2
+        for t in range(reps):
+            ref = oracle.evaluate(om, P[t], cfg["Z"], box, 1, None, nbr_mode=1)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n * reps / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{reps} full evaluations of the 24000-atom box (position sets 0-{reps - 1})"}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "atoms_per_gpu": n, "position_sets": N_POS_SETS,
+                   "l2": "flushed between timed steps (256 MiB write)", "mlp_mode": args.mlp_mode,
+                   "radial_pairs": pairs_R, "triplets": triplets, "parallelism": f"replicas x{world}"},
+        "ns_per_day_2fs": 0.1728 * args.steps / total_s,
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 12 * n + 8,
+                "ms_per_step": 1e3 * e2e_s / args.steps},
+        "gpu_launches": int(launches_per_step * args.steps),
+        "clocks": clk, "roofline": roof, "stages": stages, "cpu_baseline": cpu,
+        "ms_per_step_min": float(ms.min()), "ms_per_step_median": float(np.median(ms)), "wall_s": wall}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "bf16x3"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -126,6 +126,13 @@ int nnp_debug_neighbors(nnp_workspace*, int which, int64_t* n_pairs, int32_t* h_
 int nnp_debug_aev(nnp_workspace*, float* h_aev);
 int nnp_debug_atomic_energies(nnp_workspace*, float* h_e);
 int nnp_debug_counters(nnp_workspace*, int64_t* launches);
+/* Stage timing of nnp_eval with CUDA events on the workspace stream.  set_profiling(1) makes every later
+ * nnp_eval record an event at each stage boundary (not capturable into a CUDA graph while on);
+ * nnp_debug_stage_times waits for the last evaluation and writes HOST ms[5] = {neighbour stage K0-K2,
+ * AEV forward K3, MLP forward+backward K4-K6, AEV backward K7 (pair partials + scatter), force output +
+ * energy reduction K8}. */
+int nnp_workspace_set_profiling(nnp_workspace*, int32_t on);
+int nnp_debug_stage_times(nnp_workspace*, float* ms);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,7 @@ EXPORTS = [
     "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev",
-    "nnp_debug_atomic_energies", "nnp_debug_counters",
+    "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
 
 
@@ -74,6 +74,8 @@ def lib():
         L.nnp_debug_aev.argtypes = [vp, vp]
         L.nnp_debug_atomic_energies.argtypes = [vp, vp]
         L.nnp_debug_counters.argtypes = [vp, C.POINTER(i64)]
+        L.nnp_workspace_set_profiling.argtypes = [vp, i32]
+        L.nnp_debug_stage_times.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -146,6 +148,14 @@ def nnp_debug_counters(ws):
     n = C.c_int64(0)
     rc = lib().nnp_debug_counters(ws, C.byref(n))
     return rc, n.value
+
+
+def nnp_workspace_set_profiling(ws, on):
+    return lib().nnp_workspace_set_profiling(ws, int(on))
+
+
+def nnp_debug_stage_times(ws, h_ms):
+    return lib().nnp_debug_stage_times(ws, h_ms)
 
 
 # ---------------------------------------------------------------- convenience owners
@@ -282,6 +292,15 @@ class Workspace:
         e = np.zeros(n_ml, dtype=np.float32)
         _check(nnp_debug_atomic_energies(self.handle, e.ctypes.data), "nnp_debug_atomic_energies")
         return e
+
+    def set_profiling(self, on):
+        _check(nnp_workspace_set_profiling(self.handle, on), "nnp_workspace_set_profiling")
+
+    def stage_times(self):
+        """ms per stage of the last evaluation: neighbour, aev_fwd, mlp, aev_bwd, output."""
+        ms = np.zeros(5, dtype=np.float32)
+        _check(nnp_debug_stage_times(self.handle, ms.ctypes.data), "nnp_debug_stage_times")
+        return ms
 
     def launches(self):
         rc, n = nnp_debug_counters(self.handle)

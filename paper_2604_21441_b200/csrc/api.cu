@@ -144,6 +144,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   if (!ws) return NNP_OK;
   cudaStreamSynchronize(ws->stream);
   tc_workspace_destroy(ws);
+  for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
   void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
                   ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->hd_pos, ws->hd_Z, ws->hd_ml,
@@ -198,6 +199,21 @@ extern "C" int nnp_workspace_set_mlp_mode(nnp_workspace* ws, int32_t mode) {
   return NNP_ERR_INVALID_ARG;
 }
 
+extern "C" int nnp_workspace_set_profiling(nnp_workspace* ws, int32_t on) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  if (on && !ws->ev[0])
+    for (int i = 0; i < 6; ++i) CU_OK(cudaEventCreate(&ws->ev[i]));
+  ws->profiling = on ? 1 : 0;
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_stage_times(nnp_workspace* ws, float* ms) {
+  if (!ws || !ms || !ws->profiling) return NNP_ERR_INVALID_ARG;
+  CU_OK(cudaEventSynchronize(ws->ev[5]));
+  for (int i = 0; i < 5; ++i) CU_OK(cudaEventElapsedTime(&ms[i], ws->ev[i], ws->ev[i + 1]));
+  return NNP_OK;
+}
+
 extern "C" int nnp_workspace_set_dense_k(nnp_workspace* ws, int32_t dense) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   ws->dense_k = dense ? 1 : 0;
@@ -226,10 +242,16 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   if (rc) return rc;
   const float unit[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
   ws->n_atoms = n_atoms; ws->n_ml = n_ml; ws->d_ml_index = d_ml;
+  prof_mark(ws, 0);
   int nl = launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
+  prof_mark(ws, 1);
   nl += launch_aev_forward(ws, n_ml);
+  prof_mark(ws, 2);
   nl += (ws->mlp_mode == NNP_MLP_FP32_SIMT) ? launch_mlp_simt(ws, n_ml) : launch_mlp_tc(ws, n_ml);
+  prof_mark(ws, 3);
+  if (n_ml <= 0) prof_mark(ws, 4);
   nl += launch_force_stage(ws, n_atoms, n_ml, d_ml, d_energy, d_forces);
+  prof_mark(ws, 5);
   ws->launches = nl;
   if (cudaGetLastError() != cudaSuccess) return NNP_ERR_CUDA;
   return NNP_OK;

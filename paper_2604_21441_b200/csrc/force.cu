@@ -192,6 +192,7 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
     k_aev_backward<<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR, ws->nbrA,
                                                           ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
                                                           ws->facc);
+    prof_mark(ws, 4);
     k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces);
     nl += 2;
   }

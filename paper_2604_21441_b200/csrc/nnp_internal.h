@@ -132,11 +132,14 @@ struct nnp_workspace {
   float* e_atom;             // [max_rows]
   unsigned long long* facc;  // [max_ml][3] int64 fixed point, indexed by sorted position
   void* tc_ws;               // tensor-core path scratch
+  int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
+  cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end
   // host-buffer entry point
   float* hd_pos; int32_t* hd_Z; int32_t* hd_ml; double* hd_energy; float* hd_forces;
 };
 
 namespace nnp {
+inline void prof_mark(nnp_workspace* ws, int i) { if (ws->profiling) cudaEventRecord(ws->ev[i], ws->stream); }
 // stage launchers (each returns the number of kernels it launched)
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
