@@ -63,16 +63,19 @@ typedef struct {
 
 /* MLP arithmetic (nnp_workspace_set_mlp_mode):
  *   NNP_MLP_FP32_SIMT  fp32 FMA on CUDA cores (reference rung of the precision ladder, slow)
- *   NNP_MLP_BF16X3     tcgen05 tensor cores, operands split x = hi + lo in bf16, three products
- *                      hi*hi + hi*lo + lo*hi accumulated in fp32 TMEM (default)
- *   NNP_MLP_BF16X1     tcgen05, one bf16 product (fails the force tolerance; for the ladder only) */
+ *   NNP_MLP_F16X3      tcgen05 tensor cores, every operand split x = hi + lo in fp16, three products
+ *                      hi*hi + lo*hi + hi*lo accumulated in fp32 TMEM: fp32-grade results (default)
+ *   NNP_MLP_F16X1      tcgen05, the single fp16 product hi*hi (3x fewer MMAs; force error ~6e-4 RMS
+ *                      relative, inside the 1e-3 bar with little margin -- see DESIGN.md) */
 #define NNP_MLP_FP32_SIMT 0
-#define NNP_MLP_BF16X3 1
-#define NNP_MLP_BF16X1 2
+#define NNP_MLP_F16X3 1
+#define NNP_MLP_F16X1 2
 
-/* Creates the immutable model: copies parameters, uploads weights (and the derived bf16 hi/lo tile
+/* Creates the immutable model: copies parameters, uploads weights (and the derived fp16 hi/lo tile
  * images) to the current CUDA device.  Limits: n_species <= 8, nShfR <= 16, nShfA*nShfZ == 32,
- * hidden widths multiples of 16 and <= 256, n_layers <= 4  -> otherwise NNP_ERR_UNSUPPORTED. */
+ * hidden widths multiples of 16 and <= 256, n_layers <= 4  -> otherwise NNP_ERR_UNSUPPORTED.
+ * The tensor-core modes additionally need n_layers == 4, hidden widths multiples of 32 and |w| < 6e4
+ * (fp16 range); a model outside that runs in NNP_MLP_FP32_SIMT and set_mlp_mode(F16*) returns UNSUPPORTED. */
 int nnp_model_create(const nnp_aev_params* aev, const nnp_mlp_desc* nets /* HOST [n_species] */, nnp_model** out);
 int nnp_model_destroy(nnp_model*);
 int nnp_model_aev_length(const nnp_model*);
@@ -119,11 +122,14 @@ const char* nnp_strerror(int);
  *     ml_index order; h_col = GLOBAL atom indices, ascending within a row.  Pass h_col = NULL (or a too
  *     small cap) to query *n_pairs only.
  *   nnp_debug_aev: fp32 AEV rows [n_ml][aev_length] in ml_index order.
+ *   nnp_debug_daev: fp32 dE_i/dAEV_i rows [n_ml][aev_length] in ml_index order (output of K6); columns of
+ *     species absent from the evaluation are reported as 0 (they are never materialised).
  *   nnp_debug_atomic_energies: [n_ml] in ml_index order.
  *   nnp_debug_counters: launches[0] = number of kernels launched by the last nnp_eval. */
 int nnp_debug_neighbors(nnp_workspace*, int which, int64_t* n_pairs, int32_t* h_row_start, int32_t* h_col,
                         int64_t col_cap);
 int nnp_debug_aev(nnp_workspace*, float* h_aev);
+int nnp_debug_daev(nnp_workspace*, float* h_daev);
 int nnp_debug_atomic_energies(nnp_workspace*, float* h_e);
 int nnp_debug_counters(nnp_workspace*, int64_t* launches);
 /* Stage timing of nnp_eval with CUDA events on the workspace stream.  set_profiling(1) makes every later

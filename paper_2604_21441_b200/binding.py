@@ -12,12 +12,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 
 NNP_OK = 0
-NNP_MLP_FP32_SIMT, NNP_MLP_BF16X3, NNP_MLP_BF16X1 = 0, 1, 2
+NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
     "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
-    "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev",
+    "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
 
@@ -72,6 +72,7 @@ def lib():
         L.nnp_strerror.restype = C.c_char_p
         L.nnp_debug_neighbors.argtypes = [vp, C.c_int, C.POINTER(i64), vp, vp, i64]
         L.nnp_debug_aev.argtypes = [vp, vp]
+        L.nnp_debug_daev.argtypes = [vp, vp]
         L.nnp_debug_atomic_energies.argtypes = [vp, vp]
         L.nnp_debug_counters.argtypes = [vp, C.POINTER(i64)]
         L.nnp_workspace_set_profiling.argtypes = [vp, i32]
@@ -138,6 +139,10 @@ def nnp_debug_neighbors(ws, which, h_row_start, h_col, col_cap):
 
 def nnp_debug_aev(ws, h_aev):
     return lib().nnp_debug_aev(ws, h_aev)
+
+
+def nnp_debug_daev(ws, h_daev):
+    return lib().nnp_debug_daev(ws, h_daev)
 
 
 def nnp_debug_atomic_energies(ws, h_e):
@@ -286,6 +291,11 @@ class Workspace:
     def aev(self, n_ml):
         a = np.zeros((n_ml, self.model.aev_length), dtype=np.float32)
         _check(nnp_debug_aev(self.handle, a.ctypes.data), "nnp_debug_aev")
+        return a
+
+    def daev(self, n_ml):
+        a = np.zeros((n_ml, self.model.aev_length), dtype=np.float32)
+        _check(nnp_debug_daev(self.handle, a.ctypes.data), "nnp_debug_daev")
         return a
 
     def atomic_energies(self, n_ml):

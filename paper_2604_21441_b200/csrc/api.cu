@@ -166,7 +166,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
   ws->model = m; ws->stream = (cudaStream_t)stream; ws->max_atoms = max_atoms; ws->max_ml = max_ml;
   ws->rcap = RCAP_MAX; ws->acap = ACAP_MAX;
   ws->max_cells = (int)std::min<int64_t>(std::max<int64_t>(512, max_ml / 4), 1 << 21);
-  ws->mlp_mode = m->tc ? NNP_MLP_BF16X3 : NNP_MLP_FP32_SIMT;
+  ws->mlp_mode = m->tc ? NNP_MLP_F16X3 : NNP_MLP_FP32_SIMT;
   ws->dense_k = 0;
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
   ws->max_rows = (int64_t)ws->max_tiles * TILE_M;
@@ -191,7 +191,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
 extern "C" int nnp_workspace_set_mlp_mode(nnp_workspace* ws, int32_t mode) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   if (mode == NNP_MLP_FP32_SIMT) { ws->mlp_mode = mode; return NNP_OK; }
-  if (mode == NNP_MLP_BF16X3 || mode == NNP_MLP_BF16X1) {
+  if (mode == NNP_MLP_F16X3 || mode == NNP_MLP_F16X1) {
     if (!ws->model->tc) return NNP_ERR_UNSUPPORTED;
     ws->mlp_mode = mode;
     return NNP_OK;
@@ -379,6 +379,38 @@ extern "C" int nnp_debug_aev(nnp_workspace* ws, float* h_aev) {
     }
   }
   return NNP_OK;
+}
+
+static int export_rows(nnp_workspace* ws, const float* d_buf, float* h_out) {
+  Snapshot s;
+  int rc = take_snapshot(ws, s);
+  if (rc) return rc;
+  const AevConst& c = ws->model->aev;
+  const size_t n = (size_t)ws->n_ml, Kc = (size_t)s.grp.Kc;
+  std::vector<float> buf((size_t)s.grp.n_rows * Kc);
+  if (!buf.empty()) CU_OK(cudaMemcpy(buf.data(), d_buf, buf.size() * sizeof(float), cudaMemcpyDeviceToHost));
+  memset(h_out, 0, n * (size_t)c.L * sizeof(float));
+  for (size_t ip = 0; ip < n; ++ip) {
+    const int a = ml_local(s.spos[ip]), sl = slot_of(s.spos[ip]);
+    const float* row = buf.data() + (ip + s.grp.pad_shift[sl]) * Kc;
+    float* dst = h_out + (size_t)a * c.L;
+    for (int b = 0; b < s.grp.nblk; ++b) {
+      const int ib = s.grp.blkmap[b];
+      for (int q = 0; q < BLK; ++q) {
+        const int icol = ib * BLK + q;  // internal column -> public column
+        int pub;
+        if (ib < c.nRB) { if (icol >= c.S * NSHFR) continue; pub = icol; }
+        else pub = c.S * NSHFR + (icol - c.nRB * BLK);
+        dst[pub] = row[(size_t)b * BLK + q];
+      }
+    }
+  }
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_daev(nnp_workspace* ws, float* h_daev) {
+  if (!ws || !h_daev) return NNP_ERR_INVALID_ARG;
+  return export_rows(ws, ws->daev, h_daev);
 }
 
 extern "C" int nnp_debug_atomic_energies(nnp_workspace* ws, float* h_e) {

@@ -1,10 +1,626 @@
-// mlp_tc.cu -- K5/K6 on the tcgen05 tensor cores (placeholder until the tensor-core tile kernel lands:
-// reports "no tensor-core image", so workspaces start in NNP_MLP_FP32_SIMT).
+// mlp_tc.cu -- K5/K6 on the 5th-generation tensor cores: ONE persistent kernel runs, per 128-atom tile of one
+// element, the whole per-element MLP forward (SURVEY.md Appendix A "Network") and its analytic backward to
+// dE/dAEV (Appendix A "Backward"; eq. 2 needs dE/dr) without the activations ever leaving the SM:
+//
+//     F1  z1 = G  W1^T      F2  z2 = h1 W2^T      F3  z3 = h2 W3^T      (h = CELU(z + b), E_i = h3 . w4 + b4)
+//     B3  d2 = dl3 W3       B2  d1 = dl2 W2       B1  g  = dl1 W1       (dl3 = w4 * c3, dl_l = d_l * c_l, c = CELU')
+//
+// Every GEMM is tcgen05.mma (kind::f16, M = 128, fp32 accumulators in TMEM) issued by one thread; the A operand
+// (AEV tile, then each layer's activations / deltas) lives in shared memory in the canonical K-major
+// SWIZZLE_128B layout and is rewritten in place by the epilogue warps; the B operand (weights) is streamed from
+// L2 by the bulk-copy engine (cp.async.bulk, UBLKCP) through an mbarrier ring from images pre-tiled in exactly the
+// shared-memory layout.  CELU' of layers 1-2 waits for the backward pass in TMEM, packed to 16 bits.
+//
+// Arithmetic (NNP_MLP_F16X3): every operand x is split x = hi + lo with hi = fp16(x), lo = fp16(x - hi) and the
+// product is hi*hi + lo*hi + hi*lo (three MMAs, fp32 accumulate): ~2^-21 relative operand error, i.e. fp32-grade
+// (measured against the fp64 oracle in DESIGN.md).  NNP_MLP_F16X1 keeps only hi*hi.
+#include <cuda_fp16.h>
+#include <string.h>
+#include <vector>
 #include "nnp_internal.h"
+
 namespace nnp {
-int tc_model_create(nnp_model* m, const nnp_mlp_desc*) { m->tc = nullptr; return NNP_OK; }
-void tc_model_destroy(nnp_model*) {}
-int tc_workspace_create(nnp_workspace* ws) { ws->tc_ws = nullptr; return NNP_OK; }
-void tc_workspace_destroy(nnp_workspace*) {}
-int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) { return launch_mlp_simt(ws, n_ml); }
+
+// ------------------------------------------------------------------------------------------------ image geometry
+// A B-operand matrix [N][K] (row n = output column, K contiguous) is cut into N-chunks of tc_chunk(N) rows
+// (<= 128, one MMA each) and K-panels of 64 columns.  Block (c, p) holds rows x 64 fp16 as rows x 128 bytes in
+// the SWIZZLE_128B K-major layout (8-row atoms of 1024 B; 16-byte chunk index XOR row%8), hi half then lo half.
+__host__ __device__ inline int tc_nchunks(int N) { return (N + 127) / 128; }
+__host__ __device__ inline int tc_chunk(int N) { const int nc = tc_nchunks(N); return (((N + nc - 1) / nc) + 15) & ~15; }
+__host__ __device__ inline int tc_npanels(int K) { return (K + 63) / 64; }
+__host__ __device__ inline size_t tc_img_bytes(int N, int K) {
+  return (size_t)tc_nchunks(N) * tc_npanels(K) * 2 * tc_chunk(N) * 128;
+}
+__host__ __device__ inline size_t tc_blk_off(int N, int K, int c, int p, int half) {
+  return ((size_t)(c * tc_npanels(K) + p) * 2 + half) * tc_chunk(N) * 128;
+}
+__host__ __device__ inline int tc_elem_off(int r, int kk) {  // byte offset of element (row r, column kk < 64)
+  return r * 128 + ((((kk >> 3) ^ (r & 7))) << 4) + (kk & 7) * 2;
+}
+
+struct TcNetImg { const uint8_t* w2; const uint8_t* w3; const uint8_t* w3t; const uint8_t* w2t; };
+struct TcTable { TcNetImg n[MAX_S]; };
+
+struct TcModel {
+  TcTable tab;
+  void* blob;
+};
+
+struct TcWorkspace {
+  uint8_t* w1img[MAX_S];   // F1 image [N1][Kc] of each slot (repacked when the compacted column set changes)
+  uint8_t* w1timg[MAX_S];  // B1 image [Kc][N1]
+  unsigned long long* key; // [2]: column-set key the images were packed for / scratch
+  int num_sms;
+  int smem_bytes[2];
+};
+
+// ------------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, fp16 operands, fp32 accumulate, M = 128
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// K-major SWIZZLE_128B shared-memory matrix descriptor: start address >> 4, LBO (unused for swizzled K-major) = 1,
+// SBO = 1024 B between 8-row atoms, descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.
+__device__ __forceinline__ uint64_t tc_desc(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3FFFu) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+}
+// instruction descriptor: D fp32 (bit 4), A/B fp16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+__device__ __forceinline__ uint32_t tc_idesc(int N) { return (1u << 4) | ((uint32_t)(N >> 3) << 17) | (8u << 24); }
+
+#define TC_R8(v, o) "=r"(v[o]), "=r"(v[o + 1]), "=r"(v[o + 2]), "=r"(v[o + 3]), "=r"(v[o + 4]), "=r"(v[o + 5]), "=r"(v[o + 6]), "=r"(v[o + 7])
+#define TC_W8(v, o) "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]), "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), "r"(v[o + 7])
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* v) {  // 32 lanes x 32 columns: lane = thread
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,"
+      "%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : TC_R8(v, 0), TC_R8(v, 8), TC_R8(v, 16), TC_R8(v, 24) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : TC_R8(v, 0), TC_R8(v, 8) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
+      TC_W8(v, 0), TC_W8(v, 8) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ uint32_t h2_bits(__half2 h) { return *reinterpret_cast<uint32_t*>(&h); }
+// (x0, x1) -> packed fp16 hi pair and lo pair (lo = fp16(x - hi))
+__device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 hf = __half22float2(h);
+  hi = h2_bits(h);
+  lo = h2_bits(__floats2half2_rn(x0 - hf.x, x1 - hf.y));
+}
+// CELU' in [0, 1] as unorm16 pairs (1.0 exact); absolute error 2^-17
+__device__ __forceinline__ uint32_t pack_c(float c0, float c1) {
+  return __float2uint_rn(c0 * 65535.f) | (__float2uint_rn(c1 * 65535.f) << 16);
+}
+__device__ __forceinline__ float unpack_c_lo(uint32_t q) { return (float)(q & 0xffffu) * (1.0f / 65535.f); }
+__device__ __forceinline__ float unpack_c_hi(uint32_t q) { return (float)(q >> 16) * (1.0f / 65535.f); }
+
+// ------------------------------------------------------------------------------------------------ layer-1 images
+// The AEV columns that are materialised depend on the species present in the evaluation (GroupInfo::blkmap), so the
+// layer-1 operand images are (re)packed on the device, only when that column set changed since the last call.
+struct TcPackArgs { uint8_t* w1[MAX_S]; uint8_t* w1t[MAX_S]; };
+
+__device__ __forceinline__ unsigned long long tc_colset_key(const GroupInfo* grp) {
+  unsigned long long k = 1ull << 63;
+  for (int b = 0; b < grp->nblk; ++b) k |= 1ull << grp->blkmap[b];
+  return k;
+}
+
+__device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t blk_lo, int r, int kk, const float* x) {
+  uint32_t hi[4], lo[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) split2(x[2 * i], x[2 * i + 1], hi[i], lo[i]);
+  const int eo = tc_elem_off(r, kk);
+  *reinterpret_cast<uint4*>(img + blk_hi + eo) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+  *reinterpret_cast<uint4*>(img + blk_lo + eo) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+}
+
+__global__ void __launch_bounds__(256)
+k_tc_pack_w1(NetTable nets, const GroupInfo* __restrict__ grp, TcPackArgs a, unsigned long long* __restrict__ key) {
+  const unsigned long long want = tc_colset_key(grp);
+  if (key[0] == want) return;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) key[1] = want;
+  const int slot = blockIdx.y;
+  const Net& net = nets.net[slot];
+  if (net.n_layers == 0 || grp->count[slot] == 0) return;
+  const int Kc = grp->Kc, N1 = net.dims[1], Kfull = net.dims[0];
+  const float* __restrict__ W1 = net.W[0];  // [N1][Kfull], internal column order
+  const int nF = N1 * (Kc / 8), nB = Kc * (N1 / 8);
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < nF + nB; idx += gridDim.x * blockDim.x) {
+    float x[8];
+    if (idx < nF) {  // F1 image: B[n][k] = W1[n][col(k)]
+      const int n = idx / (Kc / 8), k = (idx % (Kc / 8)) * 8;
+      const float* src = W1 + (size_t)n * Kfull + grp->blkmap[k >> 5] * BLK + (k & 31);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) x[i] = src[i];
+      const int ch = tc_chunk(N1), c = n / ch, p = k >> 6;
+      tc_store8(a.w1[slot], tc_blk_off(N1, Kc, c, p, 0), tc_blk_off(N1, Kc, c, p, 1), n - c * ch, k & 63, x);
+    } else {         // B1 image: B[n][k] = W1[k][col(n)]
+      const int i2 = idx - nF, n = i2 / (N1 / 8), k = (i2 % (N1 / 8)) * 8;
+      const float* src = W1 + (size_t)k * Kfull + grp->blkmap[n >> 5] * BLK + (n & 31);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) x[i] = src[(size_t)i * Kfull];
+      const int ch = tc_chunk(Kc), c = n / ch, p = k >> 6;
+      tc_store8(a.w1t[slot], tc_blk_off(Kc, N1, c, p, 0), tc_blk_off(Kc, N1, c, p, 1), n - c * ch, k & 63, x);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ the fused kernel
+constexpr int TC_EPI_WARPS = 8;                       // loader / epilogue warps (two per TMEM lane quarter)
+constexpr int TC_THREADS = (TC_EPI_WARPS + 2) * 32;   // + weight producer warp + MMA issuer warp
+constexpr uint32_t TC_PANEL = 16384;                  // 128 rows x 128 B
+constexpr uint32_t TC_LO = 4 * TC_PANEL;              // lo half of the A buffer
+constexpr uint32_t TC_ACC = 256;                      // TMEM column of the 256-column accumulator
+constexpr uint32_t TC_P1 = 0, TC_P2 = 128;            // TMEM columns of the packed CELU' of layers 1 and 2
+
+template <int NPASS> struct TcCfg {
+  static constexpr int NH = (NPASS == 3) ? 2 : 1;
+  static constexpr int NST = (NPASS == 3) ? 3 : 4;
+  static constexpr uint32_t ABUF = NH * 4 * TC_PANEL;
+  static constexpr uint32_t STAGE = NH * TC_PANEL;
+  static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], a_ready, acc_full
+  static constexpr uint32_t TPTR = BARS + (2 * NST + 2) * 8;
+  static constexpr uint32_t EPART = TPTR + 16;
+  static constexpr uint32_t TOTAL = EPART + 128 * 4;
+};
+
+struct TileNet {
+  int N1, N2, N3, Kc;
+  const uint8_t *f1, *w2, *w3, *w3t, *w2t, *b1;
+};
+
+// The six GEMMs of one tile as "rounds": a round reads the A operand resident in shared memory (<= 4 K-panels) and
+// fills <= 256 accumulator columns (<= 2 N-chunks).  F1 is K-streamed in rounds of 4 panels when Kc > 256, B1 is
+// N-streamed in rounds of 2 chunks when Kc > 256.  f(img, N, K, c0, c1, p0, p1, accumulate_onto_previous_round).
+template <class F>
+__device__ __forceinline__ void tc_for_rounds(const TileNet& t, F&& f) {
+  const int np = tc_npanels(t.Kc);
+  for (int p0 = 0; p0 < np; p0 += 4) f(t.f1, t.N1, t.Kc, 0, tc_nchunks(t.N1), p0, min(np, p0 + 4), p0 > 0);
+  f(t.w2, t.N2, t.N1, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N1), false);
+  f(t.w3, t.N3, t.N2, 0, tc_nchunks(t.N3), 0, tc_npanels(t.N2), false);
+  f(t.w3t, t.N2, t.N3, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N3), false);
+  f(t.w2t, t.N1, t.N2, 0, tc_nchunks(t.N1), 0, tc_npanels(t.N2), false);
+  const int nc = tc_nchunks(t.Kc);
+  for (int c0 = 0; c0 < nc; c0 += 2) f(t.b1, t.Kc, t.N1, c0, min(nc, c0 + 2), 0, tc_npanels(t.N1), false);
+}
+
+template <int NPASS>
+__device__ __forceinline__ void tc_store_act(uint32_t abuf, int row, int j, const uint32_t* hi, const uint32_t* lo) {
+  // columns [32j, 32j+32) of `row` -> four 16-byte chunks of K-panel j/2 (conflict-free: chunk XOR row%8)
+  const uint32_t base = abuf + (uint32_t)(j >> 1) * TC_PANEL + (uint32_t)row * 128u;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const uint32_t off = (uint32_t)((((j & 1) * 4 + i) ^ (row & 7)) << 4);
+    sts128(base + off, hi[4 * i], hi[4 * i + 1], hi[4 * i + 2], hi[4 * i + 3]);
+    if (NPASS == 3) sts128(base + TC_LO + off, lo[4 * i], lo[4 * i + 1], lo[4 * i + 2], lo[4 * i + 3]);
+  }
+}
+
+template <int NPASS>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict__ grp,
+         const TileInfo* __restrict__ tiles, const float* __restrict__ aev, float* __restrict__ daev,
+         float* __restrict__ e_atom, unsigned long long* __restrict__ key) {
+  using C = TcCfg<NPASS>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t abuf = sbase, stage0 = sbase + C::ABUF;
+  const uint32_t bar_full = sbase + C::BARS, bar_empty = bar_full + 8 * C::NST;
+  const uint32_t bar_aready = bar_empty + 8 * C::NST, bar_acc = bar_aready + 8;
+  volatile uint32_t* tptr = reinterpret_cast<volatile uint32_t*>(smem + C::TPTR);
+  float* e_part = reinterpret_cast<float*>(smem + C::EPART);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_tiles = grp->n_tiles, Kc = grp->Kc;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < C::NST; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
+    mbar_init(bar_aready, TC_EPI_WARPS * 32);
+    mbar_init(bar_acc, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == TC_EPI_WARPS + 1) {  // the MMA warp owns the TMEM allocation (all 512 columns; one CTA per SM)
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + C::TPTR), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tptr;
+
+  auto tile_net = [&](int t, TileInfo& ti, TileNet& tn) {
+    ti = tiles[t];
+    const Net& net = nets.net[ti.slot];
+    tn.N1 = net.dims[1]; tn.N2 = net.dims[2]; tn.N3 = net.dims[3]; tn.Kc = Kc;
+    tn.f1 = w1.w1[ti.slot]; tn.b1 = w1.w1t[ti.slot];
+    tn.w2 = tab.n[ti.slot].w2; tn.w3 = tab.n[ti.slot].w3; tn.w3t = tab.n[ti.slot].w3t; tn.w2t = tab.n[ti.slot].w2t;
+  };
+
+  if (warp == TC_EPI_WARPS) {
+    // ===== weight producer: streams every B block of every round, in order, through the stage ring =====
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        TileInfo ti; TileNet tn; tile_net(t, ti, tn);
+        tc_for_rounds(tn, [&](const uint8_t* img, int N, int K, int c0, int c1, int p0, int p1, bool) {
+          const int ch = tc_chunk(N);
+          for (int c = c0; c < c1; ++c) {
+            const uint32_t bytes = (uint32_t)min(ch, N - c * ch) * 128u;
+            for (int p = p0; p < p1; ++p) {
+              mbar_wait(bar_empty + 8 * s, ph ^ 1);
+              mbar_expect_tx(bar_full + 8 * s, bytes * C::NH);
+              bulk_g2s(stage0 + s * C::STAGE, img + tc_blk_off(N, K, c, p, 0), bytes, bar_full + 8 * s);
+              if (C::NH == 2) bulk_g2s(stage0 + s * C::STAGE + TC_PANEL, img + tc_blk_off(N, K, c, p, 1), bytes, bar_full + 8 * s);
+              if (++s == C::NST) { s = 0; ph ^= 1; }
+            }
+          }
+        });
+      }
+    }
+  } else if (warp == TC_EPI_WARPS + 1) {
+    // ===== MMA issuer: one thread =====
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0, aph = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        TileInfo ti; TileNet tn; tile_net(t, ti, tn);
+        tc_for_rounds(tn, [&](const uint8_t*, int N, int K, int c0, int c1, int p0, int p1, bool acc_first) {
+          mbar_wait(bar_aready, aph); aph ^= 1;   // A operand in place, accumulator columns drained
+          tc_fence_after();
+          const int ch = tc_chunk(N);
+          for (int c = c0; c < c1; ++c) {
+            const int rows = min(ch, N - c * ch);
+            const uint32_t idesc = tc_idesc(rows), d = tmem + TC_ACC + (uint32_t)((c - c0) * ch);
+            for (int p = p0; p < p1; ++p) {
+              mbar_wait(bar_full + 8 * s, ph);
+              tc_fence_after();
+              const int nks = min(4, (K - p * 64) >> 4);
+              const uint32_t a0 = abuf + (uint32_t)(p - p0) * TC_PANEL, b0 = stage0 + s * C::STAGE;
+              for (int ks = 0; ks < nks; ++ks) {
+                const uint64_t ah = tc_desc(a0 + ks * 32), bh = tc_desc(b0 + ks * 32);
+                tc_mma(d, ah, bh, idesc, (acc_first || p > p0 || ks > 0) ? 1u : 0u);
+                if (NPASS == 3) {
+                  tc_mma(d, tc_desc(a0 + TC_LO + ks * 32), bh, idesc, 1u);
+                  tc_mma(d, ah, tc_desc(b0 + TC_PANEL + ks * 32), idesc, 1u);
+                }
+              }
+              tc_commit(bar_empty + 8 * s);       // frees the stage when these MMAs have read it
+              if (++s == C::NST) { s = 0; ph ^= 1; }
+            }
+          }
+          tc_commit(bar_acc);                      // accumulator complete (and the A operand no longer read)
+        });
+      }
+    }
+  } else {
+    // ===== loader / epilogue warps: thread <-> tile row (TMEM lane); warps w and w+4 split the 32-column chunks =====
+    const int q = warp & 3, hf = warp >> 2, row = q * 32 + lane;
+    const uint32_t tlane = tmem + ((uint32_t)(q * 32) << 16);
+    uint32_t fph = 0;
+    auto signal_and_wait = [&]() {
+      tc_fence_before();
+      fence_proxy_async();
+      mbar_arrive(bar_aready);
+      mbar_wait(bar_acc, fph); fph ^= 1;
+      tc_fence_after();
+    };
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      TileInfo ti; TileNet tn; tile_net(t, ti, tn);
+      const Net& net = nets.net[ti.slot];
+      const float alpha = net.alpha, kexp = 1.4426950408889634f / alpha;
+      const bool valid = row < ti.nvalid;
+      // ---- F1 rounds: AEV columns [64 p0, 64 p1) -> fp16 hi/lo panels
+      const int np = tc_npanels(Kc);
+      for (int p0 = 0; p0 < np; p0 += 4) {
+        const int k0 = p0 * 64, kw = min(Kc, k0 + 256) - k0, n16 = kw >> 3;
+        for (int idx = threadIdx.x; idx < 128 * n16; idx += TC_EPI_WARPS * 32) {
+          const int r = idx / n16, chn = idx - r * n16;
+          float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
+          if (r < ti.nvalid) {
+            const float4* src = reinterpret_cast<const float4*>(aev + (size_t)(ti.row0 + r) * Kc + k0 + chn * 8);
+            x0 = __ldg(src); x1 = __ldg(src + 1);
+          }
+          uint32_t hi[4], lo[4];
+          split2(x0.x, x0.y, hi[0], lo[0]); split2(x0.z, x0.w, hi[1], lo[1]);
+          split2(x1.x, x1.y, hi[2], lo[2]); split2(x1.z, x1.w, hi[3], lo[3]);
+          const uint32_t dst = abuf + (uint32_t)(chn >> 3) * TC_PANEL + (uint32_t)r * 128u + (uint32_t)(((chn & 7) ^ (r & 7)) << 4);
+          sts128(dst, hi[0], hi[1], hi[2], hi[3]);
+          if (NPASS == 3) sts128(dst + TC_LO, lo[0], lo[1], lo[2], lo[3]);
+        }
+        signal_and_wait();
+      }
+      // ---- forward hidden layers 1, 2: h = CELU(z + b) -> A operand of the next layer; CELU' packed into TMEM
+#pragma unroll 1
+      for (int l = 1; l <= 2; ++l) {
+        const int N = (l == 1) ? tn.N1 : tn.N2;
+        const float* __restrict__ bias = net.b[l - 1];
+        const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
+#pragma unroll 1
+        for (int j = hf; j * 32 < N; j += 2) {
+          uint32_t v[32], hi[16], lo[16], cp[16];
+          tmem_ld32(tlane + TC_ACC + j * 32, v);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; i += 2) {
+            const float z0 = __uint_as_float(v[i]) + __ldg(bias + j * 32 + i);
+            const float z1 = __uint_as_float(v[i + 1]) + __ldg(bias + j * 32 + i + 1);
+            const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
+            const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
+            cp[i >> 1] = pack_c(z0 > 0.f ? 1.f : e0, z1 > 0.f ? 1.f : e1);
+            split2(h0, h1, hi[i >> 1], lo[i >> 1]);
+          }
+          tmem_st16(tlane + pcol + j * 16, cp);
+          tc_store_act<NPASS>(abuf, row, j, hi, lo);
+        }
+        tmem_wait_st();
+        signal_and_wait();
+      }
+      // ---- layer 3 + output layer: E_i = h3 . w4 + b4;  dl3 = w4 * CELU'(z3) -> A operand of B3
+      {
+        const int nl = net.n_layers;
+        const float* __restrict__ bias = net.b[2];
+        const float* __restrict__ w4 = net.W[nl - 1];
+        float e = 0.f;
+#pragma unroll 1
+        for (int j = hf; j * 32 < tn.N3; j += 2) {
+          uint32_t v[32], hi[16], lo[16];
+          tmem_ld32(tlane + TC_ACC + j * 32, v);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; i += 2) {
+            const float z0 = __uint_as_float(v[i]) + __ldg(bias + j * 32 + i);
+            const float z1 = __uint_as_float(v[i + 1]) + __ldg(bias + j * 32 + i + 1);
+            const float wa = __ldg(w4 + j * 32 + i), wb = __ldg(w4 + j * 32 + i + 1);
+            const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
+            const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
+            e = fmaf(h0, wa, e); e = fmaf(h1, wb, e);
+            split2(wa * (z0 > 0.f ? 1.f : e0), wb * (z1 > 0.f ? 1.f : e1), hi[i >> 1], lo[i >> 1]);
+          }
+          tc_store_act<NPASS>(abuf, row, j, hi, lo);
+        }
+        if (hf == 1) e_part[row] = e;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (hf == 0) e_atom[ti.row0 + row] = valid ? (e + e_part[row]) + __ldg(net.b[nl - 1]) : 0.f;
+        signal_and_wait();
+      }
+      // ---- backward through layers 2, 1: dl_l = d_l * CELU'(z_l) -> A operand of the next backward GEMM
+#pragma unroll 1
+      for (int l = 2; l >= 1; --l) {
+        const int N = (l == 1) ? tn.N1 : tn.N2;
+        const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
+#pragma unroll 1
+        for (int j = hf; j * 32 < N; j += 2) {
+          uint32_t v[32], cp[16], hi[16], lo[16];
+          tmem_ld32(tlane + TC_ACC + j * 32, v);
+          tmem_ld16(tlane + pcol + j * 16, cp);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; i += 2)
+            split2(__uint_as_float(v[i]) * unpack_c_lo(cp[i >> 1]), __uint_as_float(v[i + 1]) * unpack_c_hi(cp[i >> 1]),
+                   hi[i >> 1], lo[i >> 1]);
+          tc_store_act<NPASS>(abuf, row, j, hi, lo);
+        }
+        signal_and_wait();
+      }
+      // ---- B1 rounds: g = dE/dAEV columns [n0, n0 + ncols) -> global (fp32, compacted AEV column order)
+      {
+        const int nc = tc_nchunks(Kc), ch = tc_chunk(Kc);
+        for (int c0 = 0; c0 < nc; c0 += 2) {
+          const int n0 = c0 * ch, ncols = min(Kc, (c0 + 2) * ch) - n0;
+          float* __restrict__ dst = daev + (size_t)(ti.row0 + row) * Kc + n0;
+#pragma unroll 1
+          for (int j = hf; j * 32 < ncols; j += 2) {
+            uint32_t v[32];
+            tmem_ld32(tlane + TC_ACC + j * 32, v);
+            tmem_wait_ld();
+            if (valid) {
+#pragma unroll
+              for (int i = 0; i < 32; i += 4)
+                *reinterpret_cast<uint4*>(dst + j * 32 + i) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+            }
+          }
+          if (c0 + 2 < nc) signal_and_wait();
+        }
+        // the first round of the next tile re-arms through its own signal_and_wait (program order: loads above done)
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (blockIdx.x == 0 && threadIdx.x == 0) key[0] = key[1];
+  if (warp == TC_EPI_WARPS + 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+namespace {
+void host_split(float x, uint16_t& hi, uint16_t& lo) {
+  const __half h = __float2half_rn(x);
+  const __half l = __float2half_rn(x - __half2float(h));
+  memcpy(&hi, &h, 2); memcpy(&lo, &l, 2);
+}
+// image of B[n][k] = get(n, k), n < N, k < K
+template <class G>
+void host_image(std::vector<uint8_t>& blob, size_t base, int N, int K, G get) {
+  const int ch = tc_chunk(N);
+  for (int n = 0; n < N; ++n)
+    for (int k = 0; k < K; ++k) {
+      uint16_t hi, lo;
+      host_split(get(n, k), hi, lo);
+      const int c = n / ch, p = k >> 6, eo = tc_elem_off(n - c * ch, k & 63);
+      memcpy(&blob[base + tc_blk_off(N, K, c, p, 0) + eo], &hi, 2);
+      memcpy(&blob[base + tc_blk_off(N, K, c, p, 1) + eo], &lo, 2);
+    }
+}
+bool tc_shape_ok(const nnp_mlp_desc& d) {
+  if (d.n_layers != 4) return false;
+  for (int l = 1; l <= 3; ++l)
+    if (d.dims[l] % 32 || d.dims[l] < 32 || d.dims[l] > 256) return false;
+  for (int l = 0; l < 4; ++l)
+    for (size_t i = 0; i < (size_t)d.dims[l] * d.dims[l + 1]; ++i)
+      if (!(fabsf(d.W[l][i]) < 6.0e4f)) return false;  // fp16 range of the hi part
+  return true;
+}
+}  // namespace
+
+int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets) {
+  m->tc = nullptr;
+  const int S = m->aev.S;
+  size_t total = 0;
+  size_t off[MAX_S][4];
+  for (int s = 0; s < S; ++s) {
+    const nnp_mlp_desc& d = nets[s];
+    if (d.n_layers == 0) continue;
+    if (!tc_shape_ok(d)) return NNP_OK;  // no tensor-core image: workspaces stay in NNP_MLP_FP32_SIMT
+    const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
+    const size_t sz[4] = {tc_img_bytes(N2, N1), tc_img_bytes(N3, N2), tc_img_bytes(N2, N3), tc_img_bytes(N1, N2)};
+    for (int i = 0; i < 4; ++i) { off[s][i] = total; total += (sz[i] + 1023) & ~(size_t)1023; }
+  }
+  std::vector<uint8_t> blob(total, 0);
+  for (int s = 0; s < S; ++s) {
+    const nnp_mlp_desc& d = nets[s];
+    if (d.n_layers == 0) continue;
+    const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
+    const float *W2 = d.W[1], *W3 = d.W[2];  // [out][in]
+    host_image(blob, off[s][0], N2, N1, [&](int n, int k) { return W2[(size_t)n * N1 + k]; });  // F2: B = W2
+    host_image(blob, off[s][1], N3, N2, [&](int n, int k) { return W3[(size_t)n * N2 + k]; });  // F3: B = W3
+    host_image(blob, off[s][2], N2, N3, [&](int n, int k) { return W3[(size_t)k * N2 + n]; });  // B3: B = W3^T
+    host_image(blob, off[s][3], N1, N2, [&](int n, int k) { return W2[(size_t)k * N1 + n]; });  // B2: B = W2^T
+  }
+  TcModel* tm = new (std::nothrow) TcModel();
+  if (!tm) return NNP_ERR_CUDA;
+  memset(tm, 0, sizeof(*tm));
+  if (cudaMalloc(&tm->blob, std::max<size_t>(total, 1024)) != cudaSuccess ||
+      cudaMemcpy(tm->blob, blob.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError();
+    if (tm->blob) cudaFree(tm->blob);
+    delete tm;
+    return NNP_ERR_CUDA;
+  }
+  for (int s = 0; s < S; ++s) {
+    if (nets[s].n_layers == 0) continue;
+    const uint8_t* b = static_cast<const uint8_t*>(tm->blob);
+    tm->tab.n[s] = TcNetImg{b + off[s][0], b + off[s][1], b + off[s][2], b + off[s][3]};
+  }
+  m->tc = tm;
+  return NNP_OK;
+}
+
+void tc_model_destroy(nnp_model* m) {
+  TcModel* tm = static_cast<TcModel*>(m->tc);
+  if (!tm) return;
+  if (tm->blob) cudaFree(tm->blob);
+  delete tm;
+  m->tc = nullptr;
+}
+
+int tc_workspace_create(nnp_workspace* ws) {
+  ws->tc_ws = nullptr;
+  const nnp_model* m = ws->model;
+  if (!m->tc) return NNP_OK;
+  TcWorkspace* tw = new (std::nothrow) TcWorkspace();
+  if (!tw) return NNP_ERR_CUDA;
+  memset(tw, 0, sizeof(*tw));
+  ws->tc_ws = tw;
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return NNP_ERR_CUDA;
+  tw->num_sms = prop.multiProcessorCount;
+  tw->smem_bytes[0] = (int)TcCfg<3>::TOTAL;
+  tw->smem_bytes[1] = (int)TcCfg<1>::TOTAL;
+  if (cudaFuncSetAttribute(k_mlp_tc<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tw->smem_bytes[0]) != cudaSuccess ||
+      cudaFuncSetAttribute(k_mlp_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tw->smem_bytes[1]) != cudaSuccess)
+    return NNP_ERR_CUDA;
+  for (int s = 0; s < m->aev.S; ++s) {
+    const Net& n = m->nets.net[s];
+    if (n.n_layers == 0) continue;
+    const size_t b1 = tc_img_bytes(n.dims[1], m->Kfull), b2 = tc_img_bytes(m->Kfull, n.dims[1]);
+    if (cudaMalloc(&tw->w1img[s], b1) != cudaSuccess || cudaMalloc(&tw->w1timg[s], b2) != cudaSuccess) return NNP_ERR_CUDA;
+    cudaMemset(tw->w1img[s], 0, b1);
+    cudaMemset(tw->w1timg[s], 0, b2);
+  }
+  if (cudaMalloc(&tw->key, 2 * sizeof(unsigned long long)) != cudaSuccess) return NNP_ERR_CUDA;
+  cudaMemset(tw->key, 0, 2 * sizeof(unsigned long long));
+  return NNP_OK;
+}
+
+void tc_workspace_destroy(nnp_workspace* ws) {
+  TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
+  if (!tw) return;
+  for (int s = 0; s < MAX_S; ++s) {
+    if (tw->w1img[s]) cudaFree(tw->w1img[s]);
+    if (tw->w1timg[s]) cudaFree(tw->w1timg[s]);
+  }
+  if (tw->key) cudaFree(tw->key);
+  cudaGetLastError();
+  delete tw;
+  ws->tc_ws = nullptr;
+}
+
+int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
+  if (n_ml <= 0) return 0;
+  const nnp_model* m = ws->model;
+  TcModel* tm = static_cast<TcModel*>(m->tc);
+  TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
+  if (!tm || !tw) return launch_mlp_simt(ws, n_ml);
+  TcPackArgs pa;
+  for (int s = 0; s < MAX_S; ++s) { pa.w1[s] = tw->w1img[s]; pa.w1t[s] = tw->w1timg[s]; }
+  k_tc_pack_w1<<<dim3(64, m->aev.S), 256, 0, ws->stream>>>(m->nets, ws->groups, pa, tw->key);
+  const int grid = std::min(ws->max_tiles, tw->num_sms);
+  if (ws->mlp_mode == NNP_MLP_F16X1)
+    k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(m->nets, tm->tab, pa, ws->groups, ws->tiles, ws->aev,
+                                                                     ws->daev, ws->e_atom, tw->key);
+  else
+    k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(m->nets, tm->tab, pa, ws->groups, ws->tiles, ws->aev,
+                                                                     ws->daev, ws->e_atom, tw->key);
+  return 2;
+}
+
 }  // namespace nnp

@@ -83,9 +83,9 @@ def test_config_small(k):
     assert np.abs(ea - ref["e_atom"]).max() <= 1e-4
     check_EF(Eg, Fg, ref, n)
     assert abs(Fg.sum(0)).max() < 1e-3
-    # every MLP arithmetic mode the library offers must meet the bar (BF16X1 is ladder-only, excluded)
+    # every MLP arithmetic mode the library offers must meet the bar (F16X1 is ladder-only, excluded)
     import paper_2604_21441_b200 as nnp
-    for mode in (nnp.NNP_MLP_FP32_SIMT, nnp.NNP_MLP_BF16X3):
+    for mode in (nnp.NNP_MLP_FP32_SIMT, nnp.NNP_MLP_F16X3):
         if nnp.nnp_workspace_set_mlp_mode(ws.handle, mode) != 0:
             continue
         Eg2, Fg2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
