@@ -133,7 +133,7 @@ def run_ours(args, rank, world, local_rank):
     model = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
     ws = nnp.Workspace(model, n)
     if args.mlp_mode != "default":
-        ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "f16x3": nnp.NNP_MLP_F16X3}[args.mlp_mode])
+        ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "f16x3": nnp.NNP_MLP_F16X3, "f16x1": nnp.NNP_MLP_F16X1}[args.mlp_mode])
     dpos = [torch.from_numpy(P[t]).cuda() for t in range(N_POS_SETS)]
     dZ = torch.from_numpy(cfg["Z"]).cuda()
     E = torch.zeros(1, dtype=torch.float64, device="cuda")
@@ -265,7 +265,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3"])
+    ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
