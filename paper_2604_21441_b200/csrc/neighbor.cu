@@ -151,15 +151,17 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
   __syncthreads();
   if (threadIdx.x <= S) gs[threadIdx.x] = bstart[threadIdx.x * g->ncell];
   __syncthreads();
+  __shared__ int pshift[MAX_S];
   if (threadIdx.x == 0) {
-    int rows = 0, nt = 0;
+    int rows = 0, nt = 0, cnt[MAX_S];
     for (int q = 0; q < MAX_S; ++q) {
-      int cnt = (q < S) ? gs[q + 1] - gs[q] : 0;
-      grp->count[q] = cnt;
+      cnt[q] = (q < S) ? gs[q + 1] - gs[q] : 0;
+      grp->count[q] = cnt[q];
       grp->start[q] = (q < S) ? gs[q] : n_ml;
-      grp->pad_shift[q] = rows - ((q < S) ? gs[q] : 0);
+      pshift[q] = rows - ((q < S) ? gs[q] : 0);
+      grp->pad_shift[q] = pshift[q];
       tb[q] = nt;
-      int t = (cnt + TILE_M - 1) / TILE_M;
+      int t = (cnt[q] + TILE_M - 1) / TILE_M;
       nt += t; rows += t * TILE_M;
     }
     grp->start[MAX_S] = n_ml;
@@ -171,14 +173,14 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
     const int nRB = (S + 1) / 2;
     int nb = 0;
     for (int b = 0; b < nRB; ++b) {
-      bool on = dense_k || grp->count[2 * b] > 0 || (2 * b + 1 < S && grp->count[2 * b + 1] > 0);
+      bool on = dense_k || cnt[2 * b] > 0 || (2 * b + 1 < S && cnt[2 * b + 1] > 0);
       grp->cpos[b] = on ? nb : -1;
       if (on) grp->blkmap[nb++] = b;
     }
     int p = 0;
     for (int s1 = 0; s1 < S; ++s1)
       for (int s2 = s1; s2 < S; ++s2, ++p) {
-        bool on = dense_k || (grp->count[s1] > 0 && grp->count[s2] > 0);
+        bool on = dense_k || (cnt[s1] > 0 && cnt[s2] > 0);
         grp->cpos[nRB + p] = on ? nb : -1;
         if (on) grp->blkmap[nb++] = nRB + p;
       }
@@ -195,7 +197,7 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
     int r = t - tb[q];
     int cnt = gs[min(q + 1, S)] - gs[min(q, S)];
     TileInfo ti;
-    ti.slot = q; ti.row0 = grp->pad_shift[q] + gs[q] + r * TILE_M; ti.nvalid = min(TILE_M, cnt - r * TILE_M); ti.pad = 0;
+    ti.slot = q; ti.row0 = pshift[q] + gs[q] + r * TILE_M; ti.nvalid = min(TILE_M, cnt - r * TILE_M); ti.pad = 0;
     tiles[t] = ti;
   }
 }
@@ -216,18 +218,30 @@ __global__ void k_scatter(const GridInfo* __restrict__ g, const float4* __restri
 }
 
 // K1c: the atomic ranks above are not reproducible; order every bucket by ML index so that the sorted order
-// (and with it every summation order downstream) is identical from run to run.
-__global__ void k_bucket_sort(const GridInfo* __restrict__ g, int S, const int* __restrict__ bstart,
-                              float4* __restrict__ spos) {
-  int k = blockIdx.x * blockDim.x + threadIdx.x;
+// (and with it every summation order downstream) is identical from run to run.  One warp per bucket: buckets of
+// <= 32 atoms are ranked by counting (all-pairs compare through shuffles); longer ones fall back to one lane.
+__global__ void __launch_bounds__(256) k_bucket_sort(const GridInfo* __restrict__ g, int S,
+                                                     const int* __restrict__ bstart, float4* __restrict__ spos) {
+  const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= S * g->ncell) return;
-  int lo = bstart[k], hi = bstart[k + 1];
-  for (int p = lo + 1; p < hi; ++p) {
-    float4 v = spos[p];
-    int key = __float_as_int(v.w) & 0x0fffffff;
-    int q = p - 1;
-    while (q >= lo && (__float_as_int(spos[q].w) & 0x0fffffff) > key) { spos[q + 1] = spos[q]; --q; }
-    spos[q + 1] = v;
+  const int lo = bstart[k], n = bstart[k + 1] - lo;
+  if (n <= 1) return;
+  if (n <= 32) {
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    int key = 0x7fffffff;
+    if (lane < n) { v = spos[lo + lane]; key = __float_as_int(v.w) & 0x0fffffff; }
+    int rank = 0;
+    for (int o = 0; o < n; ++o) rank += (__shfl_sync(0xffffffffu, key, o) < key) ? 1 : 0;
+    __syncwarp();
+    if (lane < n) spos[lo + rank] = v;   // keys (ML indices) are distinct: ranks are a permutation
+  } else if (lane == 0) {
+    for (int p = lo + 1; p < lo + n; ++p) {
+      float4 v = spos[p];
+      int key = __float_as_int(v.w) & 0x0fffffff;
+      int q = p - 1;
+      while (q >= lo && (__float_as_int(spos[q].w) & 0x0fffffff) > key) { spos[q + 1] = spos[q]; --q; }
+      spos[q + 1] = v;
+    }
   }
 }
 
@@ -245,103 +259,144 @@ __device__ __forceinline__ double exact_d2(const float* __restrict__ pos, int oi
 
 constexpr float GUARD_BAND = 2.0e-3f;  // Angstrom^2; >> fp32 error of d2 (~1e-5), reading #6
 
+constexpr int NB_CAP = 1024;            // candidates staged in shared memory per chunk
+constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of one centre cell
+
+// One block per cell.  The atoms of the 27 neighbouring cells (per species: 27 buckets of the slot-major sort) are
+// staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
+// cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
+// warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
 __global__ void __launch_bounds__(256) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
-                                                   const float4* __restrict__ spos, const int* __restrict__ scell,
+                                                   const float4* __restrict__ spos,
                                                    const int* __restrict__ bstart, const float* __restrict__ pos,
                                                    const int32_t* __restrict__ ml, int n_ml, int rcap, int acap,
                                                    uint32_t* __restrict__ nbrR, uint8_t* __restrict__ nbrA,
                                                    int* __restrict__ cntR, int* __restrict__ cntA,
                                                    int* __restrict__ flags) {
-  const int lane = threadIdx.x & 31;
-  const int ip = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (ip >= n_ml) return;
-  const float4 ci = spos[ip];
-  const int cell = scell[ip];
-  const int nc0 = g->nc[0], nc1 = g->nc[1], nc2 = g->nc[2], ncell = g->ncell, pbc = g->pbc;
+  __shared__ float4 cand[NB_CAP];
+  __shared__ int segStart[NB_SEG], segOff[NB_SEG + 1], segCode[NB_SEG];
+  __shared__ int cenStart[MAX_S], cenOff[MAX_S + 1];
+  __shared__ int wsum[8];
+  const int cell = blockIdx.x, ncell = g->ncell;
+  if (cell >= ncell) return;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nc0 = g->nc[0], nc1 = g->nc[1], nc2 = g->nc[2], pbc = g->pbc, S = c.S;
   const int cz = cell % nc2, cy = (cell / nc2) % nc1, cx = cell / (nc1 * nc2);
   const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
-  const int a_i = __float_as_int(ci.w) & 0x0fffffff;
-  const int o_i = ml ? ml[a_i] : a_i;
-  uint32_t* rowR = nbrR + (size_t)ip * rcap;
-  uint8_t* rowA = nbrA + (size_t)ip * acap;
-  int nR = 0, nA = 0, bad = 0;
+
+  // ---- centres of this cell (one bucket per species)
+  if (tid == 0) {
+    int run = 0;
+    for (int s = 0; s < MAX_S; ++s) {
+      int b0 = 0, n = 0;
+      if (s < S) { b0 = bstart[s * ncell + cell]; n = bstart[s * ncell + cell + 1] - b0; }
+      cenStart[s] = b0; cenOff[s] = run; run += n;
+    }
+    cenOff[MAX_S] = run;
+  }
+  // ---- segment table: thread t <-> (species, neighbour cell offset)
+  int len = 0, b0 = 0, code = 0;
+  if (tid < S * 27) {
+    const int s = tid / 27, r = tid - 27 * s;
+    const int ox = r / 9 - 1, oy = (r / 3) % 3 - 1, oz = r % 3 - 1;
+    bool ok = true;
+    int nx = cx + ox, ny = cy + oy, nz = cz + oz;
+    if (nc0 == 1) ok &= (ox == 0); else if (nx < 0 || nx >= nc0) { if (pbc) nx += (nx < 0) ? nc0 : -nc0; else ok = false; }
+    if (nc1 == 1) ok &= (oy == 0); else if (ny < 0 || ny >= nc1) { if (pbc) ny += (ny < 0) ? nc1 : -nc1; else ok = false; }
+    if (nc2 == 1) ok &= (oz == 0); else if (nz < 0 || nz >= nc2) { if (pbc) nz += (nz < 0) ? nc2 : -nc2; else ok = false; }
+    if (ok) {
+      const int k = s * ncell + (nx * nc1 + ny) * nc2 + nz;
+      b0 = bstart[k]; len = bstart[k + 1] - b0;
+      code = (ox + 1) | ((oy + 1) << 2) | ((oz + 1) << 4);
+    }
+  }
+  int incl = len;
+  for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+  if (lane == 31) wsum[warp] = incl;
+  __syncthreads();
+  int base = 0;
+  for (int w = 0; w < warp; ++w) base += wsum[w];
+  if (tid < NB_SEG) { segStart[tid] = b0; segOff[tid] = base + incl - len; segCode[tid] = code; }
+  int total = 0;
+  for (int w = 0; w < 8; ++w) total += wsum[w];
+  if (tid == 0) segOff[NB_SEG] = total;
+  __syncthreads();
+  const int nC = cenOff[MAX_S];
+  if (nC == 0) return;
   const unsigned lt = lanemask_lt();
-  // offsets per dimension: one cell => {0}; otherwise {-1,0,1} (wrapped if periodic, clipped if open)
-  const int nox = (nc0 == 1) ? 1 : 3, noy = (nc1 == 1) ? 1 : 3, noz = (nc2 == 1) ? 1 : 3;
-  for (int s = 0; s < c.S; ++s) {
-    if (grp->count[s] == 0) continue;
-    const int* bs = bstart + s * ncell;
-    for (int ix = 0; ix < nox; ++ix) {
-      int ox = (nox == 1) ? 0 : ix - 1;
-      int nx = cx + ox;
-      if (nx < 0 || nx >= nc0) { if (!pbc) continue; nx += (nx < 0) ? nc0 : -nc0; }
-      for (int iy = 0; iy < noy; ++iy) {
-        int oy = (noy == 1) ? 0 : iy - 1;
-        int ny = cy + oy;
-        if (ny < 0 || ny >= nc1) { if (!pbc) continue; ny += (ny < 0) ? nc1 : -nc1; }
-        // up to three z segments flattened into one candidate list
-        int segS[3], segL[3], segO[3], nseg = 0, total = 0;
-        for (int iz = 0; iz < noz; ++iz) {
-          int oz = (noz == 1) ? 0 : iz - 1;
-          int nz = cz + oz;
-          if (nz < 0 || nz >= nc2) { if (!pbc) continue; nz += (nz < 0) ? nc2 : -nc2; }
-          int k = (nx * nc1 + ny) * nc2 + nz;
-          int b0 = bs[k], b1 = bs[k + 1];
-          segS[nseg] = b0; segL[nseg] = b1 - b0; segO[nseg] = oz; total += b1 - b0; ++nseg;
-        }
-        for (int q0 = 0; q0 < total; q0 += 32) {
-          int q = q0 + lane;
-          bool valid = q < total;
-          int jp = 0, oz = 0;
-          if (valid) {
-            int r = q;
-            int sg = 0;
-            if (nseg > 1 && r >= segL[0]) { r -= segL[0]; sg = 1; if (nseg > 2 && r >= segL[1]) { r -= segL[1]; sg = 2; } }
-            jp = segS[sg] + r; oz = segO[sg];
-          }
-          bool inR = false, inA = false;
-          int cox = ox, coy = oy, coz = oz;
-          if (valid && jp != ip) {
-            float4 pj = spos[jp];
-            float dx = pj.x - ci.x, dy = pj.y - ci.y, dz = pj.z - ci.z;
-            if (nc0 == 1) { cox = pbc ? -(int)rintf(dx / ex) : 0; }
-            if (nc1 == 1) { coy = pbc ? -(int)rintf(dy / ey) : 0; }
-            if (nc2 == 1) { coz = pbc ? -(int)rintf(dz / ez) : 0; }
-            dx += (float)cox * ex; dy += (float)coy * ey; dz += (float)coz * ez;
-            float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (d2 < c.Rcr2 + GUARD_BAND) {
-              bool nearR = fabsf(d2 - c.Rcr2) <= GUARD_BAND, nearA = fabsf(d2 - c.Rca2) <= GUARD_BAND;
-              inR = !nearR;
-              inA = d2 < c.Rca2;
-              if (nearR || nearA || d2 < 1e-6f) {
-                int a_j = __float_as_int(pj.w) & 0x0fffffff;
-                int o_j = ml ? ml[a_j] : a_j;
-                double e2 = exact_d2(pos, o_i, o_j, g);
-                if (nearR) inR = e2 <= c.Rcr2_d;
-                if (nearA) inA = e2 <= c.Rca2_d;
-                if (e2 == 0.0) bad |= FLAG_COINCIDENT;
-              }
+  int bad = 0;
+
+  for (int chunk0 = 0; chunk0 < total; chunk0 += NB_CAP) {
+    const int nin = min(NB_CAP, total - chunk0);
+    if (chunk0 > 0) __syncthreads();
+    // ---- stage the candidates of this chunk, shifted into the centre cell's frame
+    for (int idx = tid; idx < nin; idx += 256) {
+      const int gq = chunk0 + idx;
+      int lo = 0, hi = NB_SEG - 1;            // last segment with segOff <= gq
+      while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (segOff[mid] <= gq) lo = mid; else hi = mid - 1; }
+      const int jp = segStart[lo] + (gq - segOff[lo]), cd = segCode[lo];
+      float4 pj = spos[jp];
+      pj.x += (float)((cd & 3) - 1) * ex; pj.y += (float)(((cd >> 2) & 3) - 1) * ey; pj.z += (float)(((cd >> 4) & 3) - 1) * ez;
+      const int a_j = __float_as_int(pj.w) & 0x0fffffff;
+      pj.w = __int_as_float(jp | (cd << JBITS));
+      cand[idx] = pj;
+      (void)a_j;
+    }
+    __syncthreads();
+    // ---- sweep: one warp per centre
+    for (int ci = warp; ci < nC; ci += 8) {
+      int s = 0;
+      while (s + 1 < MAX_S && ci >= cenOff[s + 1]) ++s;
+      const int ip = cenStart[s] + (ci - cenOff[s]);
+      const float4 pi = spos[ip];
+      const int a_i = __float_as_int(pi.w) & 0x0fffffff;
+      const int o_i = ml ? ml[a_i] : a_i;
+      uint32_t* rowR = nbrR + (size_t)ip * rcap;
+      uint8_t* rowA = nbrA + (size_t)ip * acap;
+      int nR = 0, nA = 0;
+      if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; }
+      for (int q0 = 0; q0 < nin; q0 += 32) {
+        const int q = q0 + lane;
+        bool inR = false, inA = false;
+        uint32_t ent = 0;
+        if (q < nin) {
+          const float4 pj = cand[q];
+          ent = (uint32_t)__float_as_int(pj.w);
+          const int jp = (int)(ent & JMASK);
+          float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+          if (nc0 == 1 && pbc) { const int o = -(int)rintf(dx / ex); dx += (float)o * ex; ent += (uint32_t)o << JBITS; }
+          if (nc1 == 1 && pbc) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
+          if (nc2 == 1 && pbc) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
+          const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+          if (jp != ip && d2 < c.Rcr2 + GUARD_BAND) {
+            const bool nearR = fabsf(d2 - c.Rcr2) <= GUARD_BAND, nearA = fabsf(d2 - c.Rca2) <= GUARD_BAND;
+            inR = !nearR;
+            inA = d2 < c.Rca2;
+            if (nearR || nearA || d2 < 1e-6f) {
+              const int a_j = __float_as_int(spos[jp].w) & 0x0fffffff;
+              const int o_j = ml ? ml[a_j] : a_j;
+              const double e2 = exact_d2(pos, o_i, o_j, g);
+              if (nearR) inR = e2 <= c.Rcr2_d;
+              if (nearA) inA = e2 <= c.Rca2_d;
+              if (e2 == 0.0) bad |= FLAG_COINCIDENT;
             }
           }
-          unsigned mR = __ballot_sync(0xffffffffu, inR);
-          unsigned mA = __ballot_sync(0xffffffffu, inA);
-          int pR = nR + __popc(mR & lt);
-          if (inR) {
-            if (pR < rcap) rowR[pR] = (uint32_t)jp | ((uint32_t)((cox + 1) | ((coy + 1) << 2) | ((coz + 1) << 4)) << JBITS);
-            else bad |= FLAG_CAP;
-          }
-          if (inA) {
-            int pA = nA + __popc(mA & lt);
-            if (pA < acap && pR < rcap) rowA[pA] = (uint8_t)pR; else bad |= FLAG_CAP;
-          }
-          nR += __popc(mR); nA += __popc(mA);
         }
+        const unsigned mR = __ballot_sync(0xffffffffu, inR);
+        const unsigned mA = __ballot_sync(0xffffffffu, inA);
+        const int pR = nR + __popc(mR & lt);
+        if (inR) { if (pR < rcap) rowR[pR] = ent; else bad |= FLAG_CAP; }
+        if (inA) {
+          const int pA = nA + __popc(mA & lt);
+          if (pA < acap && pR < rcap) rowA[pA] = (uint8_t)pR; else bad |= FLAG_CAP;
+        }
+        nR += __popc(mR); nA += __popc(mA);
       }
+      if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
     }
   }
   if (bad) atomicOr(flags, bad);
-  if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
 }
 
 // ---------------------------------------------------------------- host launcher
@@ -367,11 +422,11 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   if (n_ml > 0) {
     k_scatter<<<nb, 256, 0, st>>>(ws->grid, ws->tmp4, ws->rank, ws->bstart, (int)n_ml, ws->spos, ws->scell);
     // the bucket count is only known on the device: launch for the capacity, guard on S * ncell inside
-    k_bucket_sort<<<(S * ws->max_cells + 255) / 256, 256, 0, st>>>(ws->grid, S, ws->bstart, ws->spos);
-    k_neighbors<<<(int)((n_ml * 32 + 255) / 256), 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->scell,
-                                                                ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap,
-                                                                ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
-                                                                ws->flags);
+    k_bucket_sort<<<(S * ws->max_cells + 7) / 8, 256, 0, st>>>(ws->grid, S, ws->bstart, ws->spos);
+    // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside
+    k_neighbors<<<ws->max_cells, 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->bstart, d_pos, d_ml,
+                                               (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
+                                               ws->flags);
     nl += 3;
   }
   return nl;
