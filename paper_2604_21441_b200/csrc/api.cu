@@ -147,7 +147,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
   void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
-                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->hd_pos, ws->hd_Z, ws->hd_ml,
+                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_energy, ws->hd_forces};
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -179,7 +179,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
             dmalloc(&ws->cntA, nm) && dmalloc(&ws->aev, nr * K) && dmalloc(&ws->daev, nr * K) &&
             dmalloc(&ws->hbuf[0], nr * HP) && dmalloc(&ws->hbuf[1], nr * HP) && dmalloc(&ws->hbuf[2], nr * HP) &&
             dmalloc(&ws->dbuf[0], nr * HP) && dmalloc(&ws->dbuf[1], nr * HP) && dmalloc(&ws->e_atom, nr) &&
-            dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
+            dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->epart, nm / 256 + 2) && dmalloc(&ws->ticket, 1) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
             dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) && dmalloc(&ws->hd_energy, 1) &&
             dmalloc(&ws->hd_forces, 3 * (size_t)max_atoms);
   if (ok) ok = (tc_workspace_create(ws) == NNP_OK);

@@ -38,6 +38,97 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   const float* __restrict__ gi = daev + (size_t)(ip + grp->pad_shift[si]) * Kc;
 
   // ---- angular: p_ij for the angular neighbours, staged in Pacc
+  if (nA <= 32) {
+    // Every unordered pair {j,k} is evaluated ONCE and yields both p_ij and p_ik.  Lanes hold neighbours; in round m
+    // lane j pairs with k = (j + m) mod n, keeps its own share and hands k's share to lane k by shuffle (k <-> j is
+    // a permutation, so every lane receives exactly one share per round).  32 / W lane groups take alternate rounds.
+    const int n = nA;
+    const int W = (n <= 8) ? 8 : (n <= 16) ? 16 : 32;
+    const int NG = 32 / W, grp_id = lane / W, jl = lane & (W - 1);
+    const bool act = jl < n;
+    const int nrounds = n >> 1;
+    float px = 0.f, py = 0.f, pz = 0.f;
+    float4 uj = make_float4(0.f, 0.f, 1.f, 1.f);
+    float fj = 0.f, dfj = 0.f;
+    int sj = 0;
+    if (act) { uj = e.ua[jl]; fj = e.fA[jl]; dfj = e.dfA[jl]; sj = e.slotA[jl]; }
+    for (int m0 = 1; m0 <= nrounds; m0 += NG) {
+      const int m = m0 + grp_id;
+      const bool last_half = ((n & 1) == 0) && (m == nrounds);   // even n: the round m = n/2 holds each pair twice
+      const bool on = act && m <= nrounds && (!last_half || jl < nrounds);
+      float qx = 0.f, qy = 0.f, qz = 0.f;
+      if (on) {
+        int k = jl + m;
+        if (k >= n) k -= n;
+        const float4 uk = e.ua[k];
+        const float fk = e.fA[k], dfk = e.dfA[k];
+        const int sk = e.slotA[k];
+        const int s1 = min(sj, sk), s2 = max(sj, sk);
+        const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
+        const float4* __restrict__ gb = reinterpret_cast<const float4*>(gi + grp->cpos[c.nRB + pidx] * BLK);
+        const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
+        const float cc = c.cTheta * u;
+        const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
+        const float kd = 0.5f * c.zeta * c.cTheta / ss;            // -0.5 zeta dtheta/du
+        float F1[NSHFZ], dF1[NSHFZ];
+#pragma unroll
+        for (int z = 0; z < NSHFZ; ++z) {
+          const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
+          const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
+          const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 0.f);
+          float Bz, Bm;
+          bpow(c, B, Bz, Bm);
+          F1[z] = Bz;
+          dF1[z] = kd * Bm * sind;                                  // dF1/du
+        }
+        const float Rbar = 0.5f * (uj.w + uk.w);
+        float S0 = 0.f, S1 = 0.f, sV = 0.f;
+#pragma unroll
+        for (int a = 0; a < NSHFA; ++a) {
+          const float4 g0 = gb[2 * a], g1 = gb[2 * a + 1];
+          float Wv = g0.x * F1[0], V = g0.x * dF1[0];
+          Wv = fmaf(g0.y, F1[1], Wv); V = fmaf(g0.y, dF1[1], V);
+          Wv = fmaf(g0.z, F1[2], Wv); V = fmaf(g0.z, dF1[2], V);
+          Wv = fmaf(g0.w, F1[3], Wv); V = fmaf(g0.w, dF1[3], V);
+          Wv = fmaf(g1.x, F1[4], Wv); V = fmaf(g1.x, dF1[4], V);
+          Wv = fmaf(g1.y, F1[5], Wv); V = fmaf(g1.y, dF1[5], V);
+          Wv = fmaf(g1.z, F1[6], Wv); V = fmaf(g1.z, dF1[6], V);
+          Wv = fmaf(g1.w, F1[7], Wv); V = fmaf(g1.w, dF1[7], V);
+          const float x = Rbar - c.ShfA[a];
+          const float F2 = ex2f(-c.etaA_l2e * x * x);
+          const float WF = Wv * F2;
+          S0 += WF; S1 = fmaf(WF, x, S1);
+          sV = fmaf(V, F2, sV);
+        }
+        // dt/dR_ij and dt/dR_ik (through Rbar and the cut-offs), dt/du
+        const float Aj = 2.0f * fk * fmaf(-c.etaA * fj, S1, dfj * S0);
+        const float Ak = 2.0f * fj * fmaf(-c.etaA * fk, S1, dfk * S0);
+        const float Au = 2.0f * fj * fk * sV;
+        const float qj = Au / uj.w, qk = Au / uk.w;
+        const float rj = Aj - qj * u, rk = Ak - qk * u;
+        px = fmaf(rj, uj.x, fmaf(qj, uk.x, px));
+        py = fmaf(rj, uj.y, fmaf(qj, uk.y, py));
+        pz = fmaf(rj, uj.z, fmaf(qj, uk.z, pz));
+        qx = fmaf(rk, uk.x, qk * uj.x);
+        qy = fmaf(rk, uk.y, qk * uj.y);
+        qz = fmaf(rk, uk.z, qk * uj.z);
+      }
+      int src = jl - m;
+      if (src < 0) src += n;
+      const int srcl = (grp_id * W + src) & 31;
+      const float rx = __shfl_sync(0xffffffffu, qx, srcl);
+      const float ry = __shfl_sync(0xffffffffu, qy, srcl);
+      const float rz = __shfl_sync(0xffffffffu, qz, srcl);
+      if (act && m <= nrounds && (!last_half || jl >= nrounds)) { px += rx; py += ry; pz += rz; }
+    }
+    for (int o = W; o < 32; o <<= 1) {
+      px += __shfl_xor_sync(0xffffffffu, px, o);
+      py += __shfl_xor_sync(0xffffffffu, py, o);
+      pz += __shfl_xor_sync(0xffffffffu, pz, o);
+    }
+    if (act && grp_id == 0) { Pacc[w][jl][0] = px; Pacc[w][jl][1] = py; Pacc[w][jl][2] = pz; }
+  } else {
+  // more than 32 angular neighbours (beyond liquid-water densities): lanes x partner loop, every pair from both ends
   const int P = (nA <= 8) ? 4 : (nA <= 16) ? 2 : 1;   // lanes per neighbour
   const int JW = 32 / P;                               // neighbours per pass
   const int h = lane % P;
@@ -105,6 +196,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     }
     if (j < nA && h == 0) { Pacc[w][j][0] = px; Pacc[w][j][1] = py; Pacc[w][j][2] = pz; }
   }
+  }
   __syncwarp();
 
   // ---- radial + assembly: lane <-> radial neighbour
@@ -152,52 +244,66 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   }
 }
 
-// K8b: facc (sorted order, fixed point; = sum_j (p_aj - p_ja) = +F) -> forces in the caller's atom order.
-__global__ void k_force_out(const float4* __restrict__ spos, const unsigned long long* __restrict__ facc,
-                            const int32_t* __restrict__ ml, int n_ml, float* __restrict__ forces) {
+// K8b: facc (sorted order, fixed point; = sum_j (p_aj - p_ja) = +F) -> forces in the caller's atom order, and
+// E = sum_i E_i in a fixed order: fp64 block partials (shuffle tree), then the last block to finish adds the
+// partials in index order -- no floating-point atomics, bitwise reproducible.
+__global__ void __launch_bounds__(256)
+k_force_out(const float4* __restrict__ spos, const unsigned long long* __restrict__ facc,
+            const int32_t* __restrict__ ml, int n_ml, float* __restrict__ forces, const GroupInfo* __restrict__ grp,
+            const float* __restrict__ e_atom, double* __restrict__ epart, unsigned int* __restrict__ ticket,
+            double* __restrict__ energy) {
+  __shared__ double wsum[8];
+  __shared__ bool last;
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
-  if (ip >= n_ml) return;
-  const int a = __float_as_int(spos[ip].w) & 0x0fffffff;
-  const size_t o = ml ? (size_t)ml[a] : (size_t)a;
-  const double sc = 1.0 / 1099511627776.0;
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  double e = 0.0;
+  if (ip < n_ml) {
+    const int w = __float_as_int(spos[ip].w);
+    const int a = w & 0x0fffffff, slot = (w >> 28) & 7;
+    const size_t o = ml ? (size_t)ml[a] : (size_t)a;
+    const double sc = 1.0 / 1099511627776.0;
 #pragma unroll
-  for (int d = 0; d < 3; ++d) forces[3 * o + d] = (float)((double)(long long)facc[3 * (size_t)ip + d] * sc);
-}
-
-// E = sum_i E_i over the valid rows, fixed order (thread-strided partial sums in fp64, then a fixed tree).
-__global__ void __launch_bounds__(1024) k_energy(const GroupInfo* __restrict__ grp, const float* __restrict__ e_atom,
-                                                 int S, double* __restrict__ energy) {
-  __shared__ double part[1024];
-  double s = 0.0;
-  for (int q = 0; q < S; ++q) {
-    const int r0 = grp->start[q] + grp->pad_shift[q], n = grp->count[q];
-    for (int r = threadIdx.x; r < n; r += 1024) s += (double)e_atom[r0 + r];
+    for (int d = 0; d < 3; ++d) forces[3 * o + d] = (float)((double)(long long)facc[3 * (size_t)ip + d] * sc);
+    e = (double)e_atom[ip + grp->pad_shift[slot]];
   }
-  part[threadIdx.x] = s;
+  for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+  if (lane == 0) wsum[wp] = e;
   __syncthreads();
-  for (int o = 512; o > 0; o >>= 1) {
-    if ((int)threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
-    __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int i = 0; i < 8; ++i) t += wsum[i];
+    epart[blockIdx.x] = t;
+    __threadfence();
+    last = (atomicAdd(ticket, 1u) == gridDim.x - 1);
   }
-  if (threadIdx.x == 0) *energy = part[0];
+  __syncthreads();
+  if (!last || wp != 0) return;
+  __threadfence();
+  double t = 0.0;
+  for (int i = lane; i < (int)gridDim.x; i += 32) t += __ldcg(epart + i);
+  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+  if (lane == 0) { *energy = t; *ticket = 0u; }
 }
 
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
                        float* d_forces) {
   const nnp_model* m = ws->model;
   int nl = 0;
-  cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
+  // rows of non-ML atoms are +0.0f; with no index subset every row is written by k_force_out
+  if (d_ml || n_ml <= 0) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
   if (n_ml > 0) {
     const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
     k_aev_backward<<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR, ws->nbrA,
                                                           ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
                                                           ws->facc);
     prof_mark(ws, 4);
-    k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces);
+    k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces,
+                                                                   ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy);
     nl += 2;
+  } else {
+    cudaMemsetAsync(d_energy, 0, sizeof(double), ws->stream);
   }
-  k_energy<<<1, 1024, 0, ws->stream>>>(ws->groups, ws->e_atom, m->aev.S, d_energy);
-  return nl + 1;
+  return nl;
 }
 
 }  // namespace nnp

@@ -146,12 +146,6 @@ __device__ __forceinline__ float unpack_c_hi(uint32_t q) { return (float)(q >> 1
 // layer-1 operand images are (re)packed on the device, only when that column set changed since the last call.
 struct TcPackArgs { uint8_t* w1[MAX_S]; uint8_t* w1t[MAX_S]; };
 
-__device__ __forceinline__ unsigned long long tc_colset_key(const GroupInfo* grp) {
-  unsigned long long k = 1ull << 63;
-  for (int b = 0; b < grp->nblk; ++b) k |= 1ull << grp->blkmap[b];
-  return k;
-}
-
 __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t blk_lo, int r, int kk, const float* x) {
   uint32_t hi[4], lo[4];
 #pragma unroll
@@ -163,7 +157,7 @@ __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t bl
 
 __global__ void __launch_bounds__(256)
 k_tc_pack_w1(NetTable nets, const GroupInfo* __restrict__ grp, TcPackArgs a, unsigned long long* __restrict__ key) {
-  const unsigned long long want = tc_colset_key(grp);
+  const unsigned long long want = grp->colkey;
   if (key[0] == want) return;
   if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) key[1] = want;
   const int slot = blockIdx.y;
@@ -612,7 +606,7 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   if (!tm || !tw) return launch_mlp_simt(ws, n_ml);
   TcPackArgs pa;
   for (int s = 0; s < MAX_S; ++s) { pa.w1[s] = tw->w1img[s]; pa.w1t[s] = tw->w1timg[s]; }
-  k_tc_pack_w1<<<dim3(64, m->aev.S), 256, 0, ws->stream>>>(m->nets, ws->groups, pa, tw->key);
+  k_tc_pack_w1<<<dim3(32, m->aev.S), 256, 0, ws->stream>>>(m->nets, ws->groups, pa, tw->key);
   const int grid = std::min(ws->max_tiles, tw->num_sms);
   if (ws->mlp_mode == NNP_MLP_F16X1)
     k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(m->nets, tm->tab, pa, ws->groups, ws->tiles, ws->aev,

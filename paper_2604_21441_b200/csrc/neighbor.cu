@@ -130,24 +130,42 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
                                                int* __restrict__ bstart, GroupInfo* __restrict__ grp,
                                                TileInfo* __restrict__ tiles, int S, int n_ml, int max_tiles,
                                                int dense_k, int* __restrict__ flags) {
-  __shared__ int part[1024];
+  // block-wide exclusive scan of S * ncell bucket counts: each warp owns a contiguous span and sweeps it 32 at a
+  // time (coalesced, loads batched four deep), then the warp totals are scanned and added back.
+  __shared__ int wtot[32];
   __shared__ int gs[MAX_S + 1], tb[MAX_S + 1];
   const int n = S * g->ncell;
-  const int per = (n + 1023) / 1024;
-  const int lo = min(threadIdx.x * per, n), hi = min(lo + per, n);
-  int s = 0;
-  for (int k = lo; k < hi; ++k) s += count[k];
-  part[threadIdx.x] = s;
-  __syncthreads();
-  for (int o = 1; o < 1024; o <<= 1) {  // Hillis-Steele inclusive scan
-    int v = (threadIdx.x >= o) ? part[threadIdx.x - o] : 0;
-    __syncthreads();
-    part[threadIdx.x] += v;
-    __syncthreads();
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  const int span = (((n + 31) / 32 + 31) / 32) * 32;
+  const int lo = min(wp * span, n), hi = min(lo + span, n);
+  int carry = 0;
+  for (int k0 = lo; k0 < hi; k0 += 128) {
+    int v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; v[u] = (k < hi) ? count[k] : 0; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      int inc = v[u];
+      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+      const int k = k0 + 32 * u + lane;
+      if (k < hi) bstart[k] = carry + inc - v[u];
+      carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
   }
-  int run = part[threadIdx.x] - s;
-  for (int k = lo; k < hi; ++k) { bstart[k] = run; run += count[k]; }
-  if (threadIdx.x == 1023) { bstart[n] = part[1023]; if (part[1023] != n_ml) atomicOr(flags, FLAG_ARG); }
+  if (lane == 0) wtot[wp] = carry;
+  __syncthreads();
+  int base = 0, total = 0;
+  for (int w = 0; w < 32; ++w) { const int t = wtot[w]; if (w < wp) base += t; total += t; }
+  if (base != 0) {
+    for (int k0 = lo; k0 < hi; k0 += 128) {
+      int v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; v[u] = (k < hi) ? bstart[k] : 0; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; if (k < hi) bstart[k] = v[u] + base; }
+    }
+  }
+  if (threadIdx.x == 0) { bstart[n] = total; if (total != n_ml) atomicOr(flags, FLAG_ARG); }
   __syncthreads();
   if (threadIdx.x <= S) gs[threadIdx.x] = bstart[threadIdx.x * g->ncell];
   __syncthreads();
@@ -188,6 +206,9 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
     for (int b = nb; b < MAX_BLK; ++b) grp->blkmap[b] = 0;
     grp->nblk = nb;
     grp->Kc = nb * BLK;
+    unsigned long long key = 1ull << 63;
+    for (int b = 0; b < nb; ++b) key |= 1ull << grp->blkmap[b];
+    grp->colkey = key;
   }
   __syncthreads();
   const int nt = min(tb[MAX_S], max_tiles);

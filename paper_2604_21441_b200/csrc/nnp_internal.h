@@ -70,6 +70,7 @@ struct GroupInfo {
   int Kc;                // 32 * nblk = row pitch of aev / daev
   int blkmap[MAX_BLK];   // compact block -> internal block
   int cpos[MAX_BLK];     // internal block -> compact block, or -1
+  unsigned long long colkey;  // bit 63 | bit mask of the materialised internal blocks (identifies the column set)
 };
 
 struct TileInfo { int slot, row0, nvalid, pad; };
@@ -131,6 +132,8 @@ struct nnp_workspace {
   float* dbuf[2];            // deltas [max_rows][HP]
   float* e_atom;             // [max_rows]
   unsigned long long* facc;  // [max_ml][3] int64 fixed point, indexed by sorted position
+  double* epart;             // [ceil(max_ml/256)] block partial sums of E_i (K8)
+  unsigned int* ticket;      // [1] last-block ticket of K8
   void* tc_ws;               // tensor-core path scratch
   int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
   cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end
