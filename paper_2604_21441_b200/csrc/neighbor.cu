@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(256) k_bucket_sort(const GridInfo* __restrict_
 }
 
 // ---------------------------------------------------------------- K2: neighbour rows, one warp per centre
-__device__ __forceinline__ double exact_d2(const float* __restrict__ pos, int oi, int oj, const GridInfo* g) {
+__device__ __noinline__ double exact_d2(const float* __restrict__ pos, int oi, int oj, const GridInfo* g) {
   double d[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -287,7 +287,7 @@ constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of
 // staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
 // cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
 // warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
-__global__ void __launch_bounds__(256) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
+__global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
                                                    const float4* __restrict__ spos,
                                                    const int* __restrict__ bstart, const float* __restrict__ pos,
@@ -377,43 +377,42 @@ __global__ void __launch_bounds__(256) k_neighbors(AevConst c, const GridInfo* _
       uint8_t* rowA = nbrA + (size_t)ip * acap;
       int nR = 0, nA = 0;
       if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; }
+      const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
+      const float hiR = c.Rcr2 + GUARD_BAND, loR = c.Rcr2 - GUARD_BAND, hiA = c.Rca2 + GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
       for (int q0 = 0; q0 < nin; q0 += 32) {
-        const int q = q0 + lane;
-        bool inR = false, inA = false;
-        uint32_t ent = 0;
-        if (q < nin) {
-          const float4 pj = cand[q];
-          ent = (uint32_t)__float_as_int(pj.w);
-          const int jp = (int)(ent & JMASK);
-          float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-          if (nc0 == 1 && pbc) { const int o = -(int)rintf(dx / ex); dx += (float)o * ex; ent += (uint32_t)o << JBITS; }
-          if (nc1 == 1 && pbc) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
-          if (nc2 == 1 && pbc) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
-          const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-          if (jp != ip && d2 < c.Rcr2 + GUARD_BAND) {
-            const bool nearR = fabsf(d2 - c.Rcr2) <= GUARD_BAND, nearA = fabsf(d2 - c.Rca2) <= GUARD_BAND;
-            inR = !nearR;
-            inA = d2 < c.Rca2;
-            if (nearR || nearA || d2 < 1e-6f) {
-              const int a_j = __float_as_int(spos[jp].w) & 0x0fffffff;
-              const int o_j = ml ? ml[a_j] : a_j;
-              const double e2 = exact_d2(pos, o_i, o_j, g);
-              if (nearR) inR = e2 <= c.Rcr2_d;
-              if (nearA) inA = e2 <= c.Rca2_d;
-              if (e2 == 0.0) bad |= FLAG_COINCIDENT;
-            }
+        const int q = min(q0 + lane, nin - 1);
+        const float4 pj = cand[q];
+        uint32_t ent = (uint32_t)__float_as_int(pj.w);
+        float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        if (wrap) {   // block-uniform: a dimension with a single cell takes the minimum image per pair
+          if (nc0 == 1) { const int o = -(int)rintf(dx / ex); dx += (float)o * ex; ent += (uint32_t)o << JBITS; }
+          if (nc1 == 1) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
+          if (nc2 == 1) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
+        }
+        const int jp = (int)(ent & JMASK);
+        float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (q0 + lane >= nin || jp == ip) d2 = 3.0e38f;
+        bool inR = d2 < loR, inA = d2 < loA;
+        // guard bands (and coincident atoms): the pinned fp64 predicate on the original coordinates decides
+        const bool nearR = d2 >= loR && d2 <= hiR, nearA = d2 >= loA && d2 <= hiA;
+        if (__any_sync(0xffffffffu, nearR || nearA || d2 < 1e-6f)) {
+          if (nearR || nearA || d2 < 1e-6f) {
+            const int a_j = __float_as_int(spos[jp].w) & 0x0fffffff;
+            const int o_j = ml ? ml[a_j] : a_j;
+            const double e2 = exact_d2(pos, o_i, o_j, g);
+            if (nearR) inR = e2 <= c.Rcr2_d;
+            if (nearA) inA = e2 <= c.Rca2_d;
+            if (e2 == 0.0) bad |= FLAG_COINCIDENT;
           }
         }
         const unsigned mR = __ballot_sync(0xffffffffu, inR);
         const unsigned mA = __ballot_sync(0xffffffffu, inA);
-        const int pR = nR + __popc(mR & lt);
-        if (inR) { if (pR < rcap) rowR[pR] = ent; else bad |= FLAG_CAP; }
-        if (inA) {
-          const int pA = nA + __popc(mA & lt);
-          if (pA < acap && pR < rcap) rowA[pA] = (uint8_t)pR; else bad |= FLAG_CAP;
-        }
+        const int pR = nR + __popc(mR & lt), pA = nA + __popc(mA & lt);
+        if (inR && pR < rcap) rowR[pR] = ent;
+        if (inA && pA < acap && pR < rcap) rowA[pA] = (uint8_t)pR;
         nR += __popc(mR); nA += __popc(mA);
       }
+      if (nR > rcap || nA > acap) bad |= FLAG_CAP;
       if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
     }
   }
