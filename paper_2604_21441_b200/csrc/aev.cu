@@ -56,7 +56,7 @@ __device__ __forceinline__ void decode_same(int t, int n, float inv_n, int& j, i
   if (k >= n) k -= n;
 }
 
-__global__ void __launch_bounds__(AEV_WARPS * 32)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 4)
 k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
               const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
@@ -97,11 +97,17 @@ k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __res
     row[cp * BLK + lane] = out;
   }
 
-  // ---- angular
-  int p = 0;
-  for (int s1 = 0; s1 < c.S; ++s1) {
+  // ---- angular: only pairs of species that are present can hold triplets; in dense-K mode the other
+  // materialised blocks are zero-filled first (same lane, same address: program order keeps the later value)
+  const int np = grp->npres;
+  if (grp->nblk == c.nblk_full && np < c.S)
+    for (int b = c.nRB; b < c.nblk_full; ++b) row[grp->cpos[b] * BLK + lane] = 0.f;
+  for (int i1 = 0; i1 < np; ++i1) {
+    const int s1 = grp->pres[i1];
     const int a1 = e.segA[s1], n1 = e.segA[s1 + 1] - a1;
-    for (int s2 = s1; s2 < c.S; ++s2, ++p) {
+    for (int i2 = i1; i2 < np; ++i2) {
+      const int s2 = grp->pres[i2];
+      const int p = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
       const int cp = grp->cpos[c.nRB + p];
       if (cp < 0) continue;
       const int a2 = e.segA[s2], n2 = e.segA[s2 + 1] - a2;

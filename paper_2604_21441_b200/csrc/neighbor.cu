@@ -206,6 +206,10 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
     for (int b = nb; b < MAX_BLK; ++b) grp->blkmap[b] = 0;
     grp->nblk = nb;
     grp->Kc = nb * BLK;
+    int npres = 0;
+    for (int q = 0; q < MAX_S; ++q) { if (cnt[q] > 0) grp->pres[npres++] = q; }
+    for (int q = npres; q < MAX_S; ++q) grp->pres[q] = 0;
+    grp->npres = npres;
     unsigned long long key = 1ull << 63;
     for (int b = 0; b < nb; ++b) key |= 1ull << grp->blkmap[b];
     grp->colkey = key;

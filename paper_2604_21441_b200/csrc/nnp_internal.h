@@ -70,6 +70,8 @@ struct GroupInfo {
   int Kc;                // 32 * nblk = row pitch of aev / daev
   int blkmap[MAX_BLK];   // compact block -> internal block
   int cpos[MAX_BLK];     // internal block -> compact block, or -1
+  int npres;             // species present in this evaluation, ascending
+  int pres[MAX_S];
   unsigned long long colkey;  // bit 63 | bit mask of the materialised internal blocks (identifies the column set)
 };
 
