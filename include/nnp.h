@@ -132,6 +132,10 @@ int nnp_debug_aev(nnp_workspace*, float* h_aev);
 int nnp_debug_daev(nnp_workspace*, float* h_daev);
 int nnp_debug_atomic_energies(nnp_workspace*, float* h_e);
 int nnp_debug_counters(nnp_workspace*, int64_t* launches);
+/* SM-clock ticks of the tensor-core MLP kernel's CTA 0 over its first 32 GEMM rounds (HOST h_ticks[64]): even
+ * entries = operand handed to the MMA warp, odd entries = accumulator complete.  Differences give the time spent
+ * in epilogues (odd -> next even) and in MMA rounds (even -> odd); used by the profiling notes. */
+int nnp_debug_mlp_timeline(nnp_workspace*, int64_t* h_ticks);
 /* Stage timing of nnp_eval with CUDA events on the workspace stream.  set_profiling(1) makes every later
  * nnp_eval record an event at each stage boundary (not capturable into a CUDA graph while on);
  * nnp_debug_stage_times waits for the last evaluation and writes HOST ms[5] = {neighbour stage K0-K2,

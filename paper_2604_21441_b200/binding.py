@@ -18,7 +18,7 @@ EXPORTS = [
     "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
-    "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
+    "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
 
 
@@ -75,6 +75,7 @@ def lib():
         L.nnp_debug_daev.argtypes = [vp, vp]
         L.nnp_debug_atomic_energies.argtypes = [vp, vp]
         L.nnp_debug_counters.argtypes = [vp, C.POINTER(i64)]
+        L.nnp_debug_mlp_timeline.argtypes = [vp, vp]
         L.nnp_workspace_set_profiling.argtypes = [vp, i32]
         L.nnp_debug_stage_times.argtypes = [vp, vp]
         _lib = L
@@ -147,6 +148,10 @@ def nnp_debug_daev(ws, h_daev):
 
 def nnp_debug_atomic_energies(ws, h_e):
     return lib().nnp_debug_atomic_energies(ws, h_e)
+
+
+def nnp_debug_mlp_timeline(ws, h_ticks):
+    return lib().nnp_debug_mlp_timeline(ws, h_ticks)
 
 
 def nnp_debug_counters(ws):
@@ -297,6 +302,11 @@ class Workspace:
         a = np.zeros((n_ml, self.model.aev_length), dtype=np.float32)
         _check(nnp_debug_daev(self.handle, a.ctypes.data), "nnp_debug_daev")
         return a
+
+    def mlp_timeline(self):
+        t = np.zeros(64, dtype=np.int64)
+        _check(nnp_debug_mlp_timeline(self.handle, t.ctypes.data), "nnp_debug_mlp_timeline")
+        return t
 
     def atomic_energies(self, n_ml):
         e = np.zeros(n_ml, dtype=np.float32)

@@ -425,6 +425,13 @@ extern "C" int nnp_debug_atomic_energies(nnp_workspace* ws, float* h_e) {
   return NNP_OK;
 }
 
+extern "C" int nnp_debug_mlp_timeline(nnp_workspace* ws, int64_t* h_ticks) {
+  if (!ws || !h_ticks) return NNP_ERR_INVALID_ARG;
+  if (cudaStreamSynchronize(ws->stream) != cudaSuccess) { cudaGetLastError(); return NNP_ERR_CUDA; }
+  static_assert(sizeof(long long) == sizeof(int64_t), "tick type");
+  return tc_read_timeline(reinterpret_cast<long long*>(h_ticks));
+}
+
 extern "C" int nnp_debug_counters(nnp_workspace* ws, int64_t* launches) {
   if (!ws || !launches) return NNP_ERR_INVALID_ARG;
   launches[0] = ws->launches;

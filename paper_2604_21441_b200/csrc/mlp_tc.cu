@@ -121,6 +121,12 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
       "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
       TC_W8(v, 0), TC_W8(v, 8) : "memory");
 }
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];" : TC_R8(v, 0) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), TC_W8(v, 0) : "memory");
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
@@ -134,12 +140,18 @@ __device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_
   hi = h2_bits(h);
   lo = h2_bits(__floats2half2_rn(x0 - hf.x, x1 - hf.y));
 }
-// CELU' in [0, 1] as unorm16 pairs (1.0 exact); absolute error 2^-17
+// CELU' in [0, 1] as unorm16 pairs (1.0 exact; absolute error 2^-17).  Conversions go through the 2^23 trick
+// (x + 2^23 holds round-to-nearest(x) in its low mantissa bits) so that they stay on the FMA/ALU pipes.
 __device__ __forceinline__ uint32_t pack_c(float c0, float c1) {
-  return __float2uint_rn(c0 * 65535.f) | (__float2uint_rn(c1 * 65535.f) << 16);
+  const uint32_t q0 = __float_as_uint(fmaf(c0, 65535.f, 8388608.f)), q1 = __float_as_uint(fmaf(c1, 65535.f, 8388608.f));
+  return __byte_perm(q0, q1, 0x5410);
 }
-__device__ __forceinline__ float unpack_c_lo(uint32_t q) { return (float)(q & 0xffffu) * (1.0f / 65535.f); }
-__device__ __forceinline__ float unpack_c_hi(uint32_t q) { return (float)(q >> 16) * (1.0f / 65535.f); }
+__device__ __forceinline__ float unpack_c_lo(uint32_t q) {
+  return (__uint_as_float(__byte_perm(q, 0x4B000000u, 0x7610)) - 8388608.f) * (1.0f / 65535.f);
+}
+__device__ __forceinline__ float unpack_c_hi(uint32_t q) {
+  return (__uint_as_float(__byte_perm(q, 0x4B000000u, 0x7632)) - 8388608.f) * (1.0f / 65535.f);
+}
 
 // ------------------------------------------------------------------------------------------------ layer-1 images
 // The AEV columns that are materialised depend on the species present in the evaluation (GroupInfo::blkmap), so the
@@ -187,7 +199,8 @@ k_tc_pack_w1(NetTable nets, const GroupInfo* __restrict__ grp, TcPackArgs a, uns
 }
 
 // ------------------------------------------------------------------------------------------------ the fused kernel
-constexpr int TC_EPI_WARPS = 8;                       // loader / epilogue warps (two per TMEM lane quarter)
+constexpr int TC_EPI_WARPS = 16;                      // loader / epilogue warps (four per TMEM lane quarter)
+constexpr int TC_NPART = TC_EPI_WARPS / 4;            // warps sharing a lane quarter split the 16-column chunks
 constexpr int TC_THREADS = (TC_EPI_WARPS + 2) * 32;   // + weight producer warp + MMA issuer warp
 constexpr uint32_t TC_PANEL = 16384;                  // 128 rows x 128 B
 constexpr uint32_t TC_LO = 4 * TC_PANEL;              // lo half of the A buffer
@@ -202,7 +215,7 @@ template <int NPASS> struct TcCfg {
   static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], a_ready, acc_full
   static constexpr uint32_t TPTR = BARS + (2 * NST + 2) * 8;
   static constexpr uint32_t EPART = TPTR + 16;
-  static constexpr uint32_t TOTAL = EPART + 128 * 4;
+  static constexpr uint32_t TOTAL = EPART + (TC_NPART - 1) * 128 * 4;
 };
 
 struct TileNet {
@@ -227,15 +240,18 @@ __device__ __forceinline__ void tc_for_rounds(const TileNet& t, F&& f) {
 
 template <int NPASS>
 __device__ __forceinline__ void tc_store_act(uint32_t abuf, int row, int j, const uint32_t* hi, const uint32_t* lo) {
-  // columns [32j, 32j+32) of `row` -> four 16-byte chunks of K-panel j/2 (conflict-free: chunk XOR row%8)
-  const uint32_t base = abuf + (uint32_t)(j >> 1) * TC_PANEL + (uint32_t)row * 128u;
+  // columns [16j, 16j+16) of `row` -> two 16-byte chunks of K-panel j/4 (conflict-free: chunk XOR row%8)
+  const uint32_t base = abuf + (uint32_t)(j >> 2) * TC_PANEL + (uint32_t)row * 128u;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const uint32_t off = (uint32_t)((((j & 1) * 4 + i) ^ (row & 7)) << 4);
+  for (int i = 0; i < 2; ++i) {
+    const uint32_t off = (uint32_t)((((j & 3) * 2 + i) ^ (row & 7)) << 4);
     sts128(base + off, hi[4 * i], hi[4 * i + 1], hi[4 * i + 2], hi[4 * i + 3]);
     if (NPASS == 3) sts128(base + TC_LO + off, lo[4 * i], lo[4 * i + 1], lo[4 * i + 2], lo[4 * i + 3]);
   }
 }
+
+// SM-clock timeline of CTA 0's first rounds (debug export nnp_debug_mlp_timeline): where a tile's time goes.
+__device__ long long g_tc_timeline[64];
 
 template <int NPASS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
@@ -332,16 +348,20 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       }
     }
   } else {
-    // ===== loader / epilogue warps: thread <-> tile row (TMEM lane); warps w and w+4 split the 32-column chunks =====
-    const int q = warp & 3, hf = warp >> 2, row = q * 32 + lane;
+    // ===== loader / epilogue warps: thread <-> tile row (TMEM lane); the TC_NPART warps of a lane quarter take the
+    // 16-column chunks round-robin =====
+    const int q = warp & 3, part = warp >> 2, row = q * 32 + lane;
     const uint32_t tlane = tmem + ((uint32_t)(q * 32) << 16);
     uint32_t fph = 0;
+    int tl = 0;   // timeline slot (block 0, thread 0 only): even = operand handed to the MMA warp, odd = accumulator back
     auto signal_and_wait = [&]() {
       tc_fence_before();
       fence_proxy_async();
+      if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
       mbar_arrive(bar_aready);
       mbar_wait(bar_acc, fph); fph ^= 1;
       tc_fence_after();
+      if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
     };
     for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
       TileInfo ti; TileNet tn; tile_net(t, ti, tn);
@@ -352,19 +372,29 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       const int np = tc_npanels(Kc);
       for (int p0 = 0; p0 < np; p0 += 4) {
         const int k0 = p0 * 64, kw = min(Kc, k0 + 256) - k0, n16 = kw >> 3;
-        for (int idx = threadIdx.x; idx < 128 * n16; idx += TC_EPI_WARPS * 32) {
-          const int r = idx / n16, chn = idx - r * n16;
-          float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
-          if (r < ti.nvalid) {
-            const float4* src = reinterpret_cast<const float4*>(aev + (size_t)(ti.row0 + r) * Kc + k0 + chn * 8);
-            x0 = __ldg(src); x1 = __ldg(src + 1);
+        constexpr int NT = TC_EPI_WARPS * 32;
+        for (int base = threadIdx.x; base < 128 * n16; base += 4 * NT) {
+          float4 x0[4], x1[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {   // all loads of the batch in flight before the first use
+            const int idx = base + u * NT, r = idx / n16, chn = idx - r * n16;
+            x0[u] = make_float4(0.f, 0.f, 0.f, 0.f); x1[u] = x0[u];
+            if (idx < 128 * n16 && r < ti.nvalid) {
+              const float4* src = reinterpret_cast<const float4*>(aev + (size_t)(ti.row0 + r) * Kc + k0 + chn * 8);
+              x0[u] = __ldg(src); x1[u] = __ldg(src + 1);
+            }
           }
-          uint32_t hi[4], lo[4];
-          split2(x0.x, x0.y, hi[0], lo[0]); split2(x0.z, x0.w, hi[1], lo[1]);
-          split2(x1.x, x1.y, hi[2], lo[2]); split2(x1.z, x1.w, hi[3], lo[3]);
-          const uint32_t dst = abuf + (uint32_t)(chn >> 3) * TC_PANEL + (uint32_t)r * 128u + (uint32_t)(((chn & 7) ^ (r & 7)) << 4);
-          sts128(dst, hi[0], hi[1], hi[2], hi[3]);
-          if (NPASS == 3) sts128(dst + TC_LO, lo[0], lo[1], lo[2], lo[3]);
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int idx = base + u * NT, r = idx / n16, chn = idx - r * n16;
+            if (idx >= 128 * n16) break;
+            uint32_t hi[4], lo[4];
+            split2(x0[u].x, x0[u].y, hi[0], lo[0]); split2(x0[u].z, x0[u].w, hi[1], lo[1]);
+            split2(x1[u].x, x1[u].y, hi[2], lo[2]); split2(x1[u].z, x1[u].w, hi[3], lo[3]);
+            const uint32_t dst = abuf + (uint32_t)(chn >> 3) * TC_PANEL + (uint32_t)r * 128u + (uint32_t)(((chn & 7) ^ (r & 7)) << 4);
+            sts128(dst, hi[0], hi[1], hi[2], hi[3]);
+            if (NPASS == 3) sts128(dst + TC_LO, lo[0], lo[1], lo[2], lo[3]);
+          }
         }
         signal_and_wait();
       }
@@ -372,23 +402,27 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
 #pragma unroll 1
       for (int l = 1; l <= 2; ++l) {
         const int N = (l == 1) ? tn.N1 : tn.N2;
-        const float* __restrict__ bias = net.b[l - 1];
+        const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[l - 1]);
         const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
 #pragma unroll 1
-        for (int j = hf; j * 32 < N; j += 2) {
-          uint32_t v[32], hi[16], lo[16], cp[16];
-          tmem_ld32(tlane + TC_ACC + j * 32, v);
+        for (int j = part; j * 16 < N; j += TC_NPART) {
+          uint32_t v[16], hi[8], lo[8], cp[8];
+          tmem_ld16(tlane + TC_ACC + j * 16, v);
+          float4 bv[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) bv[i] = __ldg(bias4 + j * 4 + i);
           tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; i += 2) {
-            const float z0 = __uint_as_float(v[i]) + __ldg(bias + j * 32 + i);
-            const float z1 = __uint_as_float(v[i + 1]) + __ldg(bias + j * 32 + i + 1);
+          for (int i = 0; i < 16; i += 2) {
+            const float4 b4 = bv[i >> 2];
+            const float z0 = __uint_as_float(v[i]) + ((i & 2) ? b4.z : b4.x);
+            const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
             const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
             const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
             cp[i >> 1] = pack_c(z0 > 0.f ? 1.f : e0, z1 > 0.f ? 1.f : e1);
             split2(h0, h1, hi[i >> 1], lo[i >> 1]);
           }
-          tmem_st16(tlane + pcol + j * 16, cp);
+          tmem_st8(tlane + pcol + j * 8, cp);
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
         }
         tmem_wait_st();
@@ -397,19 +431,23 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       // ---- layer 3 + output layer: E_i = h3 . w4 + b4;  dl3 = w4 * CELU'(z3) -> A operand of B3
       {
         const int nl = net.n_layers;
-        const float* __restrict__ bias = net.b[2];
-        const float* __restrict__ w4 = net.W[nl - 1];
+        const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[2]);
+        const float4* __restrict__ w44 = reinterpret_cast<const float4*>(net.W[nl - 1]);
         float e = 0.f;
 #pragma unroll 1
-        for (int j = hf; j * 32 < tn.N3; j += 2) {
-          uint32_t v[32], hi[16], lo[16];
-          tmem_ld32(tlane + TC_ACC + j * 32, v);
+        for (int j = part; j * 16 < tn.N3; j += TC_NPART) {
+          uint32_t v[16], hi[8], lo[8];
+          tmem_ld16(tlane + TC_ACC + j * 16, v);
+          float4 bv[4], wv[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { bv[i] = __ldg(bias4 + j * 4 + i); wv[i] = __ldg(w44 + j * 4 + i); }
           tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; i += 2) {
-            const float z0 = __uint_as_float(v[i]) + __ldg(bias + j * 32 + i);
-            const float z1 = __uint_as_float(v[i + 1]) + __ldg(bias + j * 32 + i + 1);
-            const float wa = __ldg(w4 + j * 32 + i), wb = __ldg(w4 + j * 32 + i + 1);
+          for (int i = 0; i < 16; i += 2) {
+            const float4 b4 = bv[i >> 2], w4 = wv[i >> 2];
+            const float z0 = __uint_as_float(v[i]) + ((i & 2) ? b4.z : b4.x);
+            const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
+            const float wa = (i & 2) ? w4.z : w4.x, wb = (i & 2) ? w4.w : w4.y;
             const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
             const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
             e = fmaf(h0, wa, e); e = fmaf(h1, wb, e);
@@ -417,9 +455,13 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
           }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
         }
-        if (hf == 1) e_part[row] = e;
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (hf == 0) e_atom[ti.row0 + row] = valid ? (e + e_part[row]) + __ldg(net.b[nl - 1]) : 0.f;
+        if (part > 0) e_part[(part - 1) * 128 + row] = e;
+        asm volatile("bar.sync 1, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
+        if (part == 0) {
+#pragma unroll
+          for (int pp = 0; pp < TC_NPART - 1; ++pp) e += e_part[pp * 128 + row];   // fixed order
+          e_atom[ti.row0 + row] = valid ? e + __ldg(net.b[nl - 1]) : 0.f;
+        }
         signal_and_wait();
       }
       // ---- backward through layers 2, 1: dl_l = d_l * CELU'(z_l) -> A operand of the next backward GEMM
@@ -428,13 +470,13 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
         const int N = (l == 1) ? tn.N1 : tn.N2;
         const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
 #pragma unroll 1
-        for (int j = hf; j * 32 < N; j += 2) {
-          uint32_t v[32], cp[16], hi[16], lo[16];
-          tmem_ld32(tlane + TC_ACC + j * 32, v);
-          tmem_ld16(tlane + pcol + j * 16, cp);
+        for (int j = part; j * 16 < N; j += TC_NPART) {
+          uint32_t v[16], cp[8], hi[8], lo[8];
+          tmem_ld16(tlane + TC_ACC + j * 16, v);
+          tmem_ld8(tlane + pcol + j * 8, cp);
           tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; i += 2)
+          for (int i = 0; i < 16; i += 2)
             split2(__uint_as_float(v[i]) * unpack_c_lo(cp[i >> 1]), __uint_as_float(v[i + 1]) * unpack_c_hi(cp[i >> 1]),
                    hi[i >> 1], lo[i >> 1]);
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
@@ -448,14 +490,14 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
           const int n0 = c0 * ch, ncols = min(Kc, (c0 + 2) * ch) - n0;
           float* __restrict__ dst = daev + (size_t)(ti.row0 + row) * Kc + n0;
 #pragma unroll 1
-          for (int j = hf; j * 32 < ncols; j += 2) {
-            uint32_t v[32];
-            tmem_ld32(tlane + TC_ACC + j * 32, v);
+          for (int j = part; j * 16 < ncols; j += TC_NPART) {
+            uint32_t v[16];
+            tmem_ld16(tlane + TC_ACC + j * 16, v);
             tmem_wait_ld();
             if (valid) {
 #pragma unroll
-              for (int i = 0; i < 32; i += 4)
-                *reinterpret_cast<uint4*>(dst + j * 32 + i) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+              for (int i = 0; i < 16; i += 4)
+                *reinterpret_cast<uint4*>(dst + j * 16 + i) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
             }
           }
           if (c0 + 2 < nc) signal_and_wait();
@@ -596,6 +638,10 @@ void tc_workspace_destroy(nnp_workspace* ws) {
   cudaGetLastError();
   delete tw;
   ws->tc_ws = nullptr;
+}
+
+int tc_read_timeline(long long* h64) {
+  return cudaMemcpyFromSymbol(h64, g_tc_timeline, sizeof(long long) * 64) == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
 }
 
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {

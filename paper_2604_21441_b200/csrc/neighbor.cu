@@ -291,7 +291,7 @@ constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of
 // staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
 // cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
 // warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
-__global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
+__global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
                                                    const float4* __restrict__ spos,
                                                    const int* __restrict__ bstart, const float* __restrict__ pos,
@@ -382,10 +382,10 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
       int nR = 0, nA = 0;
       if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; }
       const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
-      const float hiR = c.Rcr2 + GUARD_BAND, loR = c.Rcr2 - GUARD_BAND, hiA = c.Rca2 + GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
-      for (int q0 = 0; q0 < nin; q0 += 32) {
-        const int q = min(q0 + lane, nin - 1);
-        const float4 pj = cand[q];
+      const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
+      const float4* cp = cand + lane;
+      for (int q0 = lane; q0 - lane < nin; q0 += 32, cp += 32) {
+        const float4 pj = (q0 < nin) ? *cp : make_float4(1.0e18f, 1.0e18f, 1.0e18f, __int_as_float(ip));
         uint32_t ent = (uint32_t)__float_as_int(pj.w);
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (wrap) {   // block-uniform: a dimension with a single cell takes the minimum image per pair
@@ -393,19 +393,18 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
           if (nc1 == 1) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
           if (nc2 == 1) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
         }
-        const int jp = (int)(ent & JMASK);
-        float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        if (q0 + lane >= nin || jp == ip) d2 = 3.0e38f;
-        bool inR = d2 < loR, inA = d2 < loA;
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        const bool other = (int)(ent & JMASK) != ip;
+        bool inR = other && d2 < loR, inA = other && d2 < loA;
         // guard bands (and coincident atoms): the pinned fp64 predicate on the original coordinates decides
-        const bool nearR = d2 >= loR && d2 <= hiR, nearA = d2 >= loA && d2 <= hiA;
-        if (__any_sync(0xffffffffu, nearR || nearA || d2 < 1e-6f)) {
-          if (nearR || nearA || d2 < 1e-6f) {
-            const int a_j = __float_as_int(spos[jp].w) & 0x0fffffff;
+        const bool near = other && (fabsf(d2 - Rcr2) <= GUARD_BAND || fabsf(d2 - Rca2) <= GUARD_BAND || d2 < 1e-6f);
+        if (__any_sync(0xffffffffu, near)) {
+          if (near) {
+            const int a_j = __float_as_int(spos[ent & JMASK].w) & 0x0fffffff;
             const int o_j = ml ? ml[a_j] : a_j;
             const double e2 = exact_d2(pos, o_i, o_j, g);
-            if (nearR) inR = e2 <= c.Rcr2_d;
-            if (nearA) inA = e2 <= c.Rca2_d;
+            if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
+            if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
             if (e2 == 0.0) bad |= FLAG_COINCIDENT;
           }
         }

@@ -157,4 +157,5 @@ int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets);
 void tc_model_destroy(nnp_model* m);
 int tc_workspace_create(nnp_workspace* ws);
 void tc_workspace_destroy(nnp_workspace* ws);
+int tc_read_timeline(long long* h64);
 }  // namespace nnp
