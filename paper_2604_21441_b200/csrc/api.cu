@@ -381,7 +381,7 @@ extern "C" int nnp_debug_aev(nnp_workspace* ws, float* h_aev) {
   return NNP_OK;
 }
 
-static int export_rows(nnp_workspace* ws, const float* d_buf, float* h_out) {
+static int export_rows(nnp_workspace* ws, const float* d_buf, float* h_out, bool piece_major) {
   Snapshot s;
   int rc = take_snapshot(ws, s);
   if (rc) return rc;
@@ -401,7 +401,7 @@ static int export_rows(nnp_workspace* ws, const float* d_buf, float* h_out) {
         int pub;
         if (ib < c.nRB) { if (icol >= c.S * NSHFR) continue; pub = icol; }
         else pub = c.S * NSHFR + (icol - c.nRB * BLK);
-        dst[pub] = row[(size_t)b * BLK + q];
+        dst[pub] = piece_major ? buf[daev_off(ip + s.grp.pad_shift[sl], b * BLK + q, (int)Kc)] : row[(size_t)b * BLK + q];
       }
     }
   }
@@ -410,7 +410,7 @@ static int export_rows(nnp_workspace* ws, const float* d_buf, float* h_out) {
 
 extern "C" int nnp_debug_daev(nnp_workspace* ws, float* h_daev) {
   if (!ws || !h_daev) return NNP_ERR_INVALID_ARG;
-  return export_rows(ws, ws->daev, h_daev);
+  return export_rows(ws, ws->daev, h_daev, true);
 }
 
 extern "C" int nnp_debug_atomic_energies(nnp_workspace* ws, float* h_e) {

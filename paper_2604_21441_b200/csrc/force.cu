@@ -35,7 +35,8 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   const uint32_t* __restrict__ rowR = nbrR + (size_t)ip * rcap;
   load_env(c, g, spos, rowR, nbrA + (size_t)ip * acap, nR, nA, ci, lane, e);
   const int Kc = grp->Kc;
-  const float* __restrict__ gi = daev + (size_t)(ip + grp->pad_shift[si]) * Kc;
+  // row of dE/dAEV in the piece-major tile layout: float4 piece q of this row = gi4[q * TILE_M]
+  const float4* __restrict__ gi4 = reinterpret_cast<const float4*>(daev + daev_off((size_t)(ip + grp->pad_shift[si]), 0, Kc));
 
   // ---- angular: p_ij for the angular neighbours, staged in Pacc
   if (nA <= 32) {
@@ -65,7 +66,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const int sk = e.slotA[k];
         const int s1 = min(sj, sk), s2 = max(sj, sk);
         const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
-        const float4* __restrict__ gb = reinterpret_cast<const float4*>(gi + grp->cpos[c.nRB + pidx] * BLK);
+        const float4* __restrict__ gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
         const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
         const float cc = c.cTheta * u;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
@@ -85,7 +86,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         float S0 = 0.f, S1 = 0.f, sV = 0.f;
 #pragma unroll
         for (int a = 0; a < NSHFA; ++a) {
-          const float4 g0 = gb[2 * a], g1 = gb[2 * a + 1];
+          const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
           float Wv = g0.x * F1[0], V = g0.x * dF1[0];
           Wv = fmaf(g0.y, F1[1], Wv); V = fmaf(g0.y, dF1[1], V);
           Wv = fmaf(g0.z, F1[2], Wv); V = fmaf(g0.z, dF1[2], V);
@@ -146,7 +147,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const int sk = e.slotA[k];
         const int s1 = min(sj, sk), s2 = max(sj, sk);
         const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
-        const float4* __restrict__ gb = reinterpret_cast<const float4*>(gi + grp->cpos[c.nRB + pidx] * BLK);
+        const float4* __restrict__ gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
         const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
         const float cc = c.cTheta * u;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
@@ -166,7 +167,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         float sW = 0.f, sV = 0.f;
 #pragma unroll
         for (int a = 0; a < NSHFA; ++a) {
-          const float4 g0 = gb[2 * a], g1 = gb[2 * a + 1];
+          const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
           float W = g0.x * F1[0], V = g0.x * dF1[0];
           W = fmaf(g0.y, F1[1], W); V = fmaf(g0.y, dF1[1], V);
           W = fmaf(g0.z, F1[2], W); V = fmaf(g0.z, dF1[2], V);
@@ -206,7 +207,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     if (q < nR) {
       const float4 uq = e.u[q];
       const int s = e.slotR[q];
-      const float4* __restrict__ gr = reinterpret_cast<const float4*>(gi + grp->cpos[s >> 1] * BLK + (s & 1) * 16);
+      const float4* __restrict__ gr = gi4 + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * TILE_M;
       const float f = e.wR[q];   // c_R f_C
       float fc, dfc;
       cutoff(fminf(uq.w, c.Rcr), c.inv_Rcr, fc, dfc);
@@ -214,7 +215,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
       float coef = 0.f;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
-        const float4 gv = gr[v];
+        const float4 gv = gr[v * TILE_M];
         const float gg[4] = {gv.x, gv.y, gv.z, gv.w};
 #pragma unroll
         for (int t = 0; t < 4; ++t) {

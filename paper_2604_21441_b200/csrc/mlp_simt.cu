@@ -92,7 +92,7 @@ k_dense(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __rest
       float v = acc[i][j];
       if (mode == 0) v = celu_f(v + net.b[layer][n], net.alpha);
       else if (mode == 1) v *= celu_grad_from_act(act[row * ldact + n], net.alpha);
-      out[row * ldout + n] = v;
+      if (mode == 2) out[daev_off(row, n, ldout)] = v; else out[row * ldout + n] = v;
     }
   }
 }
@@ -120,7 +120,7 @@ k_last(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __restr
       const int km = (nl == 1) ? grp->blkmap[k >> 5] * BLK + (k & 31) : k;
       const float a = in[row * ldin + k], wk = w[km];
       s = fmaf(a, wk, s);
-      dz[row * lddz + k] = (nl == 1) ? wk : wk * celu_grad_from_act(a, net.alpha);
+      if (nl == 1) dz[daev_off(row, k, lddz)] = wk; else dz[row * lddz + k] = wk * celu_grad_from_act(a, net.alpha);
     }
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == 0) e_atom[row] = s + net.b[nl - 1][0];

@@ -488,7 +488,7 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
         const int nc = tc_nchunks(Kc), ch = tc_chunk(Kc);
         for (int c0 = 0; c0 < nc; c0 += 2) {
           const int n0 = c0 * ch, ncols = min(Kc, (c0 + 2) * ch) - n0;
-          float* __restrict__ dst = daev + (size_t)(ti.row0 + row) * Kc + n0;
+          float* __restrict__ dst = daev + daev_off((size_t)(ti.row0 + row), n0, Kc);   // piece-major tile layout
 #pragma unroll 1
           for (int j = part; j * 16 < ncols; j += TC_NPART) {
             uint32_t v[16];
@@ -497,7 +497,7 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
             if (valid) {
 #pragma unroll
               for (int i = 0; i < 16; i += 4)
-                *reinterpret_cast<uint4*>(dst + j * 16 + i) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+                *reinterpret_cast<uint4*>(dst + (size_t)(j * 4 + (i >> 2)) * (4 * TILE_M)) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
             }
           }
           if (c0 + 2 < nc) signal_and_wait();

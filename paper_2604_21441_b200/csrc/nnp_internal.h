@@ -77,6 +77,13 @@ struct GroupInfo {
 
 struct TileInfo { int slot, row0, nvalid, pad; };
 
+// dE/dAEV is stored tile-wise "piece-major": within the 128-row tile of a row, the float4 piece q = col / 4 of all
+// 128 rows is contiguous (2 KB).  The MLP epilogue (thread = row) then writes 512 contiguous bytes per warp store,
+// and the AEV backward kernel, which only reads float4 pieces, finds the pieces of neighbouring rows in one line.
+__host__ __device__ inline size_t daev_off(size_t row, int col, int Kc) {
+  return (row >> 7) * ((size_t)Kc * TILE_M) + (size_t)(col >> 2) * (4 * TILE_M) + (row & (TILE_M - 1)) * 4 + (col & 3);
+}
+
 struct Net {             // device pointers, one per slot
   int n_layers;
   int dims[MAX_LAYERS + 1];
