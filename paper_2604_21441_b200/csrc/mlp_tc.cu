@@ -95,6 +95,40 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
       "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
+// One k-step (K = 16) of the tile product, issued by one elected lane of a CONVERGED warp (predicated, so the
+// compiler emits straight-line code instead of a per-thread retry loop): hi*hi (+ lo*hi + hi*lo for the split).
+template <int NPASS>
+__device__ __forceinline__ void tc_mma_step(uint32_t d_tmem, uint64_t a_hi, uint64_t a_lo, uint64_t b_hi, uint64_t b_lo,
+                                            uint32_t idesc, uint32_t acc) {
+  if (NPASS == 3) {
+    asm volatile(
+        "{\n"
+        ".reg .pred pe, pa, pt;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "setp.ne.b32 pa, %6, 0;\n"
+        "setp.eq.b32 pt, %6, %6;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %3, %5, pa;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %2, %3, %5, pt;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %4, %5, pt;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_hi), "l"(a_lo), "l"(b_hi), "l"(b_lo), "r"(idesc), "r"(acc) : "memory");
+  } else {
+    asm volatile(
+        "{\n"
+        ".reg .pred pe, pa;\n"
+        "elect.sync _|pe, 0xffffffff;\n"
+        "setp.ne.b32 pa, %4, 0;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, pa;\n"
+        "}\n" ::"r"(d_tmem), "l"(a_hi), "l"(b_hi), "r"(idesc), "r"(acc) : "memory");
+  }
+}
+__device__ __forceinline__ void tc_commit_elect(uint32_t bar) {
+  asm volatile(
+      "{\n"
+      ".reg .pred pe;\n"
+      "elect.sync _|pe, 0xffffffff;\n"
+      "@pe tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n"
+      "}\n" ::"r"(bar) : "memory");
+}
 // K-major SWIZZLE_128B shared-memory matrix descriptor: start address >> 4, LBO (unused for swizzled K-major) = 1,
 // SBO = 1024 B between 8-row atoms, descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.
 __device__ __forceinline__ uint64_t tc_desc(uint32_t saddr) {
@@ -209,7 +243,7 @@ constexpr uint32_t TC_P1 = 0, TC_P2 = 128;            // TMEM columns of the pac
 
 template <int NPASS> struct TcCfg {
   static constexpr int NH = (NPASS == 3) ? 2 : 1;
-  static constexpr int NST = (NPASS == 3) ? 3 : 4;
+  static constexpr int NST = (NPASS == 3) ? 3 : 6;
   static constexpr uint32_t ABUF = NH * 4 * TC_PANEL;
   static constexpr uint32_t STAGE = NH * TC_PANEL;
   static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], a_ready, acc_full
@@ -225,17 +259,27 @@ struct TileNet {
 
 // The six GEMMs of one tile as "rounds": a round reads the A operand resident in shared memory (<= 4 K-panels) and
 // fills <= 256 accumulator columns (<= 2 N-chunks).  F1 is K-streamed in rounds of 4 panels when Kc > 256, B1 is
-// N-streamed in rounds of 2 chunks when Kc > 256.  f(img, N, K, c0, c1, p0, p1, accumulate_onto_previous_round).
-template <class F>
-__device__ __forceinline__ void tc_for_rounds(const TileNet& t, F&& f) {
+// N-streamed in rounds of 2 chunks when Kc > 256.  The producer and the MMA issuer walk the same table with ONE
+// copy of their block loop (an inlined copy per GEMM made the kernel overflow the instruction cache).
+struct TcRound {
+  const uint8_t* img;   // B image [N][K]
+  int N, K, c0, c1, p0, p1, acc_first;
+};
+constexpr int TC_MAX_ROUNDS = 16;
+
+__device__ __forceinline__ int tc_build_rounds(const TileNet& t, TcRound* r) {
+  int n = 0;
   const int np = tc_npanels(t.Kc);
-  for (int p0 = 0; p0 < np; p0 += 4) f(t.f1, t.N1, t.Kc, 0, tc_nchunks(t.N1), p0, min(np, p0 + 4), p0 > 0);
-  f(t.w2, t.N2, t.N1, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N1), false);
-  f(t.w3, t.N3, t.N2, 0, tc_nchunks(t.N3), 0, tc_npanels(t.N2), false);
-  f(t.w3t, t.N2, t.N3, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N3), false);
-  f(t.w2t, t.N1, t.N2, 0, tc_nchunks(t.N1), 0, tc_npanels(t.N2), false);
+  for (int p0 = 0; p0 < np && n < TC_MAX_ROUNDS - 5; p0 += 4)
+    r[n++] = TcRound{t.f1, t.N1, t.Kc, 0, tc_nchunks(t.N1), p0, min(np, p0 + 4), p0 > 0};
+  r[n++] = TcRound{t.w2, t.N2, t.N1, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N1), 0};
+  r[n++] = TcRound{t.w3, t.N3, t.N2, 0, tc_nchunks(t.N3), 0, tc_npanels(t.N2), 0};
+  r[n++] = TcRound{t.w3t, t.N2, t.N3, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N3), 0};
+  r[n++] = TcRound{t.w2t, t.N1, t.N2, 0, tc_nchunks(t.N1), 0, tc_npanels(t.N2), 0};
   const int nc = tc_nchunks(t.Kc);
-  for (int c0 = 0; c0 < nc; c0 += 2) f(t.b1, t.Kc, t.N1, c0, min(nc, c0 + 2), 0, tc_npanels(t.N1), false);
+  for (int c0 = 0; c0 < nc && n < TC_MAX_ROUNDS; c0 += 2)
+    r[n++] = TcRound{t.b1, t.Kc, t.N1, c0, min(nc, c0 + 2), 0, tc_npanels(t.N1), 0};
+  return n;
 }
 
 template <int NPASS>
@@ -298,28 +342,47 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       int s = 0; uint32_t ph = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         TileInfo ti; TileNet tn; tile_net(t, ti, tn);
-        tc_for_rounds(tn, [&](const uint8_t* img, int N, int K, int c0, int c1, int p0, int p1, bool) {
+        TcRound rd[TC_MAX_ROUNDS];
+        const int nrd = tc_build_rounds(tn, rd);
+#pragma unroll 1
+        for (int ir = 0; ir < nrd; ++ir) {
+          const uint8_t* img = rd[ir].img;
+          const int N = rd[ir].N, K = rd[ir].K, c0 = rd[ir].c0, c1 = rd[ir].c1, p0 = rd[ir].p0, p1 = rd[ir].p1;
           const int ch = tc_chunk(N);
           for (int c = c0; c < c1; ++c) {
             const uint32_t bytes = (uint32_t)min(ch, N - c * ch) * 128u;
             for (int p = p0; p < p1; ++p) {
               mbar_wait(bar_empty + 8 * s, ph ^ 1);
               mbar_expect_tx(bar_full + 8 * s, bytes * C::NH);
-              bulk_g2s(stage0 + s * C::STAGE, img + tc_blk_off(N, K, c, p, 0), bytes, bar_full + 8 * s);
-              if (C::NH == 2) bulk_g2s(stage0 + s * C::STAGE + TC_PANEL, img + tc_blk_off(N, K, c, p, 1), bytes, bar_full + 8 * s);
+              // each half-block goes out as four bulk copies: more requests in flight towards the L2 slices
+              const uint32_t qb = bytes >> 2;
+#pragma unroll
+              for (int h = 0; h < C::NH; ++h) {
+                const uint8_t* src = img + tc_blk_off(N, K, c, p, h);
+                const uint32_t dst = stage0 + s * C::STAGE + h * TC_PANEL;
+#pragma unroll
+                for (int u = 0; u < 4; ++u) bulk_g2s(dst + u * qb, src + u * qb, qb, bar_full + 8 * s);
+              }
               if (++s == C::NST) { s = 0; ph ^= 1; }
             }
           }
-        });
+        }
       }
     }
   } else if (warp == TC_EPI_WARPS + 1) {
-    // ===== MMA issuer: one thread =====
-    if (lane == 0) {
+    // ===== MMA issuer: the warp stays converged, tcgen05 ops are predicated on one elected lane.  Descriptors are
+    // built once per block and advanced by 32 B (+2 in the address field) per k-step: the issue loop must stay a
+    // handful of instructions per MMA, or the single issuing warp, not the tensor core, paces the GEMM. =====
+    {
       int s = 0; uint32_t ph = 0, aph = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         TileInfo ti; TileNet tn; tile_net(t, ti, tn);
-        tc_for_rounds(tn, [&](const uint8_t*, int N, int K, int c0, int c1, int p0, int p1, bool acc_first) {
+        TcRound rd[TC_MAX_ROUNDS];
+        const int nrd = tc_build_rounds(tn, rd);
+#pragma unroll 1
+        for (int ir = 0; ir < nrd; ++ir) {
+          const int N = rd[ir].N, K = rd[ir].K, c0 = rd[ir].c0, c1 = rd[ir].c1, p0 = rd[ir].p0, p1 = rd[ir].p1;
+          const bool acc_first = rd[ir].acc_first != 0;
           mbar_wait(bar_aready, aph); aph ^= 1;   // A operand in place, accumulator columns drained
           tc_fence_after();
           const int ch = tc_chunk(N);
@@ -331,20 +394,21 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
               tc_fence_after();
               const int nks = min(4, (K - p * 64) >> 4);
               const uint32_t a0 = abuf + (uint32_t)(p - p0) * TC_PANEL, b0 = stage0 + s * C::STAGE;
-              for (int ks = 0; ks < nks; ++ks) {
-                const uint64_t ah = tc_desc(a0 + ks * 32), bh = tc_desc(b0 + ks * 32);
-                tc_mma(d, ah, bh, idesc, (acc_first || p > p0 || ks > 0) ? 1u : 0u);
-                if (NPASS == 3) {
-                  tc_mma(d, tc_desc(a0 + TC_LO + ks * 32), bh, idesc, 1u);
-                  tc_mma(d, ah, tc_desc(b0 + TC_PANEL + ks * 32), idesc, 1u);
+              uint64_t ah = tc_desc(a0), al = tc_desc(a0 + TC_LO), bh = tc_desc(b0), bl = tc_desc(b0 + TC_PANEL);
+              uint32_t acc = (acc_first || p > p0) ? 1u : 0u;
+#pragma unroll
+              for (int ks = 0; ks < 4; ++ks) {
+                if (ks < nks) {
+                  tc_mma_step<NPASS>(d, ah, al, bh, bl, idesc, acc);
+                  acc = 1u; ah += 2; al += 2; bh += 2; bl += 2;
                 }
               }
-              tc_commit(bar_empty + 8 * s);       // frees the stage when these MMAs have read it
+              tc_commit_elect(bar_empty + 8 * s);  // frees the stage when these MMAs have read it
               if (++s == C::NST) { s = 0; ph ^= 1; }
             }
           }
-          tc_commit(bar_acc);                      // accumulator complete (and the A operand no longer read)
-        });
+          tc_commit_elect(bar_acc);                // accumulator complete (and the A operand no longer read)
+        }
       }
     }
   } else {
@@ -359,7 +423,11 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       fence_proxy_async();
       if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
       mbar_arrive(bar_aready);
-      mbar_wait(bar_acc, fph); fph ^= 1;
+      // ONE thread polls the mbarrier; the other 511 sleep in a hardware named barrier.  (512 threads spinning on
+      // try_wait flood the shared-memory pipe that feeds the tensor core's operand reads.)
+      if (threadIdx.x == 0) mbar_wait(bar_acc, fph);
+      fph ^= 1;
+      asm volatile("bar.sync 2, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
       tc_fence_after();
       if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
     };
