@@ -28,6 +28,12 @@ __device__ __forceinline__ float ex2f(float x) {
   return y;
 }
 
+__device__ __forceinline__ float lg2f(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // f_C(R;Rc) = 0.5 cos(pi R / Rc) + 0.5 and its derivative (App. A "Cut-off"); R <= Rc is guaranteed by the list.
 __device__ __forceinline__ void cutoff(float R, float inv_Rc, float& f, float& df) {
   const float x = 3.14159265358979f * R * inv_Rc;      // in [0, pi]: sin.approx / cos.approx err < 2^-21 absolute

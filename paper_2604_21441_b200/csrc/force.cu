@@ -25,7 +25,16 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
                const float* __restrict__ daev, unsigned long long* __restrict__ facc) {
   __shared__ WarpEnv env[AEV_WARPS];
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
+  __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block, times TILE_M
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x < MAX_S * MAX_S) {
+    const int sa = threadIdx.x / MAX_S, sb = threadIdx.x % MAX_S;
+    const int s1 = min(sa, sb), s2 = max(sa, sb);
+    int off = 0;
+    if (s2 < c.S) { const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)]; off = max(cp, 0) * (BLK / 4) * TILE_M; }
+    pairoff[threadIdx.x] = off;
+  }
+  __syncthreads();
   const int ip = blockIdx.x * AEV_WARPS + w;
   if (ip >= n_ml) return;
   WarpEnv& e = env[w];
@@ -48,6 +57,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     const int NG = 32 / W, grp_id = lane / W, jl = lane & (W - 1);
     const bool act = jl < n;
     const int nrounds = n >> 1;
+    const float zm1 = c.zeta - 1.0f;
     float px = 0.f, py = 0.f, pz = 0.f;
     float4 uj = make_float4(0.f, 0.f, 1.f, 1.f);
     float fj = 0.f, dfj = 0.f;
@@ -64,9 +74,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const float4 uk = e.ua[k];
         const float fk = e.fA[k], dfk = e.dfA[k];
         const int sk = e.slotA[k];
-        const int s1 = min(sj, sk), s2 = max(sj, sk);
-        const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
-        const float4* __restrict__ gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
+        const float4* __restrict__ gb = gi4 + pairoff[sj * MAX_S + sk];
         const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
         const float cc = c.cTheta * u;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
@@ -76,10 +84,9 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         for (int z = 0; z < NSHFZ; ++z) {
           const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
           const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
-          const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 0.f);
-          float Bz, Bm;
-          bpow(c, B, Bz, Bm);
-          F1[z] = Bz;
+          const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 1e-30f);    // floor keeps lg2 finite (B^(zeta-1) -> 0 or 1)
+          const float Bm = ex2f(zm1 * lg2f(B));                     // B^(zeta-1): two MUFU ops
+          F1[z] = Bm * B;
           dF1[z] = kd * Bm * sind;                                  // dF1/du
         }
         const float Rbar = 0.5f * (uj.w + uk.w);
