@@ -85,6 +85,21 @@ def mlp_flops_per_atom(dims, K0):
     return 4 * sum(d[i] * d[i + 1] for i in range(len(d) - 1))
 
 
+def max_over_ranks(dist, vals, device):
+    """Every rank gets the element-wise maximum over ranks of `vals` (timings: a multi-GPU number is the slowest rank's)."""
+    import torch
+    if dist is None:
+        return [float(v) for v in vals]
+    t = torch.tensor(vals, dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def replica_seed(base, rank):
+    """Replicas are independent boxes of the same shape: rank r perturbs the positions with its own seed."""
+    return base + 1000 * rank
+
+
 def run_reference(args, rank):
     """The oracle as it stands on the host cores; each step = one evaluation of a sub-box of the same generator,
     density and model, sized so that the whole run ends within a few minutes."""
@@ -93,7 +108,7 @@ def run_reference(args, rank):
     import oracle
     cfg = gen.get_config(2)
     om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
-    budget_s = 150.0 / max(args.steps + args.warmup, 1)
+    budget_s = args.ref_budget_s / max(args.steps + args.warmup, 1)
     n = int(min(20, max(4, (budget_s * 4000.0 / 3.0) ** (1.0 / 3.0))))
     if n == 20:
         pos, Z, box = cfg["pos"], cfg["Z"], cfg["box"]
@@ -129,7 +144,7 @@ def run_ours(args, rank, world, local_rank):
     cfg = gen.get_config(2)
     n = cfg["pos"].shape[0]
     # replicas: rank r perturbs with its own seed, so every GPU runs an independent box of the same shape
-    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"] + 1000 * rank, N_POS_SETS)
+    P = gen.perturbed_positions(cfg["pos64"], replica_seed(cfg["perturb_seed"], rank), N_POS_SETS)
     model = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
     ws = nnp.Workspace(model, n)
     if args.mlp_mode != "default":
@@ -195,10 +210,7 @@ def run_ours(args, rank, world, local_rank):
         e2e_s += time.perf_counter() - t0
     barrier()
 
-    if dist is not None:
-        tt = torch.tensor([total_s, e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_s, e2e_s = float(tt[0]), float(tt[1])
+    total_s, e2e_s = max_over_ranks(dist, [total_s, e2e_s], torch.device("cuda"))
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -267,6 +279,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

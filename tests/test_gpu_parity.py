@@ -237,6 +237,31 @@ def test_open_boundaries_cluster_and_orthorhombic_box():
     check_EF(Eg2, Fg2, ref2, len(pos2))
 
 
+def test_dense_blob_many_angular_neighbours():
+    """More than 32 angular neighbours per centre (far beyond liquid densities): exercises the backward kernel's
+    general pair loop and rows close to the angular capacity.  40 atoms in a 2.8 A sphere, open boundaries."""
+    rng = np.random.default_rng(5)
+    pts = []
+    while len(pts) < 40:
+        p = rng.uniform(-2.8, 2.8, 3)
+        if np.linalg.norm(p) <= 2.8 and all(np.linalg.norm(p - q) >= 0.75 for q in pts):
+            pts.append(p)
+    pos = (np.array(pts) + 20.0).astype(np.float32)
+    Z = rng.choice([1, 6, 7, 8], size=40).astype(np.int32)
+    cfg = gen.get_config(4)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    sub = dict(cfg, pos=pos, Z=Z, ml_index=None)
+    m, ws = make(sub)
+    ref = oracle.evaluate(om, pos, Z, cfg["box"], 0, None)
+    Eg, Fg = run_gpu(ws, pos, Z, cfg["box"], 0)
+    sA, _ = ws.neighbors(1, 40)
+    assert np.diff(sA).max() > 32, np.diff(sA).max()
+    check_lists(ws, cfg, pos, 40, None, pbc=0)
+    Fo = ref["forces"]
+    assert abs(Eg - ref["energy"]) / 40 <= E_TOL
+    assert np.sqrt(((Fg - Fo) ** 2).sum() / (Fo ** 2).sum()) <= F_RMS_TOL
+
+
 def test_one_layer_network_golden_monomer():
     """All-ones one-layer network on a water monomer: E = 7.1130060875."""
     import json, os
