@@ -384,6 +384,11 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
       const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
       const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
       const float4* cp = cand + lane;
+      // keep the row pointers and capacities in registers: rebuilding them from the kernel parameters every
+      // iteration costs more issue slots than the distance test itself
+      uint32_t* rR = rowR; uint8_t* rA = rowA;
+      int capR = rcap, capA = acap;
+      asm volatile("" : "+l"(rR), "+l"(rA), "+r"(capR), "+r"(capA));
       for (int q0 = lane; q0 - lane < nin; q0 += 32, cp += 32) {
         const float4 pj = (q0 < nin) ? *cp : make_float4(1.0e18f, 1.0e18f, 1.0e18f, __int_as_float(ip));
         uint32_t ent = (uint32_t)__float_as_int(pj.w);
@@ -411,8 +416,8 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
         const unsigned mR = __ballot_sync(0xffffffffu, inR);
         const unsigned mA = __ballot_sync(0xffffffffu, inA);
         const int pR = nR + __popc(mR & lt), pA = nA + __popc(mA & lt);
-        if (inR && pR < rcap) rowR[pR] = ent;
-        if (inA && pA < acap && pR < rcap) rowA[pA] = (uint8_t)pR;
+        if (inR && pR < capR) rR[pR] = ent;
+        if (inA && pA < capA && pR < capR) rA[pA] = (uint8_t)pR;
         nR += __popc(mR); nA += __popc(mA);
       }
       if (nR > rcap || nA > acap) bad |= FLAG_CAP;
