@@ -126,19 +126,29 @@ __global__ void k_bin(AevConst c, const GridInfo* __restrict__ g, const float* _
 }
 
 // ---------------------------------------------------------------- K1a: exclusive scan + groups + tiles
-__global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, const int* __restrict__ count,
+__global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
                                                int* __restrict__ bstart, GroupInfo* __restrict__ grp,
                                                TileInfo* __restrict__ tiles, int S, int n_ml, int max_tiles,
                                                int dense_k, int* __restrict__ flags) {
-  // block-wide exclusive scan of S * ncell bucket counts: each warp owns a contiguous span and sweeps it 32 at a
-  // time (coalesced, loads batched four deep), then the warp totals are scanned and added back.
+  // block-wide exclusive scan of S * ncell bucket counts: each warp owns a contiguous span.  Pass A sums the span
+  // (coalesced, loads batched four deep); pass B re-reads it (L1 hits), scans with the warp's base and writes the
+  // bucket starts.  The counts are zeroed behind the read, so the next evaluation needs no memset.
   __shared__ int wtot[32];
   __shared__ int gs[MAX_S + 1], tb[MAX_S + 1];
-  const int n = S * g->ncell;
+  const int ncell = g->ncell, n = S * ncell;
   const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
   const int span = (((n + 31) / 32 + 31) / 32) * 32;
   const int lo = min(wp * span, n), hi = min(lo + span, n);
-  int carry = 0;
+  int sum = 0;
+  for (int k0 = lo; k0 < hi; k0 += 128) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; sum += (k < hi) ? count[k] : 0; }
+  }
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if (lane == 0) wtot[wp] = sum;
+  __syncthreads();
+  int carry = 0, total = 0;
+  for (int w = 0; w < 32; ++w) { const int t = wtot[w]; if (w < wp) carry += t; total += t; }
   for (int k0 = lo; k0 < hi; k0 += 128) {
     int v[4];
 #pragma unroll
@@ -148,26 +158,16 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, c
       int inc = v[u];
       for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
       const int k = k0 + 32 * u + lane;
-      if (k < hi) bstart[k] = carry + inc - v[u];
+      if (k < hi) {
+        const int st = carry + inc - v[u];
+        bstart[k] = st;
+        count[k] = 0;
+        if (k % ncell == 0) gs[k / ncell] = st;    // first bucket of a species slot = start of its group
+      }
       carry += __shfl_sync(0xffffffffu, inc, 31);
     }
   }
-  if (lane == 0) wtot[wp] = carry;
-  __syncthreads();
-  int base = 0, total = 0;
-  for (int w = 0; w < 32; ++w) { const int t = wtot[w]; if (w < wp) base += t; total += t; }
-  if (base != 0) {
-    for (int k0 = lo; k0 < hi; k0 += 128) {
-      int v[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; v[u] = (k < hi) ? bstart[k] : 0; }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) { const int k = k0 + 32 * u + lane; if (k < hi) bstart[k] = v[u] + base; }
-    }
-  }
-  if (threadIdx.x == 0) { bstart[n] = total; if (total != n_ml) atomicOr(flags, FLAG_ARG); }
-  __syncthreads();
-  if (threadIdx.x <= S) gs[threadIdx.x] = bstart[threadIdx.x * g->ncell];
+  if (threadIdx.x == 0) { bstart[n] = total; gs[S] = total; if (total != n_ml) atomicOr(flags, FLAG_ARG); }
   __syncthreads();
   __shared__ int pshift[MAX_S];
   if (threadIdx.x == 0) {
@@ -437,7 +437,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   k_grid_setup<<<1, 1024, 0, st>>>(ws->grid, ws->groups, pbc, box[0], box[4], box[8], m->aev.Rcr, ws->max_cells,
                                    d_pos, d_ml, (int)n_ml);
   ++nl;
-  cudaMemsetAsync(ws->cell_count, 0, sizeof(int) * ((size_t)MAX_S * ws->max_cells + 1), st);
+  // cell_count is all zero here: allocated zeroed, and k_scan clears every count it reads
   const int nb = (int)((n_ml + 255) / 256);
   if (n_ml > 0) {
     k_bin<<<nb, 256, 0, st>>>(m->aev, ws->grid, d_pos, d_Z, d_ml, (int)n_atoms, (int)n_ml, ws->tmp4, ws->rank,
