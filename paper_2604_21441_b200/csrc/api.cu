@@ -168,6 +168,13 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
   ws->max_cells = (int)std::min<int64_t>(std::max<int64_t>(512, max_ml / 4), 1 << 21);
   ws->mlp_mode = m->tc ? NNP_MLP_F16X3 : NNP_MLP_FP32_SIMT;
   ws->dense_k = 0;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+      cudaGetLastError(); delete ws; return NNP_ERR_CUDA;
+    }
+    ws->num_sms = sms;
+  }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
   ws->max_rows = (int64_t)ws->max_tiles * TILE_M;
   const size_t nm = (size_t)max_ml, nr = (size_t)ws->max_rows, K = (size_t)m->Kfull;

@@ -10,7 +10,11 @@
 //  * the neighbour predicate is the pinned fp64 expression of SURVEY.md section 8.c step 2 (reading #6):
 //    fp32 decides outside a guard band, inside it the expression is re-evaluated in fp64 from the original
 //    fp32 coordinates, so lists are bit-identical to the oracle's O(N^2) definition.
+#include <cooperative_groups.h>
+#include <algorithm>
 #include "nnp_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace nnp {
 
@@ -21,7 +25,7 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 }
 
 // ---------------------------------------------------------------- grid setup (1 block)
-__global__ void k_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, float Ly, float Lz, float Rcr,
+__device__ void d_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, float Ly, float Lz, float Rcr,
                              int max_cells, const float* __restrict__ pos, const int32_t* __restrict__ ml,
                              int n_ml) {
   __shared__ float smin[3][32], smax[3][32];
@@ -83,11 +87,11 @@ __global__ void k_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, flo
 }
 
 // ---------------------------------------------------------------- K0: species map, ML gather, cell key
-__global__ void k_bin(AevConst c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
+__device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
                       const int32_t* __restrict__ Z, const int32_t* __restrict__ ml, int n_atoms, int n_ml,
                       float4* __restrict__ tmp4, int* __restrict__ rank, int* __restrict__ cell_count,
                       unsigned long long* __restrict__ facc, int* __restrict__ flags) {
-  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  int a = vb * blockDim.x + threadIdx.x;
   if (a >= n_ml) return;
   int i = a;
   if (ml) {
@@ -126,7 +130,7 @@ __global__ void k_bin(AevConst c, const GridInfo* __restrict__ g, const float* _
 }
 
 // ---------------------------------------------------------------- K1a: exclusive scan + groups + tiles
-__global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
+__device__ void d_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
                                                int* __restrict__ bstart, GroupInfo* __restrict__ grp,
                                                TileInfo* __restrict__ tiles, int S, int n_ml, int max_tiles,
                                                int dense_k, int* __restrict__ flags) {
@@ -228,10 +232,10 @@ __global__ void __launch_bounds__(1024) k_scan(const GridInfo* __restrict__ g, i
 }
 
 // ---------------------------------------------------------------- K1b: scatter into slot-major cell order
-__global__ void k_scatter(const GridInfo* __restrict__ g, const float4* __restrict__ tmp4,
+__device__ void d_scatter(int vb, const GridInfo* __restrict__ g, const float4* __restrict__ tmp4,
                           const int* __restrict__ rank, const int* __restrict__ bstart, int n_ml,
                           float4* __restrict__ spos, int* __restrict__ scell) {
-  int a = blockIdx.x * blockDim.x + threadIdx.x;
+  int a = vb * blockDim.x + threadIdx.x;
   if (a >= n_ml) return;
   float4 t = tmp4[a];
   int key = __float_as_int(t.w);
@@ -245,9 +249,9 @@ __global__ void k_scatter(const GridInfo* __restrict__ g, const float4* __restri
 // K1c: the atomic ranks above are not reproducible; order every bucket by ML index so that the sorted order
 // (and with it every summation order downstream) is identical from run to run.  One warp per bucket: buckets of
 // <= 32 atoms are ranked by counting (all-pairs compare through shuffles); longer ones fall back to one lane.
-__global__ void __launch_bounds__(256) k_bucket_sort(const GridInfo* __restrict__ g, int S,
+__device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S,
                                                      const int* __restrict__ bstart, float4* __restrict__ spos) {
-  const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  const int k = (vb * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= S * g->ncell) return;
   const int lo = bstart[k], n = bstart[k + 1] - lo;
   if (n <= 1) return;
@@ -427,35 +431,67 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
   if (bad) atomicOr(flags, bad);
 }
 
+// ---------------------------------------------------------------- K0-K1 as ONE cooperative kernel
+// grid setup -> binning -> scan -> scatter -> bucket ordering are five dependent steps over < 1 MB: as separate
+// launches each costs a launch + drain (~4 us); here they are phases of one persistent grid separated by grid-wide
+// barriers.  Blocks of 1024 threads, one per SM at most (co-residency is what makes the barrier legal).
+struct PrepArgs {
+  AevConst c;
+  GridInfo* grid; GroupInfo* groups; TileInfo* tiles;
+  const float* pos; const int32_t* Z; const int32_t* ml;
+  float4* tmp4; int* rank; int* cell_count; int* bstart; float4* spos; int* scell;
+  unsigned long long* facc; int* flags;
+  float Lx, Ly, Lz;
+  int pbc, n_atoms, n_ml, max_cells, max_tiles, dense_k;
+};
+
+__global__ void __launch_bounds__(1024, 1) k_prep(PrepArgs a) {
+  cg::grid_group gridg = cg::this_grid();
+  const int S = a.c.S;
+  if (blockIdx.x == 0)
+    d_grid_setup(a.grid, a.groups, a.pbc, a.Lx, a.Ly, a.Lz, a.c.Rcr, a.max_cells, a.pos, a.ml, a.n_ml);
+  gridg.sync();
+  const int nbA = (a.n_ml + (int)blockDim.x - 1) / (int)blockDim.x;
+  for (int vb = blockIdx.x; vb < nbA; vb += gridDim.x)
+    d_bin(vb, a.c, a.grid, a.pos, a.Z, a.ml, a.n_atoms, a.n_ml, a.tmp4, a.rank, a.cell_count, a.facc, a.flags);
+  gridg.sync();
+  if (blockIdx.x == 0)
+    d_scan(a.grid, a.cell_count, a.bstart, a.groups, a.tiles, S, a.n_ml, a.max_tiles, a.dense_k, a.flags);
+  gridg.sync();
+  for (int vb = blockIdx.x; vb < nbA; vb += gridDim.x)
+    d_scatter(vb, a.grid, a.tmp4, a.rank, a.bstart, a.n_ml, a.spos, a.scell);
+  gridg.sync();
+  const int nbS = (S * a.grid->ncell * 32 + (int)blockDim.x - 1) / (int)blockDim.x;
+  for (int vb = blockIdx.x; vb < nbS; vb += gridDim.x) d_bucket_sort(vb, a.grid, S, a.bstart, a.spos);
+}
+
 // ---------------------------------------------------------------- host launcher
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml) {
   const nnp_model* m = ws->model;
   cudaStream_t st = ws->stream;
-  const int S = m->aev.S;
-  int nl = 0;
-  k_grid_setup<<<1, 1024, 0, st>>>(ws->grid, ws->groups, pbc, box[0], box[4], box[8], m->aev.Rcr, ws->max_cells,
-                                   d_pos, d_ml, (int)n_ml);
-  ++nl;
-  // cell_count is all zero here: allocated zeroed, and k_scan clears every count it reads
-  const int nb = (int)((n_ml + 255) / 256);
+  // cell_count is all zero here: allocated zeroed, and the scan phase clears every count it reads
+  PrepArgs a;
+  a.c = m->aev;
+  a.grid = ws->grid; a.groups = ws->groups; a.tiles = ws->tiles;
+  a.pos = d_pos; a.Z = d_Z; a.ml = d_ml;
+  a.tmp4 = ws->tmp4; a.rank = ws->rank; a.cell_count = ws->cell_count; a.bstart = ws->bstart; a.spos = ws->spos;
+  a.scell = ws->scell; a.facc = ws->facc; a.flags = ws->flags;
+  a.Lx = box[0]; a.Ly = box[4]; a.Lz = box[8];
+  a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
+  a.dense_k = ws->dense_k;
+  // enough blocks for the atoms and the buckets, never more than one per SM (co-residency)
+  const int64_t want = std::max<int64_t>((n_ml + 1023) / 1024, ((int64_t)m->aev.S * ws->max_cells * 32 + 1023) / 1024);
+  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, ws->num_sms));
+  void* args[] = {&a};
+  cudaLaunchCooperativeKernel((const void*)k_prep, dim3(grid), dim3(1024), args, 0, st);
+  int nl = 1;
   if (n_ml > 0) {
-    k_bin<<<nb, 256, 0, st>>>(m->aev, ws->grid, d_pos, d_Z, d_ml, (int)n_atoms, (int)n_ml, ws->tmp4, ws->rank,
-                              ws->cell_count, ws->facc, ws->flags);
-    ++nl;
-  }
-  k_scan<<<1, 1024, 0, st>>>(ws->grid, ws->cell_count, ws->bstart, ws->groups, ws->tiles, S, (int)n_ml,
-                             ws->max_tiles, ws->dense_k, ws->flags);
-  ++nl;
-  if (n_ml > 0) {
-    k_scatter<<<nb, 256, 0, st>>>(ws->grid, ws->tmp4, ws->rank, ws->bstart, (int)n_ml, ws->spos, ws->scell);
-    // the bucket count is only known on the device: launch for the capacity, guard on S * ncell inside
-    k_bucket_sort<<<(S * ws->max_cells + 7) / 8, 256, 0, st>>>(ws->grid, S, ws->bstart, ws->spos);
     // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside
     k_neighbors<<<ws->max_cells, 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->bstart, d_pos, d_ml,
                                                (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
                                                ws->flags);
-    nl += 3;
+    ++nl;
   }
   return nl;
 }

@@ -113,6 +113,7 @@ struct nnp_workspace {
   int64_t max_atoms, max_ml;
   int rcap, acap;            // neighbour row capacities
   int max_cells;
+  int num_sms;               // multiprocessor count of the device (cooperative grid size)
   int mlp_mode;
   int dense_k;               // 1: materialise every column block (no structural-zero compaction)
   int64_t max_rows;          // padded AEV rows
