@@ -174,6 +174,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
       cudaGetLastError(); delete ws; return NNP_ERR_CUDA;
     }
     ws->num_sms = sms;
+    ws->prep_cluster = prep_cluster_size();
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
   ws->max_rows = (int64_t)ws->max_tiles * TILE_M;

@@ -445,27 +445,50 @@ struct PrepArgs {
   int pbc, n_atoms, n_ml, max_cells, max_tiles, dense_k;
 };
 
+// CLUSTER = true: the whole grid is ONE thread-block cluster (<= 16 CTAs) and the phases are separated by the
+// hardware cluster barrier (~0.2 us) -- these steps are latency-bound, a few SMs are plenty up to ~1e5 atoms.
+// CLUSTER = false: cooperative launch over up to one CTA per SM with grid-wide barriers (larger systems).
+template <bool CLUSTER>
 __global__ void __launch_bounds__(1024, 1) k_prep(PrepArgs a) {
-  cg::grid_group gridg = cg::this_grid();
+  auto sync_all = [&]() {
+    if (CLUSTER) cg::this_cluster().sync(); else cg::this_grid().sync();
+  };
   const int S = a.c.S;
   if (blockIdx.x == 0)
     d_grid_setup(a.grid, a.groups, a.pbc, a.Lx, a.Ly, a.Lz, a.c.Rcr, a.max_cells, a.pos, a.ml, a.n_ml);
-  gridg.sync();
+  sync_all();
   const int nbA = (a.n_ml + (int)blockDim.x - 1) / (int)blockDim.x;
   for (int vb = blockIdx.x; vb < nbA; vb += gridDim.x)
     d_bin(vb, a.c, a.grid, a.pos, a.Z, a.ml, a.n_atoms, a.n_ml, a.tmp4, a.rank, a.cell_count, a.facc, a.flags);
-  gridg.sync();
+  sync_all();
   if (blockIdx.x == 0)
     d_scan(a.grid, a.cell_count, a.bstart, a.groups, a.tiles, S, a.n_ml, a.max_tiles, a.dense_k, a.flags);
-  gridg.sync();
+  sync_all();
   for (int vb = blockIdx.x; vb < nbA; vb += gridDim.x)
     d_scatter(vb, a.grid, a.tmp4, a.rank, a.bstart, a.n_ml, a.spos, a.scell);
-  gridg.sync();
+  sync_all();
   const int nbS = (S * a.grid->ncell * 32 + (int)blockDim.x - 1) / (int)blockDim.x;
   for (int vb = blockIdx.x; vb < nbS; vb += gridDim.x) d_bucket_sort(vb, a.grid, S, a.bstart, a.spos);
 }
 
 // ---------------------------------------------------------------- host launcher
+// Largest cluster (16, else the portable 8) that can hold k_prep's 1024-thread CTAs on this device; 0 = none.
+int prep_cluster_size() {
+  cudaFuncSetAttribute((const void*)k_prep<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  for (int cs = 16; cs >= 8; cs >>= 1) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cs); cfg.blockDim = dim3(1024);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    int ncl = 0;
+    if (cudaOccupancyMaxActiveClusters(&ncl, (const void*)k_prep<true>, &cfg) == cudaSuccess && ncl >= 1) return cs;
+    cudaGetLastError();
+  }
+  return 0;
+}
+
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml) {
   const nnp_model* m = ws->model;
@@ -480,11 +503,21 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.Lx = box[0]; a.Ly = box[4]; a.Lz = box[8];
   a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
   a.dense_k = ws->dense_k;
-  // enough blocks for the atoms and the buckets, never more than one per SM (co-residency)
-  const int64_t want = std::max<int64_t>((n_ml + 1023) / 1024, ((int64_t)m->aev.S * ws->max_cells * 32 + 1023) / 1024);
-  const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, ws->num_sms));
   void* args[] = {&a};
-  cudaLaunchCooperativeKernel((const void*)k_prep, dim3(grid), dim3(1024), args, 0, st);
+  if (ws->prep_cluster > 0 && n_ml <= 8192) {   // small systems: barrier latency dominates, a few SMs suffice
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ws->prep_cluster); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = ws->prep_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelExC(&cfg, (const void*)k_prep<true>, args);
+  } else {
+    // enough blocks for the atoms and the buckets, never more than one per SM (co-residency)
+    const int64_t want = std::max<int64_t>((n_ml + 1023) / 1024, ((int64_t)m->aev.S * ws->max_cells * 32 + 1023) / 1024);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, ws->num_sms));
+    cudaLaunchCooperativeKernel((const void*)k_prep<false>, dim3(grid), dim3(1024), args, 0, st);
+  }
   int nl = 1;
   if (n_ml > 0) {
     // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside

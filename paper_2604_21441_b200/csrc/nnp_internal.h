@@ -114,6 +114,7 @@ struct nnp_workspace {
   int rcap, acap;            // neighbour row capacities
   int max_cells;
   int num_sms;               // multiprocessor count of the device (cooperative grid size)
+  int prep_cluster;          // CTAs of the single-cluster prep kernel (0: cooperative grid only)
   int mlp_mode;
   int dense_k;               // 1: materialise every column block (no structural-zero compaction)
   int64_t max_rows;          // padded AEV rows
@@ -156,6 +157,7 @@ inline void prof_mark(nnp_workspace* ws, int i) { if (ws->profiling) cudaEventRe
 // stage launchers (each returns the number of kernels it launched)
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
+int prep_cluster_size();
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
