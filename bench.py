@@ -32,6 +32,12 @@ FLOP_FWD_PAIR, FLOP_FWD_TRIPLET = 16 * 6, 170
 FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's main kernel, from the committed ncu full-set
+# capture profiles/r01c_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
+NCU_TRAFFIC_BYTES = {"neighbour": 0.563e6 + 62.5e3, "aev_forward": 8.08e6, "mlp": 18.3e6 + 170e3, "aev_backward": 21.0e6,
+                     "output": 1.06e6}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -149,6 +155,8 @@ def run_ours(args, rank, world, local_rank):
     ws = nnp.Workspace(model, n)
     if args.mlp_mode != "default":
         ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "f16x3": nnp.NNP_MLP_F16X3, "f16x1": nnp.NNP_MLP_F16X1}[args.mlp_mode])
+    if args.dense_k:
+        ws.set_dense_k(1)
     dpos = [torch.from_numpy(P[t]).cuda() for t in range(N_POS_SETS)]
     dZ = torch.from_numpy(cfg["Z"]).cuda()
     E = torch.zeros(1, dtype=torch.float64, device="cuda")
@@ -222,7 +230,8 @@ def run_ours(args, rank, world, local_rank):
     stage_ms = stage / args.steps
     names = ["neighbour", "aev_forward", "mlp", "aev_backward", "output"]
     nH, nO = int((cfg["Z"] == 1).sum()), int((cfg["Z"] == 8).sum())
-    Kc = 160   # compacted AEV width for an H/O-only system: 2 radial + 3 angular 32-column blocks
+    # compacted AEV width for an H/O-only system: 2 radial + 3 angular 32-column blocks (dense-K: all 32 blocks)
+    Kc = 1024 if args.dense_k else 160
     mlp_flops = nH * mlp_flops_per_atom(cfg["nets"][1][0], Kc) + nO * mlp_flops_per_atom(cfg["nets"][8][0], Kc)
     work = {
         "neighbour": ("hbm", n * (16 + 32 + 8) + 4 * pairs_R + pairs_R // 4, pk["hbm"], "GB/s", 1e9),
@@ -240,7 +249,10 @@ def run_ours(args, rank, world, local_rank):
     dom = names[int(np.argmax(stage_ms))]
     roof = dict(stages[dom])
     roof.pop("ms")
-    roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md)", traffic=None)
+    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k
+    roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
+                traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
+                traffic_source="profiles/r01c_launches.md (ncu --set full, per launch)")
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -259,7 +271,7 @@ def run_ours(args, rank, world, local_rank):
         "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "atoms_per_gpu": n, "position_sets": N_POS_SETS,
-                   "l2": "flushed between timed steps (256 MiB write)", "mlp_mode": args.mlp_mode,
+                   "l2": "flushed between timed steps (256 MiB write)", "mlp_mode": args.mlp_mode, "dense_k": bool(args.dense_k),
                    "radial_pairs": pairs_R, "triplets": triplets, "parallelism": f"replicas x{world}"},
         "ns_per_day_2fs": 0.1728 * args.steps / total_s,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 12 * n + 8,
@@ -274,10 +286,11 @@ def run_ours(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
+    ap.add_argument("--dense-k", action="store_true", help="materialise all 1008 AEV columns (K = 1024 first layer)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")
     args = ap.parse_args()
