@@ -18,6 +18,56 @@ __device__ __forceinline__ long long shfl_xor_ll(long long v, int o) {
   return ((long long)hi << 32) | (unsigned int)lo;
 }
 
+// Both shares of one unordered angular pair {j,k} of centre i: oj = dE_i/dr_j and ok = dE_i/dr_k contributions of the
+// 32 sub-features of the pair's species block (SURVEY.md Appendix A "Forces"; gb = this centre's dE/dAEV pieces).
+struct PairShares { float jx, jy, jz, kx, ky, kz; };
+__device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, const float4* __restrict__ gb, float4 uj,
+                                                  float fj, float dfj, float4 uk, float fk, float dfk) {
+  const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
+  const float cc = c.cTheta * u;
+  const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
+  const float kd = 0.5f * c.zeta * c.cTheta / ss;            // -0.5 zeta dtheta/du
+  float F1[NSHFZ], dF1[NSHFZ];
+#pragma unroll
+  for (int z = 0; z < NSHFZ; ++z) {
+    const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
+    const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
+    const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 1e-30f);    // floor keeps lg2 finite (B^(zeta-1) -> 0 or 1)
+    const float Bm = ex2f(zm1 * lg2f(B));                     // B^(zeta-1): two MUFU ops
+    F1[z] = Bm * B;
+    dF1[z] = kd * Bm * sind;                                  // dF1/du
+  }
+  const float Rbar = 0.5f * (uj.w + uk.w);
+  float S0 = 0.f, S1 = 0.f, sV = 0.f;
+#pragma unroll
+  for (int a = 0; a < NSHFA; ++a) {
+    const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
+    float Wv = g0.x * F1[0], V = g0.x * dF1[0];
+    Wv = fmaf(g0.y, F1[1], Wv); V = fmaf(g0.y, dF1[1], V);
+    Wv = fmaf(g0.z, F1[2], Wv); V = fmaf(g0.z, dF1[2], V);
+    Wv = fmaf(g0.w, F1[3], Wv); V = fmaf(g0.w, dF1[3], V);
+    Wv = fmaf(g1.x, F1[4], Wv); V = fmaf(g1.x, dF1[4], V);
+    Wv = fmaf(g1.y, F1[5], Wv); V = fmaf(g1.y, dF1[5], V);
+    Wv = fmaf(g1.z, F1[6], Wv); V = fmaf(g1.z, dF1[6], V);
+    Wv = fmaf(g1.w, F1[7], Wv); V = fmaf(g1.w, dF1[7], V);
+    const float x = Rbar - c.ShfA[a];
+    const float F2 = ex2f(-c.etaA_l2e * x * x);
+    const float WF = Wv * F2;
+    S0 += WF; S1 = fmaf(WF, x, S1);
+    sV = fmaf(V, F2, sV);
+  }
+  // dt/dR_ij and dt/dR_ik (through Rbar and the cut-offs), dt/du
+  const float Aj = 2.0f * fk * fmaf(-c.etaA * fj, S1, dfj * S0);
+  const float Ak = 2.0f * fj * fmaf(-c.etaA * fk, S1, dfk * S0);
+  const float Au = 2.0f * fj * fk * sV;
+  const float qj = Au / uj.w, qk = Au / uk.w;
+  const float rj = Aj - qj * u, rk = Ak - qk * u;
+  PairShares o;
+  o.jx = fmaf(rj, uj.x, qj * uk.x); o.jy = fmaf(rj, uj.y, qj * uk.y); o.jz = fmaf(rj, uj.z, qj * uk.z);
+  o.kx = fmaf(rk, uk.x, qk * uj.x); o.ky = fmaf(rk, uk.y, qk * uj.y); o.kz = fmaf(rk, uk.z, qk * uj.z);
+  return o;
+}
+
 __global__ void __launch_bounds__(AEV_WARPS * 32, 4)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
@@ -49,92 +99,91 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
 
   // ---- angular: p_ij for the angular neighbours, staged in Pacc
   if (nA <= 32) {
-    // Every unordered pair {j,k} is evaluated ONCE and yields both p_ij and p_ik.  Lanes hold neighbours; in round m
-    // lane j pairs with k = (j + m) mod n, keeps its own share and hands k's share to lane k by shuffle (k <-> j is
-    // a permutation, so every lane receives exactly one share per round).  32 / W lane groups take alternate rounds.
+    // Every unordered pair {j,k} is evaluated ONCE and yields both p_ij and p_ik.
+    //  * within a subset of <= 16 neighbours: lanes hold neighbours; in round m lane j pairs with k = (j + m) mod n,
+    //    keeps its own share and hands k's share to lane k by shuffle (j -> k is a permutation, so every lane receives
+    //    exactly one share per round); the 32 / W lane groups take alternate rounds;
+    //  * 17..32 neighbours: A = the first 16, B = the rest: pairs within A, pairs within B, and the cross pairs
+    //    A x B with both 16-lane groups holding A and each taking every other k in B (k's share = a 16-lane butterfly).
+    // All orders are fixed by (round, lane): results are bitwise reproducible.  Pacc accumulates over the passes.
     const int n = nA;
-    const int W = (n <= 8) ? 8 : (n <= 16) ? 16 : 32;
-    const int NG = 32 / W, grp_id = lane / W, jl = lane & (W - 1);
-    const bool act = jl < n;
-    const int nrounds = n >> 1;
     const float zm1 = c.zeta - 1.0f;
-    float px = 0.f, py = 0.f, pz = 0.f;
-    float4 uj = make_float4(0.f, 0.f, 1.f, 1.f);
-    float fj = 0.f, dfj = 0.f;
-    int sj = 0;
-    if (act) { uj = e.ua[jl]; fj = e.fA[jl]; dfj = e.dfA[jl]; sj = e.slotA[jl]; }
-    for (int m0 = 1; m0 <= nrounds; m0 += NG) {
-      const int m = m0 + grp_id;
-      const bool last_half = ((n & 1) == 0) && (m == nrounds);   // even n: the round m = n/2 holds each pair twice
-      const bool on = act && m <= nrounds && (!last_half || jl < nrounds);
-      float qx = 0.f, qy = 0.f, qz = 0.f;
-      if (on) {
-        int k = jl + m;
-        if (k >= n) k -= n;
-        const float4 uk = e.ua[k];
-        const float fk = e.fA[k], dfk = e.dfA[k];
-        const int sk = e.slotA[k];
-        const float4* __restrict__ gb = gi4 + pairoff[sj * MAX_S + sk];
-        const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
-        const float cc = c.cTheta * u;
-        const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
-        const float kd = 0.5f * c.zeta * c.cTheta / ss;            // -0.5 zeta dtheta/du
-        float F1[NSHFZ], dF1[NSHFZ];
-#pragma unroll
-        for (int z = 0; z < NSHFZ; ++z) {
-          const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
-          const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
-          const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 1e-30f);    // floor keeps lg2 finite (B^(zeta-1) -> 0 or 1)
-          const float Bm = ex2f(zm1 * lg2f(B));                     // B^(zeta-1): two MUFU ops
-          F1[z] = Bm * B;
-          dF1[z] = kd * Bm * sind;                                  // dF1/du
+    for (int j = lane; j < n; j += 32) { Pacc[w][j][0] = 0.f; Pacc[w][j][1] = 0.f; Pacc[w][j][2] = 0.f; }
+    __syncwarp();
+    auto rr_pass = [&](int base, int ns) {
+      const int W = (ns <= 8) ? 8 : 16;
+      const int NG = 32 / W, grp_id = lane / W, jl = lane & (W - 1);
+      const bool act = jl < ns;
+      const int nrounds = ns >> 1;
+      float px = 0.f, py = 0.f, pz = 0.f;
+      float4 uj = make_float4(0.f, 0.f, 1.f, 1.f);
+      float fj = 0.f, dfj = 0.f;
+      int sj = 0;
+      if (act) { uj = e.ua[base + jl]; fj = e.fA[base + jl]; dfj = e.dfA[base + jl]; sj = e.slotA[base + jl]; }
+      for (int m0 = 1; m0 <= nrounds; m0 += NG) {
+        const int m = m0 + grp_id;
+        const bool last_half = ((ns & 1) == 0) && (m == nrounds);   // even ns: the round m = ns/2 holds each pair twice
+        const bool on = act && m <= nrounds && (!last_half || jl < nrounds);
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        if (on) {
+          int k = jl + m;
+          if (k >= ns) k -= ns;
+          k += base;
+          const PairShares o = pair_shares(c, zm1, gi4 + pairoff[sj * MAX_S + e.slotA[k]], uj, fj, dfj, e.ua[k], e.fA[k],
+                                           e.dfA[k]);
+          px += o.jx; py += o.jy; pz += o.jz;
+          qx = o.kx; qy = o.ky; qz = o.kz;
         }
-        const float Rbar = 0.5f * (uj.w + uk.w);
-        float S0 = 0.f, S1 = 0.f, sV = 0.f;
-#pragma unroll
-        for (int a = 0; a < NSHFA; ++a) {
-          const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
-          float Wv = g0.x * F1[0], V = g0.x * dF1[0];
-          Wv = fmaf(g0.y, F1[1], Wv); V = fmaf(g0.y, dF1[1], V);
-          Wv = fmaf(g0.z, F1[2], Wv); V = fmaf(g0.z, dF1[2], V);
-          Wv = fmaf(g0.w, F1[3], Wv); V = fmaf(g0.w, dF1[3], V);
-          Wv = fmaf(g1.x, F1[4], Wv); V = fmaf(g1.x, dF1[4], V);
-          Wv = fmaf(g1.y, F1[5], Wv); V = fmaf(g1.y, dF1[5], V);
-          Wv = fmaf(g1.z, F1[6], Wv); V = fmaf(g1.z, dF1[6], V);
-          Wv = fmaf(g1.w, F1[7], Wv); V = fmaf(g1.w, dF1[7], V);
-          const float x = Rbar - c.ShfA[a];
-          const float F2 = ex2f(-c.etaA_l2e * x * x);
-          const float WF = Wv * F2;
-          S0 += WF; S1 = fmaf(WF, x, S1);
-          sV = fmaf(V, F2, sV);
-        }
-        // dt/dR_ij and dt/dR_ik (through Rbar and the cut-offs), dt/du
-        const float Aj = 2.0f * fk * fmaf(-c.etaA * fj, S1, dfj * S0);
-        const float Ak = 2.0f * fj * fmaf(-c.etaA * fk, S1, dfk * S0);
-        const float Au = 2.0f * fj * fk * sV;
-        const float qj = Au / uj.w, qk = Au / uk.w;
-        const float rj = Aj - qj * u, rk = Ak - qk * u;
-        px = fmaf(rj, uj.x, fmaf(qj, uk.x, px));
-        py = fmaf(rj, uj.y, fmaf(qj, uk.y, py));
-        pz = fmaf(rj, uj.z, fmaf(qj, uk.z, pz));
-        qx = fmaf(rk, uk.x, qk * uj.x);
-        qy = fmaf(rk, uk.y, qk * uj.y);
-        qz = fmaf(rk, uk.z, qk * uj.z);
+        int src = jl - m;
+        if (src < 0) src += ns;
+        const int srcl = (grp_id * W + src) & 31;
+        const float rx = __shfl_sync(0xffffffffu, qx, srcl);
+        const float ry = __shfl_sync(0xffffffffu, qy, srcl);
+        const float rz = __shfl_sync(0xffffffffu, qz, srcl);
+        if (act && m <= nrounds && (!last_half || jl >= nrounds)) { px += rx; py += ry; pz += rz; }
       }
-      int src = jl - m;
-      if (src < 0) src += n;
-      const int srcl = (grp_id * W + src) & 31;
-      const float rx = __shfl_sync(0xffffffffu, qx, srcl);
-      const float ry = __shfl_sync(0xffffffffu, qy, srcl);
-      const float rz = __shfl_sync(0xffffffffu, qz, srcl);
-      if (act && m <= nrounds && (!last_half || jl >= nrounds)) { px += rx; py += ry; pz += rz; }
+      for (int o = W; o < 32; o <<= 1) {
+        px += __shfl_xor_sync(0xffffffffu, px, o);
+        py += __shfl_xor_sync(0xffffffffu, py, o);
+        pz += __shfl_xor_sync(0xffffffffu, pz, o);
+      }
+      if (act && grp_id == 0) { Pacc[w][base + jl][0] += px; Pacc[w][base + jl][1] += py; Pacc[w][base + jl][2] += pz; }
+      __syncwarp();
+    };
+    if (n <= 16) {
+      rr_pass(0, n);
+    } else {
+      rr_pass(0, 16);
+      rr_pass(16, n - 16);
+      // cross pairs A x B
+      const int g2 = lane >> 4, jl = lane & 15, nb = n - 16;
+      const float4 uj = e.ua[jl];
+      const float fj = e.fA[jl], dfj = e.dfA[jl];
+      const int sj = e.slotA[jl];
+      float px = 0.f, py = 0.f, pz = 0.f;
+      for (int r0 = 0; r0 < nb; r0 += 2) {
+        const int r = r0 + g2, k = 16 + r;
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        if (r < nb) {
+          const PairShares o = pair_shares(c, zm1, gi4 + pairoff[sj * MAX_S + e.slotA[k]], uj, fj, dfj, e.ua[k], e.fA[k],
+                                           e.dfA[k]);
+          px += o.jx; py += o.jy; pz += o.jz;
+          qx = o.kx; qy = o.ky; qz = o.kz;
+        }
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) {   // k's share: sum over the 16 lanes of the group
+          qx += __shfl_xor_sync(0xffffffffu, qx, o);
+          qy += __shfl_xor_sync(0xffffffffu, qy, o);
+          qz += __shfl_xor_sync(0xffffffffu, qz, o);
+        }
+        if (jl == 0 && r < nb) { Pacc[w][k][0] += qx; Pacc[w][k][1] += qy; Pacc[w][k][2] += qz; }
+      }
+      px += __shfl_xor_sync(0xffffffffu, px, 16);
+      py += __shfl_xor_sync(0xffffffffu, py, 16);
+      pz += __shfl_xor_sync(0xffffffffu, pz, 16);
+      __syncwarp();
+      if (g2 == 0) { Pacc[w][jl][0] += px; Pacc[w][jl][1] += py; Pacc[w][jl][2] += pz; }
     }
-    for (int o = W; o < 32; o <<= 1) {
-      px += __shfl_xor_sync(0xffffffffu, px, o);
-      py += __shfl_xor_sync(0xffffffffu, py, o);
-      pz += __shfl_xor_sync(0xffffffffu, pz, o);
-    }
-    if (act && grp_id == 0) { Pacc[w][jl][0] = px; Pacc[w][jl][1] = py; Pacc[w][jl][2] = pz; }
   } else {
   // more than 32 angular neighbours (beyond liquid-water densities): lanes x partner loop, every pair from both ends
   const int P = (nA <= 8) ? 4 : (nA <= 16) ? 2 : 1;   // lanes per neighbour
