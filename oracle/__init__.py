@@ -171,6 +171,34 @@ def evaluate(model, pos, Z, box, pbc=1, ml_index=None, nbr_mode=0, want_forces=T
     return out
 
 
+def link_place(pos_ext, n_atoms, link_ml, link_mm, box, d=1.0, pbc=1):
+    """Writes the link-atom rows n_atoms.. of pos_ext (fp32, (n_atoms + n_links, 3)) in place (eq. 4)."""
+    assert pos_ext.dtype == np.float32 and pos_ext.flags["C_CONTIGUOUS"]
+    lm = np.ascontiguousarray(link_ml, dtype=np.int32); lb = np.ascontiguousarray(link_mm, dtype=np.int32)
+    box = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+    f = lib().orc_link_place
+    f.argtypes = [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_int32, C.c_void_p]
+    rc = f(n_atoms, len(lm), lm.ctypes.data, lb.ctypes.data, float(d), box.ctypes.data, pbc, pos_ext.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_link_place error {rc}")
+    return pos_ext
+
+
+def link_spread(forces_ext, pos_ext, n_atoms, link_ml, link_mm, box, d=1.0, pbc=1):
+    """Redistributes the link-atom force rows of forces_ext (fp64, in place) onto the bonded atoms (chain rule of eq. 4)."""
+    assert forces_ext.dtype == np.float64 and forces_ext.flags["C_CONTIGUOUS"]
+    pos_ext = np.ascontiguousarray(pos_ext, dtype=np.float32)
+    lm = np.ascontiguousarray(link_ml, dtype=np.int32); lb = np.ascontiguousarray(link_mm, dtype=np.int32)
+    box = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+    f = lib().orc_link_spread
+    f.argtypes = [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    rc = f(n_atoms, len(lm), lm.ctypes.data, lb.ctypes.data, float(d), box.ctypes.data, pbc, pos_ext.ctypes.data,
+           forces_ext.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_link_spread error {rc}")
+    return forces_ext
+
+
 def num_threads():
     return lib().orc_num_threads()
 

@@ -480,3 +480,59 @@ void orc_set_num_threads(int n) {
   (void)n;
 #endif
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * Link atoms (section 3, eq. 4): where the ML/MM boundary cuts a covalent bond between
+ * ML atom a and MM atom b, a link atom (hydrogen by default) is placed along the bond at a fixed distance d
+ * (1 Angstrom by default) from the ML atom,
+ *     r_L = r_a + d (r_b - r_a) / |r_b - r_a|,
+ * it enters the model as an additional ML atom, and the force the model puts on it is "redistributed" onto a and b
+ * (PAPER.md line 82).  The redistribution is the chain rule of eq. 4: with l = |r_b - r_a|, u = (r_b - r_a)/l,
+ *     dr_L/dr_a = I - (d/l)(I - u u^T),   dr_L/dr_b = (d/l)(I - u u^T)      (both symmetric), so
+ *     F_a += F_L - (d/l)(F_L - u (u.F_L)),   F_b += (d/l)(F_L - u (u.F_L)).
+ * Reading (#30): the bond vector is taken under the minimum-image convention when pbc != 0, the link
+ * atoms are stored as rows n_atoms .. n_atoms + n_links - 1 of the position / force arrays, and after the spread
+ * their force rows are zero.  fp32 in / fp32 out like the hot path, arithmetic in fp64.
+ * Pins (tests/test_oracle_pins.py): |r_L - r_a| = d and collinearity; total force and total torque conserved;
+ * central finite differences of a scalar function of r_L with respect to r_a and r_b.
+ * --------------------------------------------------------------------------------------------- */
+static void link_bond(const float* pos, const float* box, int32_t pbc, int32_t a, int32_t b, double* u, double* l) {
+  double v[3], s = 0.0;
+  for (int k = 0; k < 3; ++k) {
+    v[k] = (double)pos[3 * (size_t)b + k] - (double)pos[3 * (size_t)a + k];
+    if (pbc) { const double L = (double)box[4 * k]; v[k] -= L * rint(v[k] / L); }
+    s += v[k] * v[k];
+  }
+  *l = sqrt(s);
+  for (int k = 0; k < 3; ++k) u[k] = v[k] / *l;
+}
+
+int orc_link_place(int64_t n_atoms, int64_t n_links, const int32_t* link_ml, const int32_t* link_mm, double d,
+                   const float* box, int32_t pbc, float* pos /* [n_atoms + n_links][3] */) {
+  for (int64_t q = 0; q < n_links; ++q) {
+    double u[3], l;
+    link_bond(pos, box, pbc, link_ml[q], link_mm[q], u, &l);
+    if (!(l > 0.0)) return -1;
+    for (int k = 0; k < 3; ++k)
+      pos[3 * (size_t)(n_atoms + q) + k] = (float)((double)pos[3 * (size_t)link_ml[q] + k] + d * u[k]);
+  }
+  return 0;
+}
+
+int orc_link_spread(int64_t n_atoms, int64_t n_links, const int32_t* link_ml, const int32_t* link_mm, double d,
+                    const float* box, int32_t pbc, const float* pos, double* forces /* [n_atoms + n_links][3] */) {
+  for (int64_t q = 0; q < n_links; ++q) {
+    double u[3], l, uf = 0.0;
+    link_bond(pos, box, pbc, link_ml[q], link_mm[q], u, &l);
+    if (!(l > 0.0)) return -1;
+    double* FL = forces + 3 * (size_t)(n_atoms + q);
+    for (int k = 0; k < 3; ++k) uf += u[k] * FL[k];
+    for (int k = 0; k < 3; ++k) {
+      const double perp = (d / l) * (FL[k] - u[k] * uf);
+      forces[3 * (size_t)link_ml[q] + k] += FL[k] - perp;
+      forces[3 * (size_t)link_mm[q] + k] += perp;
+    }
+    for (int k = 0; k < 3; ++k) FL[k] = 0.0;
+  }
+  return 0;
+}

@@ -437,3 +437,93 @@ def test_errors():
     # empty input
     o = oracle.evaluate(model4(), np.zeros((0, 3)), np.zeros(0, np.int32), BOX30)
     assert o["energy"] == 0.0 and o["forces"].shape == (0, 3)
+
+
+# ------------------------------------------------------------------ link atoms (eq. 4)
+def _link_case(pbc):
+    rng = np.random.default_rng(17)
+    n, L = 6, 12.0
+    pos = rng.uniform(2.0, 10.0, size=(n, 3))
+    if pbc:
+        pos[4] = pos[1] + np.array([1.1, 0.4, -0.3]) + np.array([L, 0.0, -L])   # bonded MM partner in another image
+    else:
+        pos[4] = pos[1] + np.array([1.1, 0.4, -0.3])
+    pos[5] = pos[2] + np.array([-0.7, 0.9, 0.6])
+    link_ml, link_mm = np.array([1, 2], np.int32), np.array([4, 5], np.int32)
+    box = np.diag([L, L, L]).astype(np.float32).reshape(9)
+    ext = np.zeros((n + 2, 3), np.float32)
+    ext[:n] = pos
+    return n, ext, link_ml, link_mm, box
+
+
+@pytest.mark.parametrize("pbc", [0, 1])
+@pytest.mark.parametrize("d", [1.0, 0.73])
+def test_link_atom_placement_eq4(pbc, d):
+    """r_L lies on the (minimum-image) bond at distance d from the ML atom (eq. 4, written out here independently)."""
+    n, ext, lm, lb, box = _link_case(pbc)
+    oracle.link_place(ext, n, lm, lb, box, d, pbc)
+    L = float(box[0])
+    for q in range(2):
+        ra, rb = ext[lm[q]].astype(np.float64), ext[lb[q]].astype(np.float64)
+        v = rb - ra
+        if pbc:
+            v -= L * np.round(v / L)
+        rl = ext[n + q].astype(np.float64)
+        assert abs(np.linalg.norm(rl - ra) - d) < 2e-6
+        assert np.linalg.norm(np.cross(rl - ra, v)) < 2e-6 * np.linalg.norm(v)      # collinear
+        assert np.dot(rl - ra, v) > 0                                             # on the MM side
+        np.testing.assert_allclose(rl, ra + d * v / np.linalg.norm(v), atol=2e-6)
+
+
+@pytest.mark.parametrize("pbc", [0, 1])
+def test_link_force_spread_conserves_force_and_torque(pbc):
+    """Redistribution moves F_L onto the two bonded atoms without changing the total force; the total torque is
+    conserved when taken with the link atom at r_L (minimum-image geometry)."""
+    n, ext, lm, lb, box = _link_case(pbc)
+    oracle.link_place(ext, n, lm, lb, box, 1.0, pbc)
+    rng = np.random.default_rng(3)
+    F0 = rng.normal(size=(n + 2, 3))
+    F = F0.copy()
+    oracle.link_spread(F, ext, n, lm, lb, box, 1.0, pbc)
+    assert np.all(F[n:] == 0.0)
+    np.testing.assert_allclose(F.sum(0), F0.sum(0), atol=1e-12)
+    untouched = np.setdiff1d(np.arange(n), np.concatenate([lm, lb]))
+    assert np.array_equal(F[untouched], F0[untouched])
+    L = float(box[0])
+    for q in range(2):
+        ra = ext[lm[q]].astype(np.float64)
+        v = ext[lb[q]].astype(np.float64) - ra
+        if pbc:
+            v -= L * np.round(v / L)
+        rl = ext[n + q].astype(np.float64)
+        dFa, dFb = F[lm[q]] - F0[lm[q]], F[lb[q]] - F0[lb[q]]
+        # torque about the ML atom: only the MM share and the link force have a lever arm
+        np.testing.assert_allclose(np.cross(v, dFb), np.cross(rl - ra, F0[n + q]), atol=2e-6)
+        np.testing.assert_allclose(dFa + dFb, F0[n + q], atol=1e-12)
+
+
+def test_link_force_spread_is_the_chain_rule_finite_differences():
+    """For any scalar function phi(r_L), d phi / d r_a and d phi / d r_b through eq. 4 equal the spread of grad phi."""
+    n, ext, lm, lb, box = _link_case(0)
+    w = np.array([[0.3, -1.2, 0.7], [1.1, 0.5, -0.4]])
+
+    def phi(p):
+        e = np.zeros((n + 2, 3), np.float32)
+        e[:n] = p
+        oracle.link_place(e, n, lm, lb, box, 1.0, 0)
+        rl = e[n:].astype(np.float64)
+        return float(np.sum(np.sin(rl * w) + 0.1 * rl ** 2)), e
+
+    p0 = ext[:n].astype(np.float64)
+    _, e0 = phi(p0)
+    rl = e0[n:].astype(np.float64)
+    G = np.zeros((n + 2, 3))
+    G[n:] = w * np.cos(rl * w) + 0.2 * rl          # d phi / d r_L, treated like a (negative) force on the link atoms
+    oracle.link_spread(G, e0, n, lm, lb, box, 1.0, 0)
+    h = 2e-3   # positions are fp32 inside the oracle: a larger step keeps the difference quotient clean
+    for a in (int(lm[0]), int(lb[0]), int(lm[1]), int(lb[1])):
+        for k in range(3):
+            pp, pm = p0.copy(), p0.copy()
+            pp[a, k] += h; pm[a, k] -= h
+            fd = (phi(pp)[0] - phi(pm)[0]) / (2 * h)
+            assert abs(fd - G[a, k]) < 2e-3 * (1 + abs(G[a, k])), (a, k, fd, G[a, k])
