@@ -112,6 +112,23 @@ int nnp_eval(nnp_workspace*, int64_t n_atoms, const float* d_pos, const int32_t*
 int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int32_t* h_Z, const float box[9],
                   int32_t pbc, const int32_t* h_ml_index, int64_t n_ml, double* h_energy, float* h_forces);
 
+/* Link atoms at the ML/MM boundary (eq. 4).  Where the ML region cuts a covalent bond between ML
+ * atom link_ml[q] and MM atom link_mm[q], link atom q is stored as row n_atoms + q of the position and force arrays
+ * (the arrays hold n_atoms + n_links rows; the caller lists the link rows in the ML index with the link element's
+ * atomic number, hydrogen by default).
+ *   nnp_link_place : writes r_L = r_ML + d (r_MM - r_ML)/|r_MM - r_ML| into rows n_atoms.. of d_pos (call before nnp_eval)
+ *   nnp_link_spread: adds the chain-rule shares of the link rows of d_forces onto the bonded atoms and zeroes the
+ *                    link rows (call after nnp_eval): F_ML += F_L - (d/l)(F_L - u(u.F_L)), F_MM += (d/l)(F_L - u(u.F_L))
+ * d = link distance in Angstrom (PAPER.md default 1.0); bond vectors take the minimum image when pbc != 0 (box as in
+ * nnp_eval, HOST).  d_link_ml / d_link_mm: DEVICE [n_links] int32 atom indices < n_atoms.  Asynchronous on the given
+ * cudaStream_t; out-of-range indices and zero-length bonds are skipped.  Returns NNP_ERR_INVALID_ARG / _BOX_UNSUPPORTED
+ * for bad arguments. */
+int nnp_link_place(void* cuda_stream, int64_t n_atoms, int64_t n_links, const int32_t* d_link_ml,
+                   const int32_t* d_link_mm, double d, const float box[9], int32_t pbc, float* d_pos);
+int nnp_link_spread(void* cuda_stream, int64_t n_atoms, int64_t n_links, const int32_t* d_link_ml,
+                    const int32_t* d_link_mm, double d, const float box[9], int32_t pbc, const float* d_pos,
+                    float* d_forces);
+
 /* Synchronises the stream and returns the sticky device status (NNP_OK or the first NNP_ERR_* seen),
  * then clears it. */
 int nnp_status(nnp_workspace*);

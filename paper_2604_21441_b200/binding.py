@@ -18,7 +18,7 @@ EXPORTS = [
     "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
-    "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
+    "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
 
 
@@ -76,6 +76,8 @@ def lib():
         L.nnp_debug_atomic_energies.argtypes = [vp, vp]
         L.nnp_debug_counters.argtypes = [vp, C.POINTER(i64)]
         L.nnp_debug_mlp_timeline.argtypes = [vp, vp]
+        L.nnp_link_place.argtypes = [vp, i64, i64, vp, vp, C.c_double, vp, i32, vp]
+        L.nnp_link_spread.argtypes = [vp, i64, i64, vp, vp, C.c_double, vp, i32, vp, vp]
         L.nnp_workspace_set_profiling.argtypes = [vp, i32]
         L.nnp_debug_stage_times.argtypes = [vp, vp]
         _lib = L
@@ -148,6 +150,14 @@ def nnp_debug_daev(ws, h_daev):
 
 def nnp_debug_atomic_energies(ws, h_e):
     return lib().nnp_debug_atomic_energies(ws, h_e)
+
+
+def nnp_link_place(stream, n_atoms, n_links, d_link_ml, d_link_mm, d, box, pbc, d_pos):
+    return lib().nnp_link_place(stream, n_atoms, n_links, d_link_ml, d_link_mm, float(d), box, pbc, d_pos)
+
+
+def nnp_link_spread(stream, n_atoms, n_links, d_link_ml, d_link_mm, d, box, pbc, d_pos, d_forces):
+    return lib().nnp_link_spread(stream, n_atoms, n_links, d_link_ml, d_link_mm, float(d), box, pbc, d_pos, d_forces)
 
 
 def nnp_debug_mlp_timeline(ws, h_ticks):
@@ -263,6 +273,18 @@ class Workspace:
         if check:
             _check(nnp_status(self.handle), "nnp_status")
         return energy, forces
+
+    def link_place(self, pos_ext, n_atoms, link_ml, link_mm, box, d=1.0, pbc=1):
+        """Writes the link-atom rows n_atoms.. of pos_ext ((n_atoms + n_links, 3) float32 cuda) on the workspace stream."""
+        b = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+        _check(nnp_link_place(self.stream.cuda_stream, n_atoms, link_ml.shape[0], link_ml.data_ptr(), link_mm.data_ptr(), d,
+                              b.ctypes.data, pbc, pos_ext.data_ptr()), "nnp_link_place")
+
+    def link_spread(self, forces_ext, pos_ext, n_atoms, link_ml, link_mm, box, d=1.0, pbc=1):
+        """Redistributes the link rows of forces_ext onto the bonded atoms (chain rule of PAPER.md eq. 4)."""
+        b = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+        _check(nnp_link_spread(self.stream.cuda_stream, n_atoms, link_ml.shape[0], link_ml.data_ptr(), link_mm.data_ptr(), d,
+                               b.ctypes.data, pbc, pos_ext.data_ptr(), forces_ext.data_ptr()), "nnp_link_spread")
 
     def eval_host(self, pos, Z, box, pbc=1, ml_index=None, forces_out=None):
         """numpy in / numpy out through nnp_eval_host (copies + synchronisation inside the library)."""

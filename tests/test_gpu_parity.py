@@ -333,3 +333,68 @@ def test_error_reporting():
     ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, None)
     Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
     check_EF(Eg, Fg, ref, cfg["pos"].shape[0])
+
+
+# ------------------------------------------------------------------ link atoms (eq. 4)
+@pytest.mark.parametrize("pbc", [0, 1])
+def test_link_atoms_place_eval_spread(pbc):
+    """ML/MM boundary cutting two bonds of the cfg-4 cluster: link atoms placed on the device (eq. 4), evaluated as
+    regular ML hydrogens, their forces redistributed by the chain rule -- every step against the oracle, and the
+    final forces against central finite differences of the oracle energy with respect to the REAL atoms."""
+    torch = _torch()
+    cfg = gen.get_config(4)
+    ml_full = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    box = cfg["box"]
+    L = float(box[0])
+    # ML region = the first 40 cluster atoms; the two bonds to atoms 40 and 41 of the chain are cut
+    ml = ml_full[:40]
+    bonded = []
+    for b in (int(ml_full[40]), int(ml_full[41])):
+        dv = cfg["pos"][ml].astype(np.float64) - cfg["pos"][b].astype(np.float64)
+        dv -= L * np.round(dv / L)
+        bonded.append(int(ml[np.argmin((dv ** 2).sum(1))]))
+    link_ml = np.array(bonded, np.int32)
+    link_mm = np.array([int(ml_full[40]), int(ml_full[41])], np.int32)
+    pos_ext = np.zeros((n + 2, 3), np.float32)
+    pos_ext[:n] = cfg["pos"]
+    if pbc == 0:
+        pos_ext[:n] -= L * np.floor(pos_ext[:n] / L)      # open boundaries: keep the cluster in one piece
+    Z_ext = np.concatenate([cfg["Z"], np.array([1, 1], np.int32)])
+    ml_ext = np.concatenate([ml, np.array([n, n + 1], np.int32)]).astype(np.int32)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    # oracle chain
+    p_or = pos_ext.copy()
+    oracle.link_place(p_or, n, link_ml, link_mm, box, 1.0, pbc)
+    ref = oracle.evaluate(om, p_or, Z_ext, box, pbc, ml_ext)
+    F_or = ref["forces"].copy()
+    oracle.link_spread(F_or, p_or, n, link_ml, link_mm, box, 1.0, pbc)
+    # device chain
+    m, ws = make(dict(cfg, pos=pos_ext, ml_index=ml_ext))
+    dpos = torch.from_numpy(pos_ext).cuda(); dZ = torch.from_numpy(Z_ext).cuda(); dml = torch.from_numpy(ml_ext).cuda()
+    dlm = torch.from_numpy(link_ml).cuda(); dlb = torch.from_numpy(link_mm).cuda()
+    ws.link_place(dpos, n, dlm, dlb, box, 1.0, pbc)
+    E, F = ws.eval(dpos, dZ, box, pbc, dml)
+    ws.link_spread(F, dpos, n, dlm, dlb, box, 1.0, pbc)
+    torch.cuda.synchronize()
+    assert ws.status() == 0
+    np.testing.assert_allclose(dpos.cpu().numpy()[n:], p_or[n:], atol=1e-6)           # placement
+    Fg = F.cpu().numpy().astype(np.float64)
+    assert np.all(Fg[n:] == 0.0)
+    rows = np.concatenate([ml, link_mm])
+    dF = Fg[rows] - F_or[rows]
+    assert abs(float(E.cpu()[0]) - ref["energy"]) / len(ml_ext) <= E_TOL
+    assert np.sqrt((dF ** 2).sum() / (F_or[rows] ** 2).sum()) <= F_RMS_TOL and np.abs(dF).max() <= F_MAX_TOL
+    assert np.any(Fg[link_mm] != 0.0)                                                 # MM partners receive their share
+    # finite differences of the oracle energy through the placement, with respect to a bonded ML and MM atom
+    def energy(p):
+        e = p.copy()
+        oracle.link_place(e, n, link_ml, link_mm, box, 1.0, pbc)
+        return oracle.evaluate(om, e, Z_ext, box, pbc, ml_ext, want_forces=False)["energy"]
+    h = 1e-3
+    for a in (int(link_ml[0]), int(link_mm[0])):
+        for k in range(3):
+            pp, pm = pos_ext.copy(), pos_ext.copy()
+            pp[a, k] += h; pm[a, k] -= h
+            fd = -(energy(pp) - energy(pm)) / float(pp[a, k] - pm[a, k])
+            assert abs(fd - Fg[a, k]) <= 2e-2 * (1.0 + abs(fd)), (a, k, fd, Fg[a, k])
