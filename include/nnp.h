@@ -77,6 +77,10 @@ typedef struct {
  * The tensor-core modes additionally need n_layers == 4, hidden widths multiples of 32 and |w| < 6e4
  * (fp16 range); a model outside that runs in NNP_MLP_FP32_SIMT and set_mlp_mode(F16*) returns UNSUPPORTED. */
 int nnp_model_create(const nnp_aev_params* aev, const nnp_mlp_desc* nets /* HOST [n_species] */, nnp_model** out);
+/* Ensemble of n_members (1..8) networks per element, E = mean of the members' energies -- ANI-2x "is an ensemble of 8
+ * networks".  nets: HOST [n_members][n_species], member-major; every member must have the same
+ * layer widths per species.  nnp_model_create is the n_members = 1 case.  All members share one AEV. */
+int nnp_model_create_ensemble(const nnp_aev_params* aev, const nnp_mlp_desc* nets, int32_t n_members, nnp_model** out);
 int nnp_model_destroy(nnp_model*);
 int nnp_model_aev_length(const nnp_model*);
 

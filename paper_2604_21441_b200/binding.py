@@ -15,7 +15,7 @@ NNP_OK = 0
 NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
-    "nnp_model_create", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
+    "nnp_model_create", "nnp_model_create_ensemble", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
@@ -59,6 +59,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
         L.nnp_model_create.argtypes = [vp, vp, C.POINTER(vp)]
+        L.nnp_model_create_ensemble.argtypes = [vp, vp, i32, C.POINTER(vp)]
         L.nnp_model_destroy.argtypes = [vp]
         L.nnp_model_aev_length.argtypes = [vp]
         L.nnp_workspace_create.argtypes = [vp, i64, i64, vp, C.POINTER(vp)]
@@ -92,6 +93,12 @@ def nnp_strerror(code):
 def nnp_model_create(aev_struct, nets_array):
     out = C.c_void_p()
     rc = lib().nnp_model_create(C.addressof(aev_struct), C.addressof(nets_array), C.byref(out))
+    return rc, out.value
+
+
+def nnp_model_create_ensemble(aev_struct, nets_array, n_members):
+    out = C.c_void_p()
+    rc = lib().nnp_model_create_ensemble(C.addressof(aev_struct), C.addressof(nets_array), n_members, C.byref(out))
     return rc, out.value
 
 
@@ -186,7 +193,8 @@ def _check(rc, where):
 
 class Model:
     """aev: dict with Rcr, Rca, EtaR, EtaA, Zeta, ShfR, ShfA, ShfZ, radial_prefactor, cos_scale, species_Z;
-    nets: {Z: (dims, [W_l], [b_l])}; species without an entry have no network."""
+    nets: {Z: (dims, [W_l], [b_l])}; species without an entry have no network.  A list of such dicts makes an
+    ensemble (E = mean over the members: ANI-2x is an ensemble of 8 networks)."""
 
     def __init__(self, aev, nets, celu_alpha=0.1):
         keep = []
@@ -200,10 +208,13 @@ class Model:
         p = _AevParams(aev["Rcr"], aev["Rca"], aev["EtaR"], aev["EtaA"], aev["Zeta"], len(ShfR), len(ShfA),
                        len(ShfZ), dp(ShfR), dp(ShfA), dp(ShfZ), aev["radial_prefactor"], aev["cos_scale"], S,
                        sZ.ctypes.data_as(C.POINTER(C.c_int32)))
-        arr = (_MlpDesc * S)()
-        for s, Z in enumerate(sZ):
+        members = list(nets) if isinstance(nets, (list, tuple)) else [nets]
+        M = len(members)
+        arr = (_MlpDesc * (S * M))()
+        for mem, s, Z in ((mem, s, Z) for mem in range(M) for s, Z in enumerate(sZ)):
+            nets = members[mem]
             if int(Z) not in nets:
-                arr[s] = _MlpDesc(0, None, None, None, celu_alpha)
+                arr[mem * S + s] = _MlpDesc(0, None, None, None, celu_alpha)
                 continue
             dims, W, b = nets[int(Z)]
             d = k(np.ascontiguousarray(dims, dtype=np.int32))
@@ -217,9 +228,10 @@ class Model:
                     raise ValueError("weight/bias shape mismatch")
                 Wp[l] = w.ctypes.data_as(C.POINTER(C.c_float))
                 bp[l] = bb.ctypes.data_as(C.POINTER(C.c_float))
-            arr[s] = _MlpDesc(nl, d.ctypes.data_as(C.POINTER(C.c_int32)), Wp, bp, celu_alpha)
-        rc, h = nnp_model_create(p, arr)
+            arr[mem * S + s] = _MlpDesc(nl, d.ctypes.data_as(C.POINTER(C.c_int32)), Wp, bp, celu_alpha)
+        rc, h = nnp_model_create_ensemble(p, arr, M) if M > 1 else nnp_model_create(p, arr)
         _check(rc, "nnp_model_create")
+        self.n_members = M
         self.handle = h
         self.aev_length = nnp_model_aev_length(h)
 

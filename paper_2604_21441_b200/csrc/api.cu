@@ -29,7 +29,13 @@ extern "C" const char* nnp_strerror(int code) {
 
 // ------------------------------------------------------------------------------------------------ model
 extern "C" int nnp_model_create(const nnp_aev_params* p, const nnp_mlp_desc* nets, nnp_model** out) {
-  if (!p || !nets || !out) return NNP_ERR_INVALID_ARG;
+  return nnp_model_create_ensemble(p, nets, 1, out);
+}
+
+extern "C" int nnp_model_create_ensemble(const nnp_aev_params* p, const nnp_mlp_desc* nets_all, int32_t n_members,
+                                         nnp_model** out) {
+  if (!p || !nets_all || !out || n_members < 1 || n_members > MAX_MEMBERS) return NNP_ERR_INVALID_ARG;
+  const nnp_mlp_desc* nets = nets_all;   // member 0 defines the architecture
   *out = nullptr;
   if (p->n_species < 1 || !p->species_Z || !p->ShfR || !p->ShfA || !p->ShfZ) return NNP_ERR_INVALID_ARG;
   if (!(p->Rcr > 0) || !(p->Rca > 0) || p->Rca > p->Rcr) return NNP_ERR_INVALID_ARG;
@@ -81,13 +87,23 @@ extern "C" int nnp_model_create(const nnp_aev_params* p, const nnp_mlp_desc* net
   }
   if (nl_common == 0) { delete m; return NNP_ERR_INVALID_ARG; }
   m->n_layers = nl_common;
+  m->n_members = n_members;
+  for (int mem = 1; mem < n_members; ++mem)      // every member: same architecture as member 0
+    for (int s = 0; s < S; ++s) {
+      const nnp_mlp_desc &d0 = nets[s], &d = nets_all[(size_t)mem * S + s];
+      bool same = d.n_layers == d0.n_layers && (d.n_layers == 0 || (d.dims && d.W && d.b));
+      for (int l = 0; same && l <= d.n_layers && d.n_layers > 0; ++l) same = d.dims[l] == d0.dims[l];
+      if (!same) { delete m; return NNP_ERR_UNSUPPORTED; }
+    }
+  total *= (size_t)n_members;
   std::vector<float> blob(total, 0.f);
   float* dbase = nullptr;
   if (cudaMalloc(&dbase, std::max<size_t>(total, 4) * sizeof(float)) != cudaSuccess) { cudaGetLastError(); delete m; return NNP_ERR_CUDA; }
   size_t off = 0;
+  for (int mem = 0; mem < n_members; ++mem)
   for (int s = 0; s < S; ++s) {
-    const nnp_mlp_desc& d = nets[s];
-    Net& n = m->nets.net[s];
+    const nnp_mlp_desc& d = nets_all[(size_t)mem * S + s];
+    Net& n = m->nets[mem].net[s];
     n.n_layers = d.n_layers;
     if (d.n_layers == 0) continue;
     n.alpha = (float)d.celu_alpha;
@@ -116,7 +132,7 @@ extern "C" int nnp_model_create(const nnp_aev_params* p, const nnp_mlp_desc* net
   }
   m->dev_blob = dbase; m->blob_bytes = total * sizeof(float);
   m->tc = nullptr;
-  int rc = tc_model_create(m, nets);
+  int rc = tc_model_create(m, nets_all);
   if (rc != NNP_OK) { cudaFree(dbase); delete m; return rc; }
   *out = m;
   return NNP_OK;

@@ -22,7 +22,7 @@ __device__ __forceinline__ float celu_grad_from_act(float a, float alpha) { retu
 __global__ void __launch_bounds__(256)
 k_dense(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __restrict__ tiles, int layer, int mode,
         const float* __restrict__ in, int ldin, float* __restrict__ out, int ldout, const float* __restrict__ act,
-        int ldact) {
+        int ldact, int accumulate) {
   if ((int)blockIdx.x >= grp->n_tiles) return;
   const TileInfo ti = tiles[blockIdx.x];
   const Net& net = nets.net[ti.slot];
@@ -92,7 +92,8 @@ k_dense(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __rest
       float v = acc[i][j];
       if (mode == 0) v = celu_f(v + net.b[layer][n], net.alpha);
       else if (mode == 1) v *= celu_grad_from_act(act[row * ldact + n], net.alpha);
-      if (mode == 2) out[daev_off(row, n, ldout)] = v; else out[row * ldout + n] = v;
+      if (mode == 2) { float* o = out + daev_off(row, n, ldout); *o = accumulate ? *o + v : v; }   // ensemble: sum over members
+      else out[row * ldout + n] = v;
     }
   }
 }
@@ -101,7 +102,8 @@ k_dense(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __rest
 // n_layers == 1: the input is the AEV itself and dE/dAEV = w (mapped columns).
 __global__ void __launch_bounds__(256)
 k_last(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __restrict__ tiles,
-       const float* __restrict__ in, int ldin, float* __restrict__ e_atom, float* __restrict__ dz, int lddz) {
+       const float* __restrict__ in, int ldin, float* __restrict__ e_atom, float* __restrict__ dz, int lddz,
+       float scale, int accumulate) {
   if ((int)blockIdx.x >= grp->n_tiles) return;
   const TileInfo ti = tiles[blockIdx.x];
   const Net& net = nets.net[ti.slot];
@@ -114,16 +116,17 @@ k_last(NetTable nets, const GroupInfo* __restrict__ grp, const TileInfo* __restr
   if (lddz == 0) lddz = grp->Kc;
   for (int r = wp; r < TILE_M; r += 8) {
     const size_t row = (size_t)(ti.row0 + r);
-    if (r >= ti.nvalid) { if (lane == 0) e_atom[row] = 0.f; continue; }
+    if (r >= ti.nvalid) { if (lane == 0 && !accumulate) e_atom[row] = 0.f; continue; }
     float s = 0.f;
     for (int k = lane; k < K; k += 32) {
       const int km = (nl == 1) ? grp->blkmap[k >> 5] * BLK + (k & 31) : k;
       const float a = in[row * ldin + k], wk = w[km];
       s = fmaf(a, wk, s);
-      if (nl == 1) dz[daev_off(row, k, lddz)] = wk; else dz[row * lddz + k] = wk * celu_grad_from_act(a, net.alpha);
+      if (nl == 1) { float* o = dz + daev_off(row, k, lddz); *o = accumulate ? *o + scale * wk : scale * wk; }
+      else dz[row * lddz + k] = scale * wk * celu_grad_from_act(a, net.alpha);
     }
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == 0) e_atom[row] = s + net.b[nl - 1][0];
+    if (lane == 0) { const float ev = scale * (s + net.b[nl - 1][0]); e_atom[row] = accumulate ? e_atom[row] + ev : ev; }
   }
 }
 
@@ -135,29 +138,34 @@ int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml) {
   int launches = 0;
   const dim3 blk(256);
   const int nyh = (HP + SM_BN - 1) / SM_BN, nya = (m->Kfull + SM_BN - 1) / SM_BN;
-  // forward hidden layers: a_{l+1} = CELU(W_l a_l + b_l); a_0 = aev (pitch 0 = compacted pitch)
-  for (int l = 0; l + 1 < nl; ++l) {
-    k_dense<<<dim3(ws->max_tiles, nyh), blk, 0, st>>>(m->nets, ws->groups, ws->tiles, l, 0,
-                                                      (l == 0) ? ws->aev : ws->hbuf[l - 1], (l == 0) ? 0 : HP,
-                                                      ws->hbuf[l], HP, nullptr, 0);
-    ++launches;
-  }
-  // last layer: E_i and dz of the last hidden layer (or dE/dAEV itself for a one-layer network)
-  if (nl == 1) k_last<<<ws->max_tiles, blk, 0, st>>>(m->nets, ws->groups, ws->tiles, ws->aev, 0, ws->e_atom, ws->daev, 0);
-  else k_last<<<ws->max_tiles, blk, 0, st>>>(m->nets, ws->groups, ws->tiles, ws->hbuf[nl - 2], HP, ws->e_atom, ws->dbuf[0], HP);
-  ++launches;
-  // backward: dz_{l-1} = (W_l^T dz_l) * CELU'(a_l) for l = nl-2 .. 1, then dE/dAEV = W_0^T dz_0
-  int cur = 0;
-  for (int l = nl - 2; l >= 0; --l) {
-    if (l > 0) {
-      k_dense<<<dim3(ws->max_tiles, nyh), blk, 0, st>>>(m->nets, ws->groups, ws->tiles, l, 1, ws->dbuf[cur], HP,
-                                                        ws->dbuf[cur ^ 1], HP, ws->hbuf[l - 1], HP);
-      cur ^= 1;
-    } else {
-      k_dense<<<dim3(ws->max_tiles, nya), blk, 0, st>>>(m->nets, ws->groups, ws->tiles, 0, 2, ws->dbuf[cur], HP,
-                                                        ws->daev, 0, nullptr, 0);
+  const float scale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members; the 1/M rides on dz of the last layer
+  for (int mem = 0; mem < m->n_members; ++mem) {
+    const NetTable& nets = m->nets[mem];
+    const int acc = mem > 0;
+    // forward hidden layers: a_{l+1} = CELU(W_l a_l + b_l); a_0 = aev (pitch 0 = compacted pitch)
+    for (int l = 0; l + 1 < nl; ++l) {
+      k_dense<<<dim3(ws->max_tiles, nyh), blk, 0, st>>>(nets, ws->groups, ws->tiles, l, 0,
+                                                        (l == 0) ? ws->aev : ws->hbuf[l - 1], (l == 0) ? 0 : HP,
+                                                        ws->hbuf[l], HP, nullptr, 0, 0);
+      ++launches;
     }
+    // last layer: E_i and dz of the last hidden layer (or dE/dAEV itself for a one-layer network)
+    if (nl == 1) k_last<<<ws->max_tiles, blk, 0, st>>>(nets, ws->groups, ws->tiles, ws->aev, 0, ws->e_atom, ws->daev, 0, scale, acc);
+    else k_last<<<ws->max_tiles, blk, 0, st>>>(nets, ws->groups, ws->tiles, ws->hbuf[nl - 2], HP, ws->e_atom, ws->dbuf[0], HP, scale, acc);
     ++launches;
+    // backward: dz_{l-1} = (W_l^T dz_l) * CELU'(a_l) for l = nl-2 .. 1, then dE/dAEV = W_0^T dz_0
+    int cur = 0;
+    for (int l = nl - 2; l >= 0; --l) {
+      if (l > 0) {
+        k_dense<<<dim3(ws->max_tiles, nyh), blk, 0, st>>>(nets, ws->groups, ws->tiles, l, 1, ws->dbuf[cur], HP,
+                                                          ws->dbuf[cur ^ 1], HP, ws->hbuf[l - 1], HP, 0);
+        cur ^= 1;
+      } else {
+        k_dense<<<dim3(ws->max_tiles, nya), blk, 0, st>>>(nets, ws->groups, ws->tiles, 0, 2, ws->dbuf[cur], HP,
+                                                          ws->daev, 0, nullptr, 0, acc);
+      }
+      ++launches;
+    }
   }
   return launches;
 }

@@ -42,13 +42,14 @@ struct TcNetImg { const uint8_t* w2; const uint8_t* w3; const uint8_t* w3t; cons
 struct TcTable { TcNetImg n[MAX_S]; };
 
 struct TcModel {
-  TcTable tab;
+  TcTable tab[MAX_MEMBERS];
   void* blob;
+  NetTable* d_nets;        // device copy of the members' network tables (layer-1 repacking walks all members)
 };
 
 struct TcWorkspace {
-  uint8_t* w1img[MAX_S];   // F1 image [N1][Kc] of each slot (repacked when the compacted column set changes)
-  uint8_t* w1timg[MAX_S];  // B1 image [Kc][N1]
+  uint8_t* w1img[MAX_MEMBERS][MAX_S];   // F1 image [N1][Kc] per member and slot (repacked when the column set changes)
+  uint8_t* w1timg[MAX_MEMBERS][MAX_S];  // B1 image [Kc][N1]
   unsigned long long* key; // [2]: column-set key the images were packed for / scratch
   int num_sms;
   int smem_bytes[2];
@@ -191,6 +192,7 @@ __device__ __forceinline__ float unpack_c_hi(uint32_t q) {
 // The AEV columns that are materialised depend on the species present in the evaluation (GroupInfo::blkmap), so the
 // layer-1 operand images are (re)packed on the device, only when that column set changed since the last call.
 struct TcPackArgs { uint8_t* w1[MAX_S]; uint8_t* w1t[MAX_S]; };
+struct TcPackAll { TcPackArgs m[MAX_MEMBERS]; };
 
 __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t blk_lo, int r, int kk, const float* x) {
   uint32_t hi[4], lo[4];
@@ -202,12 +204,14 @@ __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t bl
 }
 
 __global__ void __launch_bounds__(256)
-k_tc_pack_w1(NetTable nets, const GroupInfo* __restrict__ grp, TcPackArgs a, unsigned long long* __restrict__ key) {
+k_tc_pack_w1(const NetTable* __restrict__ all_nets, const GroupInfo* __restrict__ grp, TcPackAll all,
+             unsigned long long* __restrict__ key) {
   const unsigned long long want = grp->colkey;
   if (key[0] == want) return;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) key[1] = want;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) key[1] = want;
   const int slot = blockIdx.y;
-  const Net& net = nets.net[slot];
+  const TcPackArgs& a = all.m[blockIdx.z];
+  const Net& net = all_nets[blockIdx.z].net[slot];
   if (net.n_layers == 0 || grp->count[slot] == 0) return;
   const int Kc = grp->Kc, N1 = net.dims[1], Kfull = net.dims[0];
   const float* __restrict__ W1 = net.W[0];  // [N1][Kfull], internal column order
@@ -301,7 +305,7 @@ template <int NPASS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict__ grp,
          const TileInfo* __restrict__ tiles, const float* __restrict__ aev, float* __restrict__ daev,
-         float* __restrict__ e_atom, unsigned long long* __restrict__ key) {
+         float* __restrict__ e_atom, unsigned long long* __restrict__ key, float escale, int accumulate) {
   using C = TcCfg<NPASS>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
@@ -515,11 +519,11 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
             const float4 b4 = bv[i >> 2], w4 = wv[i >> 2];
             const float z0 = __uint_as_float(v[i]) + ((i & 2) ? b4.z : b4.x);
             const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
-            const float wa = (i & 2) ? w4.z : w4.x, wb = (i & 2) ? w4.w : w4.y;
+            const float wa = (i & 2) ? w4.z : w4.x, wb = (i & 2) ? w4.w : w4.y;   // escale = 1/members rides on dl3
             const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
             const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
             e = fmaf(h0, wa, e); e = fmaf(h1, wb, e);
-            split2(wa * (z0 > 0.f ? 1.f : e0), wb * (z1 > 0.f ? 1.f : e1), hi[i >> 1], lo[i >> 1]);
+            split2(escale * wa * (z0 > 0.f ? 1.f : e0), escale * wb * (z1 > 0.f ? 1.f : e1), hi[i >> 1], lo[i >> 1]);
           }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
         }
@@ -528,7 +532,8 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
         if (part == 0) {
 #pragma unroll
           for (int pp = 0; pp < TC_NPART - 1; ++pp) e += e_part[pp * 128 + row];   // fixed order
-          e_atom[ti.row0 + row] = valid ? e + __ldg(net.b[nl - 1]) : 0.f;
+          const float ev = valid ? escale * (e + __ldg(net.b[nl - 1])) : 0.f;
+          e_atom[ti.row0 + row] = accumulate ? e_atom[ti.row0 + row] + ev : ev;   // ensemble: mean over members
         }
         signal_and_wait();
       }
@@ -564,8 +569,12 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
             tmem_wait_ld();
             if (valid) {
 #pragma unroll
-              for (int i = 0; i < 16; i += 4)
-                *reinterpret_cast<uint4*>(dst + (size_t)(j * 4 + (i >> 2)) * (4 * TILE_M)) = make_uint4(v[i], v[i + 1], v[i + 2], v[i + 3]);
+              for (int i = 0; i < 16; i += 4) {
+                float4* o = reinterpret_cast<float4*>(dst + (size_t)(j * 4 + (i >> 2)) * (4 * TILE_M));
+                float4 g = make_float4(__uint_as_float(v[i]), __uint_as_float(v[i + 1]), __uint_as_float(v[i + 2]), __uint_as_float(v[i + 3]));
+                if (accumulate) { const float4 p = *o; g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w; }   // sum over members
+                *o = g;
+              }
             }
           }
           if (c0 + 2 < nc) signal_and_wait();
@@ -614,45 +623,51 @@ bool tc_shape_ok(const nnp_mlp_desc& d) {
 }
 }  // namespace
 
-int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets) {
+int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][S] */) {
   m->tc = nullptr;
-  const int S = m->aev.S;
+  const int S = m->aev.S, M = m->n_members;
   size_t total = 0;
-  size_t off[MAX_S][4];
-  for (int s = 0; s < S; ++s) {
-    const nnp_mlp_desc& d = nets[s];
-    if (d.n_layers == 0) continue;
-    if (!tc_shape_ok(d)) return NNP_OK;  // no tensor-core image: workspaces stay in NNP_MLP_FP32_SIMT
-    const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
-    const size_t sz[4] = {tc_img_bytes(N2, N1), tc_img_bytes(N3, N2), tc_img_bytes(N2, N3), tc_img_bytes(N1, N2)};
-    for (int i = 0; i < 4; ++i) { off[s][i] = total; total += (sz[i] + 1023) & ~(size_t)1023; }
-  }
+  size_t off[MAX_MEMBERS][MAX_S][4];
+  for (int mem = 0; mem < M; ++mem)
+    for (int s = 0; s < S; ++s) {
+      const nnp_mlp_desc& d = nets[(size_t)mem * S + s];
+      if (d.n_layers == 0) continue;
+      if (!tc_shape_ok(d)) return NNP_OK;  // no tensor-core image: workspaces stay in NNP_MLP_FP32_SIMT
+      const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
+      const size_t sz[4] = {tc_img_bytes(N2, N1), tc_img_bytes(N3, N2), tc_img_bytes(N2, N3), tc_img_bytes(N1, N2)};
+      for (int i = 0; i < 4; ++i) { off[mem][s][i] = total; total += (sz[i] + 1023) & ~(size_t)1023; }
+    }
   std::vector<uint8_t> blob(total, 0);
-  for (int s = 0; s < S; ++s) {
-    const nnp_mlp_desc& d = nets[s];
-    if (d.n_layers == 0) continue;
-    const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
-    const float *W2 = d.W[1], *W3 = d.W[2];  // [out][in]
-    host_image(blob, off[s][0], N2, N1, [&](int n, int k) { return W2[(size_t)n * N1 + k]; });  // F2: B = W2
-    host_image(blob, off[s][1], N3, N2, [&](int n, int k) { return W3[(size_t)n * N2 + k]; });  // F3: B = W3
-    host_image(blob, off[s][2], N2, N3, [&](int n, int k) { return W3[(size_t)k * N2 + n]; });  // B3: B = W3^T
-    host_image(blob, off[s][3], N1, N2, [&](int n, int k) { return W2[(size_t)k * N1 + n]; });  // B2: B = W2^T
-  }
+  for (int mem = 0; mem < M; ++mem)
+    for (int s = 0; s < S; ++s) {
+      const nnp_mlp_desc& d = nets[(size_t)mem * S + s];
+      if (d.n_layers == 0) continue;
+      const int N1 = d.dims[1], N2 = d.dims[2], N3 = d.dims[3];
+      const float *W2 = d.W[1], *W3 = d.W[2];  // [out][in]
+      host_image(blob, off[mem][s][0], N2, N1, [&](int n, int k) { return W2[(size_t)n * N1 + k]; });  // F2: B = W2
+      host_image(blob, off[mem][s][1], N3, N2, [&](int n, int k) { return W3[(size_t)n * N2 + k]; });  // F3: B = W3
+      host_image(blob, off[mem][s][2], N2, N3, [&](int n, int k) { return W3[(size_t)k * N2 + n]; });  // B3: B = W3^T
+      host_image(blob, off[mem][s][3], N1, N2, [&](int n, int k) { return W2[(size_t)k * N1 + n]; });  // B2: B = W2^T
+    }
   TcModel* tm = new (std::nothrow) TcModel();
   if (!tm) return NNP_ERR_CUDA;
   memset(tm, 0, sizeof(*tm));
   if (cudaMalloc(&tm->blob, std::max<size_t>(total, 1024)) != cudaSuccess ||
-      cudaMemcpy(tm->blob, blob.data(), total, cudaMemcpyHostToDevice) != cudaSuccess) {
+      cudaMemcpy(tm->blob, blob.data(), total, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMalloc(&tm->d_nets, sizeof(NetTable) * MAX_MEMBERS) != cudaSuccess ||
+      cudaMemcpy(tm->d_nets, m->nets, sizeof(NetTable) * MAX_MEMBERS, cudaMemcpyHostToDevice) != cudaSuccess) {
     cudaGetLastError();
     if (tm->blob) cudaFree(tm->blob);
+    if (tm->d_nets) cudaFree(tm->d_nets);
     delete tm;
     return NNP_ERR_CUDA;
   }
-  for (int s = 0; s < S; ++s) {
-    if (nets[s].n_layers == 0) continue;
-    const uint8_t* b = static_cast<const uint8_t*>(tm->blob);
-    tm->tab.n[s] = TcNetImg{b + off[s][0], b + off[s][1], b + off[s][2], b + off[s][3]};
-  }
+  for (int mem = 0; mem < M; ++mem)
+    for (int s = 0; s < S; ++s) {
+      if (nets[(size_t)mem * S + s].n_layers == 0) continue;
+      const uint8_t* b = static_cast<const uint8_t*>(tm->blob);
+      tm->tab[mem].n[s] = TcNetImg{b + off[mem][s][0], b + off[mem][s][1], b + off[mem][s][2], b + off[mem][s][3]};
+    }
   m->tc = tm;
   return NNP_OK;
 }
@@ -661,6 +676,7 @@ void tc_model_destroy(nnp_model* m) {
   TcModel* tm = static_cast<TcModel*>(m->tc);
   if (!tm) return;
   if (tm->blob) cudaFree(tm->blob);
+  if (tm->d_nets) cudaFree(tm->d_nets);
   delete tm;
   m->tc = nullptr;
 }
@@ -682,14 +698,15 @@ int tc_workspace_create(nnp_workspace* ws) {
   if (cudaFuncSetAttribute(k_mlp_tc<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, tw->smem_bytes[0]) != cudaSuccess ||
       cudaFuncSetAttribute(k_mlp_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tw->smem_bytes[1]) != cudaSuccess)
     return NNP_ERR_CUDA;
-  for (int s = 0; s < m->aev.S; ++s) {
-    const Net& n = m->nets.net[s];
-    if (n.n_layers == 0) continue;
-    const size_t b1 = tc_img_bytes(n.dims[1], m->Kfull), b2 = tc_img_bytes(m->Kfull, n.dims[1]);
-    if (cudaMalloc(&tw->w1img[s], b1) != cudaSuccess || cudaMalloc(&tw->w1timg[s], b2) != cudaSuccess) return NNP_ERR_CUDA;
-    cudaMemset(tw->w1img[s], 0, b1);
-    cudaMemset(tw->w1timg[s], 0, b2);
-  }
+  for (int mem = 0; mem < m->n_members; ++mem)
+    for (int s = 0; s < m->aev.S; ++s) {
+      const Net& n = m->nets[mem].net[s];
+      if (n.n_layers == 0) continue;
+      const size_t b1 = tc_img_bytes(n.dims[1], m->Kfull), b2 = tc_img_bytes(m->Kfull, n.dims[1]);
+      if (cudaMalloc(&tw->w1img[mem][s], b1) != cudaSuccess || cudaMalloc(&tw->w1timg[mem][s], b2) != cudaSuccess) return NNP_ERR_CUDA;
+      cudaMemset(tw->w1img[mem][s], 0, b1);
+      cudaMemset(tw->w1timg[mem][s], 0, b2);
+    }
   if (cudaMalloc(&tw->key, 2 * sizeof(unsigned long long)) != cudaSuccess) return NNP_ERR_CUDA;
   cudaMemset(tw->key, 0, 2 * sizeof(unsigned long long));
   return NNP_OK;
@@ -698,10 +715,11 @@ int tc_workspace_create(nnp_workspace* ws) {
 void tc_workspace_destroy(nnp_workspace* ws) {
   TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
   if (!tw) return;
-  for (int s = 0; s < MAX_S; ++s) {
-    if (tw->w1img[s]) cudaFree(tw->w1img[s]);
-    if (tw->w1timg[s]) cudaFree(tw->w1timg[s]);
-  }
+  for (int mem = 0; mem < MAX_MEMBERS; ++mem)
+    for (int s = 0; s < MAX_S; ++s) {
+      if (tw->w1img[mem][s]) cudaFree(tw->w1img[mem][s]);
+      if (tw->w1timg[mem][s]) cudaFree(tw->w1timg[mem][s]);
+    }
   if (tw->key) cudaFree(tw->key);
   cudaGetLastError();
   delete tw;
@@ -718,17 +736,23 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   TcModel* tm = static_cast<TcModel*>(m->tc);
   TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
   if (!tm || !tw) return launch_mlp_simt(ws, n_ml);
-  TcPackArgs pa;
-  for (int s = 0; s < MAX_S; ++s) { pa.w1[s] = tw->w1img[s]; pa.w1t[s] = tw->w1timg[s]; }
-  k_tc_pack_w1<<<dim3(32, m->aev.S), 256, 0, ws->stream>>>(m->nets, ws->groups, pa, tw->key);
+  TcPackAll pall;
+  for (int mem = 0; mem < MAX_MEMBERS; ++mem)
+    for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
+  k_tc_pack_w1<<<dim3(32, m->aev.S, m->n_members), 256, 0, ws->stream>>>(tm->d_nets, ws->groups, pall, tw->key);
   const int grid = std::min(ws->max_tiles, tw->num_sms);
-  if (ws->mlp_mode == NNP_MLP_F16X1)
-    k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(m->nets, tm->tab, pa, ws->groups, ws->tiles, ws->aev,
-                                                                     ws->daev, ws->e_atom, tw->key);
-  else
-    k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(m->nets, tm->tab, pa, ws->groups, ws->tiles, ws->aev,
-                                                                     ws->daev, ws->e_atom, tw->key);
-  return 2;
+  const float escale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members
+  for (int mem = 0; mem < m->n_members; ++mem) {
+    if (ws->mlp_mode == NNP_MLP_F16X1)
+      k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(m->nets[mem], tm->tab[mem], pall.m[mem], ws->groups,
+                                                                       ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key,
+                                                                       escale, mem > 0);
+    else
+      k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(m->nets[mem], tm->tab[mem], pall.m[mem], ws->groups,
+                                                                       ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key,
+                                                                       escale, mem > 0);
+  }
+  return 1 + m->n_members;
 }
 
 }  // namespace nnp

@@ -8,6 +8,7 @@ namespace nnp {
 
 constexpr int MAX_S = 8;          // species slots
 constexpr int MAX_LAYERS = 4;
+constexpr int MAX_MEMBERS = 8;    // networks per element in an ensemble (ANI-2x: 8)
 constexpr int TILE_M = 128;       // MLP row tile (tcgen05 M)
 constexpr int HP = 256;           // pitch of the hidden-activation / delta scratch rows (max hidden width)
 constexpr int NSHFR = 16;         // radial shifts (fixed by the kernels)
@@ -99,7 +100,8 @@ struct NetTable { Net net[MAX_S]; };
 
 struct nnp_model {
   nnp::AevConst aev;
-  nnp::NetTable nets;        // device pointers
+  nnp::NetTable nets[nnp::MAX_MEMBERS];  // device pointers, one table per ensemble member
+  int n_members;             // E = mean over the members' energies (1 = a single network per element)
   int n_layers;              // common to all networks
   int Kfull;                 // 32 * nblk_full
   void* dev_blob;            // single allocation holding all fp32 weights
@@ -163,7 +165,7 @@ int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
                        float* d_forces);
-int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets);
+int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][n_species] */);
 void tc_model_destroy(nnp_model* m);
 int tc_workspace_create(nnp_workspace* ws);
 void tc_workspace_destroy(nnp_workspace* ws);

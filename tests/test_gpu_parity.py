@@ -398,3 +398,33 @@ def test_link_atoms_place_eval_spread(pbc):
             pp[a, k] += h; pm[a, k] -= h
             fd = -(energy(pp) - energy(pm)) / float(pp[a, k] - pm[a, k])
             assert abs(fd - Fg[a, k]) <= 2e-2 * (1.0 + abs(fd)), (a, k, fd, Fg[a, k])
+
+
+# ------------------------------------------------------------------ ensemble (ANI-2x = 8 networks)
+@pytest.mark.parametrize("k,members", [(1, 3), (4, 8)])
+def test_ensemble_mean_of_members(k, members):
+    """E = mean over the members' energies (one AEV, `members` weight sets per element): against the mean of the
+    oracle's single-network evaluations, in every MLP arithmetic mode."""
+    import paper_2604_21441_b200 as nnp
+    cfg = gen.get_config(k)
+    ml = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    n_ml = n if ml is None else len(ml)
+    nets = []
+    for mem in range(members):
+        nets.append({Z: (d,) + gen.make_weights(40 + mem, Z, d, 0.1 if mem % 2 else 0.0) for Z, (d, _, _) in cfg["nets"].items()})
+    E_or, F_or = 0.0, 0.0
+    for mem in range(members):
+        om = oracle.Model(cfg["aev"], nets[mem], cfg["celu_alpha"])
+        r = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nbr_mode=1 if n_ml > 2000 else 0)
+        E_or += r["energy"] / members
+        F_or = F_or + r["forces"] / members
+    ref = dict(energy=E_or, forces=F_or)
+    m = nnp.Model(cfg["aev"], nets, cfg["celu_alpha"])
+    ws = nnp.Workspace(m, n, n_ml)
+    for mode in (nnp.NNP_MLP_FP32_SIMT, nnp.NNP_MLP_F16X3, nnp.NNP_MLP_F16X1):
+        ws.set_mlp_mode(mode)
+        Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+        check_EF(Eg, Fg, ref, n_ml, rows=ml)
+    E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert E2 == Eg and np.array_equal(F2, Fg)      # accumulation over members is reproducible
