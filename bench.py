@@ -151,7 +151,11 @@ def run_ours(args, rank, world, local_rank):
     n = cfg["pos"].shape[0]
     # replicas: rank r perturbs with its own seed, so every GPU runs an independent box of the same shape
     P = gen.perturbed_positions(cfg["pos64"], replica_seed(cfg["perturb_seed"], rank), N_POS_SETS)
-    model = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    nets = cfg["nets"]
+    if args.ensemble > 1:   # member m: the same shapes, weights drawn with seed 1 + m (cfg 2's recipe, reading #16)
+        nets = [{Z: (d,) + gen.make_weights(1 + mem, Z, d) for Z, (d, _, _) in cfg["nets"].items()}
+                for mem in range(args.ensemble)]
+    model = nnp.Model(cfg["aev"], nets, cfg["celu_alpha"])
     ws = nnp.Workspace(model, n)
     if args.mlp_mode != "default":
         ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "f16x3": nnp.NNP_MLP_F16X3, "f16x1": nnp.NNP_MLP_F16X1}[args.mlp_mode])
@@ -232,7 +236,7 @@ def run_ours(args, rank, world, local_rank):
     nH, nO = int((cfg["Z"] == 1).sum()), int((cfg["Z"] == 8).sum())
     # compacted AEV width for an H/O-only system: 2 radial + 3 angular 32-column blocks (dense-K: all 32 blocks)
     Kc = 1024 if args.dense_k else 160
-    mlp_flops = nH * mlp_flops_per_atom(cfg["nets"][1][0], Kc) + nO * mlp_flops_per_atom(cfg["nets"][8][0], Kc)
+    mlp_flops = args.ensemble * (nH * mlp_flops_per_atom(cfg["nets"][1][0], Kc) + nO * mlp_flops_per_atom(cfg["nets"][8][0], Kc))
     work = {
         "neighbour": ("hbm", n * (16 + 32 + 8) + 4 * pairs_R + pairs_R // 4, pk["hbm"], "GB/s", 1e9),
         "aev_forward": ("alu", pairs_R * FLOP_FWD_PAIR + triplets * FLOP_FWD_TRIPLET, FP32_PEAK_TFLOPS, "TFLOP/s", 1e12),
@@ -249,13 +253,13 @@ def run_ours(args, rank, world, local_rank):
     dom = names[int(np.argmax(stage_ms))]
     roof = dict(stages[dom])
     roof.pop("ms")
-    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k
+    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1
     roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
                 traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
                 traffic_source="profiles/r01c_launches.md (ncu --set full, per launch)")
 
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and args.ensemble == 1:
         import oracle
         om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
         t0 = time.perf_counter()
@@ -271,7 +275,7 @@ def run_ours(args, rank, world, local_rank):
         "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "atoms_per_gpu": n, "position_sets": N_POS_SETS,
-                   "l2": "flushed between timed steps (256 MiB write)", "mlp_mode": args.mlp_mode, "dense_k": bool(args.dense_k),
+                   "l2": "flushed between timed steps (256 MiB write)", "mlp_mode": args.mlp_mode, "dense_k": bool(args.dense_k), "ensemble": args.ensemble,
                    "radial_pairs": pairs_R, "triplets": triplets, "parallelism": f"replicas x{world}"},
         "ns_per_day_2fs": 0.1728 * args.steps / total_s,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 12 * n + 8,
@@ -290,6 +294,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
+    ap.add_argument("--ensemble", type=int, default=1, help="networks per element (ANI-2x: 8); E = mean over members")
     ap.add_argument("--dense-k", action="store_true", help="materialise all 1008 AEV columns (K = 1024 first layer)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")

@@ -41,16 +41,22 @@ __host__ __device__ inline int tc_elem_off(int r, int kk) {  // byte offset of e
 struct TcNetImg { const uint8_t* w2; const uint8_t* w3; const uint8_t* w3t; const uint8_t* w2t; };
 struct TcTable { TcNetImg n[MAX_S]; };
 
+struct TcPackArgs { uint8_t* w1[MAX_S]; uint8_t* w1t[MAX_S]; };
+struct TcPackAll { TcPackArgs m[MAX_MEMBERS]; };
+
 struct TcModel {
   TcTable tab[MAX_MEMBERS];
   void* blob;
-  NetTable* d_nets;        // device copy of the members' network tables (layer-1 repacking walks all members)
+  NetTable* d_nets;        // device copy of the members' network tables
+  TcTable* d_tabs;         // device copy of tab[]
 };
 
 struct TcWorkspace {
   uint8_t* w1img[MAX_MEMBERS][MAX_S];   // F1 image [N1][Kc] per member and slot (repacked when the column set changes)
   uint8_t* w1timg[MAX_MEMBERS][MAX_S];  // B1 image [Kc][N1]
   unsigned long long* key; // [2]: column-set key the images were packed for / scratch
+  TcPackAll* d_pall;       // device copy of the layer-1 image pointer table
+  int* done;               // [max_tiles] ensemble hand-over: members of a tile already accumulated (reset every call)
   int num_sms;
   int smem_bytes[2];
 };
@@ -191,8 +197,6 @@ __device__ __forceinline__ float unpack_c_hi(uint32_t q) {
 // ------------------------------------------------------------------------------------------------ layer-1 images
 // The AEV columns that are materialised depend on the species present in the evaluation (GroupInfo::blkmap), so the
 // layer-1 operand images are (re)packed on the device, only when that column set changed since the last call.
-struct TcPackArgs { uint8_t* w1[MAX_S]; uint8_t* w1t[MAX_S]; };
-struct TcPackAll { TcPackArgs m[MAX_MEMBERS]; };
 
 __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t blk_lo, int r, int kk, const float* x) {
   uint32_t hi[4], lo[4];
@@ -205,7 +209,12 @@ __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t bl
 
 __global__ void __launch_bounds__(256)
 k_tc_pack_w1(const NetTable* __restrict__ all_nets, const GroupInfo* __restrict__ grp, TcPackAll all,
-             unsigned long long* __restrict__ key) {
+             unsigned long long* __restrict__ key, int* __restrict__ done, int max_tiles) {
+  {  // every call: clear the ensemble hand-over flags of the MLP kernel that follows
+    const int nthr = gridDim.x * gridDim.y * gridDim.z * blockDim.x;
+    const int gid = ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+    for (int i = gid; i < max_tiles; i += nthr) done[i] = 0;
+  }
   const unsigned long long want = grp->colkey;
   if (key[0] == want) return;
   if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) key[1] = want;
@@ -303,9 +312,11 @@ __device__ long long g_tc_timeline[64];
 
 template <int NPASS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict__ grp,
+k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_tabs,
+         const TcPackAll* __restrict__ w1all, const GroupInfo* __restrict__ grp,
          const TileInfo* __restrict__ tiles, const float* __restrict__ aev, float* __restrict__ daev,
-         float* __restrict__ e_atom, unsigned long long* __restrict__ key, float escale, int accumulate) {
+         float* __restrict__ e_atom, unsigned long long* __restrict__ key, int* __restrict__ done, int n_members,
+         float escale) {
   using C = TcCfg<NPASS>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
@@ -332,20 +343,27 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
   tc_fence_after();
   const uint32_t tmem = *tptr;
 
-  auto tile_net = [&](int t, TileInfo& ti, TileNet& tn) {
+  // Work items are (member, tile) pairs in member-major order, dealt round-robin to the resident CTAs: with an
+  // ensemble the 8 x 188 items fill the SMs evenly instead of 8 launches of 1.27 waves each.  Members of one tile
+  // accumulate into e_atom / dE/dAEV in member order: a CTA waits (done[tile] == member) before its first
+  // read-modify-write; the awaited item has a smaller index, so it is already running on a resident CTA.
+  const int n_items = n_tiles * n_members;
+  auto tile_net = [&](int w, int& t, int& mem, TileInfo& ti, TileNet& tn) {
+    mem = w / n_tiles; t = w - mem * n_tiles;   // n_items > 0 implies n_tiles > 0
     ti = tiles[t];
-    const Net& net = nets.net[ti.slot];
+    const Net& net = all_nets[mem].net[ti.slot];
     tn.N1 = net.dims[1]; tn.N2 = net.dims[2]; tn.N3 = net.dims[3]; tn.Kc = Kc;
-    tn.f1 = w1.w1[ti.slot]; tn.b1 = w1.w1t[ti.slot];
-    tn.w2 = tab.n[ti.slot].w2; tn.w3 = tab.n[ti.slot].w3; tn.w3t = tab.n[ti.slot].w3t; tn.w2t = tab.n[ti.slot].w2t;
+    tn.f1 = w1all->m[mem].w1[ti.slot]; tn.b1 = w1all->m[mem].w1t[ti.slot];
+    const TcNetImg& im = all_tabs[mem].n[ti.slot];
+    tn.w2 = im.w2; tn.w3 = im.w3; tn.w3t = im.w3t; tn.w2t = im.w2t;
   };
 
   if (warp == TC_EPI_WARPS) {
     // ===== weight producer: streams every B block of every round, in order, through the stage ring =====
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        TileInfo ti; TileNet tn; tile_net(t, ti, tn);
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+        int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
         TcRound rd[TC_MAX_ROUNDS];
         const int nrd = tc_build_rounds(tn, rd);
 #pragma unroll 1
@@ -379,8 +397,8 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
     // handful of instructions per MMA, or the single issuing warp, not the tensor core, paces the GEMM. =====
     {
       int s = 0; uint32_t ph = 0, aph = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        TileInfo ti; TileNet tn; tile_net(t, ti, tn);
+      for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+        int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
         TcRound rd[TC_MAX_ROUNDS];
         const int nrd = tc_build_rounds(tn, rd);
 #pragma unroll 1
@@ -435,9 +453,10 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
       tc_fence_after();
       if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
     };
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      TileInfo ti; TileNet tn; tile_net(t, ti, tn);
-      const Net& net = nets.net[ti.slot];
+    for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
+      int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
+      const Net& net = all_nets[mem].net[ti.slot];
+      const bool accumulate = mem > 0;
       const float alpha = net.alpha, kexp = 1.4426950408889634f / alpha;
       const bool valid = row < ti.nvalid;
       // ---- F1 rounds: AEV columns [64 p0, 64 p1) -> fp16 hi/lo panels
@@ -528,6 +547,13 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
         }
         if (part > 0) e_part[(part - 1) * 128 + row] = e;
+        if (accumulate && threadIdx.x == 0) {   // the previous member of this tile must have finished its updates
+          int seen;
+          do {
+            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(done + t) : "memory");
+            if (seen < mem) __nanosleep(100);
+          } while (seen < mem);
+        }
         asm volatile("bar.sync 1, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
         if (part == 0) {
 #pragma unroll
@@ -580,6 +606,11 @@ k_mlp_tc(NetTable nets, TcTable tab, TcPackArgs w1, const GroupInfo* __restrict_
           if (c0 + 2 < nc) signal_and_wait();
         }
         // the first round of the next tile re-arms through its own signal_and_wait (program order: loads above done)
+        if (n_members > 1) {   // publish this member's updates of the tile to the CTA that holds the next member
+          __threadfence();
+          asm volatile("bar.sync 2, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
+          if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(done + t), "r"(mem + 1) : "memory");
+        }
       }
     }
   }
@@ -655,10 +686,12 @@ int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][S] */)
   if (cudaMalloc(&tm->blob, std::max<size_t>(total, 1024)) != cudaSuccess ||
       cudaMemcpy(tm->blob, blob.data(), total, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMalloc(&tm->d_nets, sizeof(NetTable) * MAX_MEMBERS) != cudaSuccess ||
-      cudaMemcpy(tm->d_nets, m->nets, sizeof(NetTable) * MAX_MEMBERS, cudaMemcpyHostToDevice) != cudaSuccess) {
+      cudaMemcpy(tm->d_nets, m->nets, sizeof(NetTable) * MAX_MEMBERS, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMalloc(&tm->d_tabs, sizeof(TcTable) * MAX_MEMBERS) != cudaSuccess) {
     cudaGetLastError();
     if (tm->blob) cudaFree(tm->blob);
     if (tm->d_nets) cudaFree(tm->d_nets);
+    if (tm->d_tabs) cudaFree(tm->d_tabs);
     delete tm;
     return NNP_ERR_CUDA;
   }
@@ -668,6 +701,12 @@ int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][S] */)
       const uint8_t* b = static_cast<const uint8_t*>(tm->blob);
       tm->tab[mem].n[s] = TcNetImg{b + off[mem][s][0], b + off[mem][s][1], b + off[mem][s][2], b + off[mem][s][3]};
     }
+  if (cudaMemcpy(tm->d_tabs, tm->tab, sizeof(TcTable) * MAX_MEMBERS, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(tm->blob); cudaFree(tm->d_nets); cudaFree(tm->d_tabs);
+    delete tm;
+    return NNP_ERR_CUDA;
+  }
   m->tc = tm;
   return NNP_OK;
 }
@@ -677,6 +716,7 @@ void tc_model_destroy(nnp_model* m) {
   if (!tm) return;
   if (tm->blob) cudaFree(tm->blob);
   if (tm->d_nets) cudaFree(tm->d_nets);
+  if (tm->d_tabs) cudaFree(tm->d_tabs);
   delete tm;
   m->tc = nullptr;
 }
@@ -709,6 +749,15 @@ int tc_workspace_create(nnp_workspace* ws) {
     }
   if (cudaMalloc(&tw->key, 2 * sizeof(unsigned long long)) != cudaSuccess) return NNP_ERR_CUDA;
   cudaMemset(tw->key, 0, 2 * sizeof(unsigned long long));
+  TcPackAll pall;
+  memset(&pall, 0, sizeof(pall));
+  for (int mem = 0; mem < MAX_MEMBERS; ++mem)
+    for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
+  if (cudaMalloc(&tw->d_pall, sizeof(TcPackAll)) != cudaSuccess ||
+      cudaMemcpy(tw->d_pall, &pall, sizeof(TcPackAll), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMalloc(&tw->done, sizeof(int) * (size_t)std::max(ws->max_tiles, 1)) != cudaSuccess)
+    return NNP_ERR_CUDA;
+  cudaMemset(tw->done, 0, sizeof(int) * (size_t)std::max(ws->max_tiles, 1));
   return NNP_OK;
 }
 
@@ -721,6 +770,8 @@ void tc_workspace_destroy(nnp_workspace* ws) {
       if (tw->w1timg[mem][s]) cudaFree(tw->w1timg[mem][s]);
     }
   if (tw->key) cudaFree(tw->key);
+  if (tw->d_pall) cudaFree(tw->d_pall);
+  if (tw->done) cudaFree(tw->done);
   cudaGetLastError();
   delete tw;
   ws->tc_ws = nullptr;
@@ -739,20 +790,20 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   TcPackAll pall;
   for (int mem = 0; mem < MAX_MEMBERS; ++mem)
     for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
-  k_tc_pack_w1<<<dim3(32, m->aev.S, m->n_members), 256, 0, ws->stream>>>(tm->d_nets, ws->groups, pall, tw->key);
-  const int grid = std::min(ws->max_tiles, tw->num_sms);
+  k_tc_pack_w1<<<dim3(32, m->aev.S, m->n_members), 256, 0, ws->stream>>>(tm->d_nets, ws->groups, pall, tw->key, tw->done,
+                                                                         ws->max_tiles);
+  // one persistent CTA per SM over the (member, tile) work items (all CTAs are co-resident: 1 CTA/SM by shared memory)
+  const int grid = (int)std::min<int64_t>((int64_t)ws->max_tiles * m->n_members, tw->num_sms);
   const float escale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members
-  for (int mem = 0; mem < m->n_members; ++mem) {
-    if (ws->mlp_mode == NNP_MLP_F16X1)
-      k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(m->nets[mem], tm->tab[mem], pall.m[mem], ws->groups,
-                                                                       ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key,
-                                                                       escale, mem > 0);
-    else
-      k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(m->nets[mem], tm->tab[mem], pall.m[mem], ws->groups,
-                                                                       ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key,
-                                                                       escale, mem > 0);
-  }
-  return 1 + m->n_members;
+  if (ws->mlp_mode == NNP_MLP_F16X1)
+    k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(tm->d_nets, tm->d_tabs, tw->d_pall, ws->groups, ws->tiles,
+                                                                     ws->aev, ws->daev, ws->e_atom, tw->key, tw->done,
+                                                                     m->n_members, escale);
+  else
+    k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(tm->d_nets, tm->d_tabs, tw->d_pall, ws->groups, ws->tiles,
+                                                                     ws->aev, ws->daev, ws->e_atom, tw->key, tw->done,
+                                                                     m->n_members, escale);
+  return 2;
 }
 
 }  // namespace nnp
