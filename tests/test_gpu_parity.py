@@ -428,3 +428,34 @@ def test_ensemble_mean_of_members(k, members):
         check_EF(Eg, Fg, ref, n_ml, rows=ml)
     E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
     assert E2 == Eg and np.array_equal(F2, Fg)      # accumulation over members is reproducible
+
+
+def test_cuda_graph_capture_and_replay():
+    """nnp_eval allocates nothing and never synchronises: one evaluation (cooperative prep kernel included) can be
+    captured into a CUDA graph and replayed with bitwise identical results (PAPER.md line 164 names CUDA graphs as the
+    remedy for the launch-overhead plateau of small systems)."""
+    torch = _torch()
+    cfg = gen.get_config(0)
+    n = cfg["pos"].shape[0]
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        import paper_2604_21441_b200 as nnp
+        m = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+        ws = nnp.Workspace(m, n)
+        dpos = torch.from_numpy(cfg["pos"]).cuda()
+        dZ = torch.from_numpy(cfg["Z"]).cuda()
+        E = torch.zeros(1, dtype=torch.float64, device="cuda")
+        F = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
+        for _ in range(2):
+            ws.eval(dpos, dZ, cfg["box"], 1, None, E, F)
+        torch.cuda.synchronize()
+        E0, F0 = E.clone(), F.clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ws.eval(dpos, dZ, cfg["box"], 1, None, E, F)
+        for _ in range(3):
+            E.zero_(); F.zero_()
+            g.replay()
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        assert torch.equal(E, E0) and torch.equal(F, F0)
