@@ -171,6 +171,28 @@ def evaluate(model, pos, Z, box, pbc=1, ml_index=None, nbr_mode=0, want_forces=T
     return out
 
 
+def evaluate_virial(model, pos, Z, box, pbc=1, ml_index=None, nbr_mode=0):
+    """Energy, forces and the strain derivative W[a][b] = dE/d eps_ab = sum_i sum_j p_ij[a] d_ij[b] (3x3, fp64)."""
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    Z = np.ascontiguousarray(Z, dtype=np.int32)
+    box = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+    n = pos.shape[0]
+    ml = None if ml_index is None else np.ascontiguousarray(ml_index, dtype=np.int32)
+    n_ml = n if ml is None else len(ml)
+    E = C.c_double(0.0)
+    F = np.zeros((n, 3), dtype=np.float64)
+    W = np.zeros((3, 3), dtype=np.float64)
+    f = lib().orc_eval_virial
+    f.restype = C.c_int
+    f.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p,
+                  C.c_int64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    rc = f(C.addressof(model.p), C.addressof(model.nets), n, pos.ctypes.data, Z.ctypes.data, box.ctypes.data, pbc,
+           None if ml is None else ml.ctypes.data, n_ml, nbr_mode, C.addressof(E), F.ctypes.data, W.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"orc_eval_virial error {rc}")
+    return dict(energy=E.value, forces=F, virial=W)
+
+
 def link_place(pos_ext, n_atoms, link_ml, link_mm, box, d=1.0, pbc=1):
     """Writes the link-atom rows n_atoms.. of pos_ext (fp32, (n_atoms + n_links, 3)) in place (eq. 4)."""
     assert pos_ext.dtype == np.float32 and pos_ext.flags["C_CONTIGUOUS"]

@@ -374,10 +374,16 @@ double orc_mlp_forward(const orc_mlp* net, const double* G, double* g) { return 
  * Optional outputs (NULL to skip): aev_out [n_ml][L], e_atom [n_ml], daev_out [n_ml][L].
  * want_forces = 0 skips the backward pass (used by the finite-difference driver).
  * ------------------------------------------------------------------------------------------- */
-int orc_eval(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_atoms, const float* pos,
+/* virial9 (may be NULL): the strain derivative of the energy, W[a][b] = dE/d eps_ab for the homogeneous deformation
+ * r -> (1 + eps) r of positions and box, written out from its pair form:
+ *     W[a][b] = sum_i sum_{j in N(i)} p_ij[a] * d_ij[b],   p_ij = dE_i/dr_j,  d_ij = r_j - r_i (minimum image),
+ * because E_i depends on the positions only through the displacements d_ij, each of which deforms as d -> (1 + eps) d.
+ * Pins (tests/test_oracle_pins.py): central finite differences of the energy under axis scaling (periodic) and shear
+ * (open boundaries); symmetry; W = -sum_a F_a (x) r_a for an isolated cluster. */
+static int eval_impl(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_atoms, const float* pos,
              const int32_t* Z, const float* box, int32_t pbc, const int32_t* ml_index, int64_t n_ml,
              int32_t nbr_mode, int32_t want_forces, double* energy, double* forces,
-             double* aev_out, double* e_atom, double* daev_out) {
+             double* aev_out, double* e_atom, double* daev_out, double* virial9) {
   double L3[3];
   int rc = check_box(box, L3);
   if (rc) return rc;
@@ -409,6 +415,7 @@ int orc_eval(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_a
 #endif
   double* Fth = NULL;
   if (want_forces) Fth = (double*)calloc((size_t)nthreads * 3 * (size_t)(n_atoms > 0 ? n_atoms : 1), sizeof(double));
+  double* Wth = (double*)calloc((size_t)nthreads * 9, sizeof(double));
   double* Ei = (double*)calloc((size_t)(n_ml > 0 ? n_ml : 1), sizeof(double));
 
 #pragma omp parallel
@@ -445,6 +452,8 @@ int orc_eval(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_a
         for (int q = 0; q < n; ++q) {
           int64_t j = nl.col[nl.start[a] + q];
           for (int c = 0; c < 3; ++c) { F[3 * j + c] -= P[3 * q + c]; F[3 * i + c] += P[3 * q + c]; }
+          for (int c = 0; c < 3; ++c)
+            for (int b = 0; b < 3; ++b) Wth[(size_t)tid * 9 + 3 * c + b] += P[3 * q + c] * d[3 * q + b];
         }
       }
     }
@@ -462,8 +471,30 @@ int orc_eval(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_a
     }
     free(Fth);
   }
+  if (virial9)
+    for (int q = 0; q < 9; ++q) {
+      double w = 0.0;
+      for (int t = 0; t < nthreads; ++t) w += Wth[(size_t)t * 9 + q];
+      virial9[q] = w;
+    }
+  free(Wth);
   free(Ei); nbr_free(&nl); free(act); free(slot_of);
   return ORC_OK;
+}
+
+int orc_eval(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_atoms, const float* pos,
+             const int32_t* Z, const float* box, int32_t pbc, const int32_t* ml_index, int64_t n_ml,
+             int32_t nbr_mode, int32_t want_forces, double* energy, double* forces,
+             double* aev_out, double* e_atom, double* daev_out) {
+  return eval_impl(p, nets, n_atoms, pos, Z, box, pbc, ml_index, n_ml, nbr_mode, want_forces, energy, forces, aev_out,
+                   e_atom, daev_out, NULL);
+}
+
+int orc_eval_virial(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int64_t n_atoms, const float* pos,
+                    const int32_t* Z, const float* box, int32_t pbc, const int32_t* ml_index, int64_t n_ml,
+                    int32_t nbr_mode, double* energy, double* forces, double* virial9) {
+  return eval_impl(p, nets, n_atoms, pos, Z, box, pbc, ml_index, n_ml, nbr_mode, 1, energy, forces, NULL, NULL, NULL,
+                   virial9);
 }
 
 int orc_num_threads(void) {

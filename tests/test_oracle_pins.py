@@ -527,3 +527,45 @@ def test_link_force_spread_is_the_chain_rule_finite_differences():
             pp[a, k] += h; pm[a, k] -= h
             fd = (phi(pp)[0] - phi(pm)[0]) / (2 * h)
             assert abs(fd - G[a, k]) < 2e-3 * (1 + abs(G[a, k])), (a, k, fd, G[a, k])
+
+
+# ------------------------------------------------------------------ strain derivative / virial
+def _fd_strain(model, pos64, Z, box, pbc, a, b, h):
+    """Central finite difference of the oracle energy under r -> (1 + eps) r, box -> (1 + eps) box, eps = h e_a e_b^T."""
+    out = []
+    for sgn in (+1.0, -1.0):
+        eps = np.eye(3)
+        eps[a, b] += sgn * h
+        p = (pos64 @ eps.T).astype(np.float32)
+        bx = (np.asarray(box, np.float64).reshape(3, 3) @ eps.T).astype(np.float32).reshape(9) if pbc else box
+        out.append(oracle.evaluate(model, p, Z, bx, pbc, None, want_forces=False)["energy"])
+    return (out[0] - out[1]) / (2 * h)
+
+
+def test_virial_is_the_strain_derivative_periodic_axes():
+    cfg = get_config(0)
+    m = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    r = oracle.evaluate_virial(m, cfg["pos"], cfg["Z"], cfg["box"], 1)
+    W = r["virial"]
+    ref = oracle.evaluate(m, cfg["pos"], cfg["Z"], cfg["box"], 1)
+    assert abs(r["energy"] - ref["energy"]) < 1e-12 and np.allclose(r["forces"], ref["forces"], atol=1e-12)
+    assert np.abs(W - W.T).max() < 1e-8 * np.abs(W).max()          # rotation invariance of every E_i
+    for a in range(3):                                             # axis scaling keeps the box orthorhombic
+        fd = _fd_strain(m, cfg["pos64"], cfg["Z"], cfg["box"], 1, a, a, 2e-4)
+        assert abs(fd - W[a, a]) < 2e-3 * (1 + abs(W[a, a])), (a, fd, W[a, a])
+
+
+def test_virial_shear_and_force_moment_open_boundaries():
+    cfg = get_config(4)
+    ml = cfg["ml_index"]
+    pos64 = cfg["pos64"][ml] - cfg["pos64"][ml].mean(0) + 20.0
+    Z = cfg["Z"][ml]
+    m = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    r = oracle.evaluate_virial(m, pos64.astype(np.float32), Z, cfg["box"], 0)
+    W, F = r["virial"], r["forces"]
+    # isolated cluster: W = -sum_a F_a (x) r_a  (sum F = 0 makes it origin independent)
+    M = -(F[:, :, None] * pos64.astype(np.float32).astype(np.float64)[:, None, :]).sum(0)
+    assert np.abs(W - M).max() < 1e-8 * (1 + np.abs(W).max())
+    for a, b in ((0, 1), (2, 0), (1, 2), (1, 1)):
+        fd = _fd_strain(m, pos64, Z, cfg["box"], 0, a, b, 2e-4)
+        assert abs(fd - W[a, b]) < 2e-3 * (1 + abs(W[a, b])), (a, b, fd, W[a, b])
