@@ -95,6 +95,12 @@ int nnp_workspace_set_mlp_mode(nnp_workspace*, int32_t mode);
  * 0 (default): only the column blocks that can be non-zero for the species present in the evaluation
  * (exact structural-zero compaction).  Results are identical up to summation order. */
 int nnp_workspace_set_dense_k(nnp_workspace*, int32_t dense);
+/* Strain derivative of the energy (the quantity a barostat needs; NPT runs in PAPER.md lines 92-94): with
+ * d_virial9 != NULL every later nnp_eval also writes DEVICE d_virial9[3*a+b] = dE/d eps_ab for the homogeneous
+ * deformation r -> (1 + eps) r of positions and box, accumulated from the pair partials of the force kernel,
+ *     W[a][b] = sum_i sum_{j in N(i)} (dE_i/dr_j)[a] (r_j - r_i)[b]      (minimum-image displacements),
+ * in 2^-32 fixed point (reproducible).  NULL (default) switches it off; the pointer must stay valid while set. */
+int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
 
 /* One energy+force evaluation.  Asynchronous on the workspace stream.
  *   d_pos      DEVICE [n_atoms][3] fp32, Angstrom, any periodic image

@@ -16,7 +16,7 @@ NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
     "nnp_model_create", "nnp_model_create_ensemble", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
-    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_eval",
+    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
@@ -66,6 +66,7 @@ def lib():
         L.nnp_workspace_destroy.argtypes = [vp]
         L.nnp_workspace_set_mlp_mode.argtypes = [vp, i32]
         L.nnp_workspace_set_dense_k.argtypes = [vp, i32]
+        L.nnp_workspace_set_virial_output.argtypes = [vp, vp]
         L.nnp_eval.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_eval_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_status.argtypes = [vp]
@@ -126,6 +127,10 @@ def nnp_workspace_set_mlp_mode(ws, mode):
 
 def nnp_workspace_set_dense_k(ws, dense):
     return lib().nnp_workspace_set_dense_k(ws, int(dense))
+
+
+def nnp_workspace_set_virial_output(ws, d_virial9):
+    return lib().nnp_workspace_set_virial_output(ws, d_virial9)
 
 
 def nnp_eval(ws, n_atoms, d_pos, d_Z, box_ptr, pbc, d_ml_index, n_ml, d_energy, d_forces):
@@ -257,6 +262,12 @@ class Workspace:
 
     def set_mlp_mode(self, mode):
         _check(nnp_workspace_set_mlp_mode(self.handle, mode), "nnp_workspace_set_mlp_mode")
+
+    def set_virial_output(self, virial):
+        """virial: (9,) or (3,3) float64 cuda tensor that every later eval fills with dE/d eps, or None to switch off."""
+        self._virial = virial
+        _check(nnp_workspace_set_virial_output(self.handle, None if virial is None else virial.data_ptr()),
+               "nnp_workspace_set_virial_output")
 
     def set_dense_k(self, dense):
         _check(nnp_workspace_set_dense_k(self.handle, dense), "nnp_workspace_set_dense_k")

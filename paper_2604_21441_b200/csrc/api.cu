@@ -163,7 +163,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
   void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
-                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->hd_pos, ws->hd_Z, ws->hd_ml,
+                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_energy, ws->hd_forces};
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -203,7 +203,8 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
             dmalloc(&ws->cntA, nm) && dmalloc(&ws->aev, nr * K) && dmalloc(&ws->daev, nr * K) &&
             dmalloc(&ws->hbuf[0], nr * HP) && dmalloc(&ws->hbuf[1], nr * HP) && dmalloc(&ws->hbuf[2], nr * HP) &&
             dmalloc(&ws->dbuf[0], nr * HP) && dmalloc(&ws->dbuf[1], nr * HP) && dmalloc(&ws->e_atom, nr) &&
-            dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->epart, nm / 256 + 2) && dmalloc(&ws->ticket, 1) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
+            dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->epart, nm / 256 + 2) && dmalloc(&ws->ticket, 1) && dmalloc(&ws->wcentre, 9 * nm) &&
+            dmalloc(&ws->wblk, 9 * (nm / 256 + 2)) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
             dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) && dmalloc(&ws->hd_energy, 1) &&
             dmalloc(&ws->hd_forces, 3 * (size_t)max_atoms);
   if (ok) ok = (tc_workspace_create(ws) == NNP_OK);
@@ -235,6 +236,12 @@ extern "C" int nnp_debug_stage_times(nnp_workspace* ws, float* ms) {
   if (!ws || !ms || !ws->profiling) return NNP_ERR_INVALID_ARG;
   CU_OK(cudaEventSynchronize(ws->ev[5]));
   for (int i = 0; i < 5; ++i) CU_OK(cudaEventElapsedTime(&ms[i], ws->ev[i], ws->ev[i + 1]));
+  return NNP_OK;
+}
+
+extern "C" int nnp_workspace_set_virial_output(nnp_workspace* ws, double* d_virial9) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  ws->d_virial = d_virial9;
   return NNP_OK;
 }
 

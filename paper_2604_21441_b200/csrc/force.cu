@@ -68,11 +68,12 @@ __device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, 
   return o;
 }
 
+template <bool VIRIAL>
 __global__ void __launch_bounds__(AEV_WARPS * 32, 4)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
-               const float* __restrict__ daev, unsigned long long* __restrict__ facc) {
+               const float* __restrict__ daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre) {
   __shared__ WarpEnv env[AEV_WARPS];
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
   __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block, times TILE_M
@@ -258,6 +259,9 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
 
   // ---- radial + assembly: lane <-> radial neighbour
   long long ox = 0, oy = 0, oz = 0;   // sum_j p_ij in fixed point
+  long long wv[9];                    // VIRIAL: sum_j p_ij (x) d_ij of this centre, 2^-32 fixed point
+#pragma unroll
+  for (int k = 0; k < 9; ++k) wv[k] = 0;
   for (int q0 = 0; q0 < nR; q0 += 32) {
     const int q = q0 + lane;
     if (q < nR) {
@@ -287,6 +291,13 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
       if (lo < nA && e.posA[lo] == q) { px += Pacc[w][lo][0]; py += Pacc[w][lo][1]; pz += Pacc[w][lo][2]; }
       const long long fx = to_fix(px), fy = to_fix(py), fz = to_fix(pz);
       ox += fx; oy += fy; oz += fz;
+      if (VIRIAL) {   // strain derivative dE/d eps_ab = sum p_ij[a] d_ij[b], d_ij = R u
+        const float pp[3] = {px, py, pz}, dd[3] = {uq.w * uq.x, uq.w * uq.y, uq.w * uq.z};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int b = 0; b < 3; ++b) wv[3 * a + b] += __float2ll_rn(pp[a] * dd[b] * 4294967296.0f);
+      }
       const int jp = (int)(rowR[q] & JMASK);
       atomicAdd(&facc[3 * (size_t)jp + 0], (unsigned long long)(-fx));
       atomicAdd(&facc[3 * (size_t)jp + 1], (unsigned long long)(-fy));
@@ -299,6 +310,13 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     atomicAdd(&facc[3 * (size_t)ip + 1], (unsigned long long)oy);
     atomicAdd(&facc[3 * (size_t)ip + 2], (unsigned long long)oz);
   }
+  if (VIRIAL) {
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+      for (int o = 16; o > 0; o >>= 1) wv[k] += shfl_xor_ll(wv[k], o);   // integer sums: exact, order free
+      if (lane == 0) wcentre[9 * (size_t)ip + k] = wv[k];
+    }
+  }
 }
 
 // K8b: facc (sorted order, fixed point; = sum_j (p_aj - p_ja) = +F) -> forces in the caller's atom order, and
@@ -308,8 +326,10 @@ __global__ void __launch_bounds__(256)
 k_force_out(const float4* __restrict__ spos, const unsigned long long* __restrict__ facc,
             const int32_t* __restrict__ ml, int n_ml, float* __restrict__ forces, const GroupInfo* __restrict__ grp,
             const float* __restrict__ e_atom, double* __restrict__ epart, unsigned int* __restrict__ ticket,
-            double* __restrict__ energy) {
+            double* __restrict__ energy, const long long* __restrict__ wcentre, long long* __restrict__ wblk,
+            double* __restrict__ virial) {
   __shared__ double wsum[8];
+  __shared__ long long vsum[8][9];
   __shared__ bool last;
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
@@ -325,7 +345,21 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
   }
   for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
   if (lane == 0) wsum[wp] = e;
+  if (virial) {   // per-centre strain derivatives (fixed point) -> block partial
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+      long long v = (ip < n_ml) ? wcentre[9 * (size_t)ip + k] : 0ll;
+      for (int o = 16; o > 0; o >>= 1) v += shfl_xor_ll(v, o);
+      if (lane == 0) vsum[wp][k] = v;
+    }
+  }
   __syncthreads();
+  if (virial && threadIdx.x < 9) {
+    long long v = 0;
+    for (int i = 0; i < 8; ++i) v += vsum[i][threadIdx.x];
+    wblk[9 * (size_t)blockIdx.x + threadIdx.x] = v;
+  }
+  if (virial) __syncthreads();
   if (threadIdx.x == 0) {
     double t = 0.0;
     for (int i = 0; i < 8; ++i) t += wsum[i];
@@ -339,6 +373,11 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
   double t = 0.0;
   for (int i = lane; i < (int)gridDim.x; i += 32) t += __ldcg(epart + i);
   for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+  if (virial && lane < 9) {
+    long long v = 0;
+    for (int i = 0; i < (int)gridDim.x; ++i) v += __ldcg(wblk + 9 * (size_t)i + lane);
+    virial[lane] = (double)v * (1.0 / 4294967296.0);
+  }
   if (lane == 0) { *energy = t; *ticket = 0u; }
 }
 
@@ -350,15 +389,22 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
   if (d_ml || n_ml <= 0) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
   if (n_ml > 0) {
     const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
-    k_aev_backward<<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR, ws->nbrA,
-                                                          ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
-                                                          ws->facc);
+    if (ws->d_virial)
+      k_aev_backward<true><<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR,
+                                                                  ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap,
+                                                                  ws->acap, ws->daev, ws->facc, ws->wcentre);
+    else
+      k_aev_backward<false><<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR,
+                                                                   ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap,
+                                                                   ws->acap, ws->daev, ws->facc, nullptr);
     prof_mark(ws, 4);
     k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces,
-                                                                   ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy);
+                                                                   ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy,
+                                                                   ws->wcentre, ws->wblk, ws->d_virial);
     nl += 2;
   } else {
     cudaMemsetAsync(d_energy, 0, sizeof(double), ws->stream);
+    if (ws->d_virial) cudaMemsetAsync(ws->d_virial, 0, 9 * sizeof(double), ws->stream);
   }
   return nl;
 }

@@ -147,6 +147,9 @@ struct nnp_workspace {
   unsigned long long* facc;  // [max_ml][3] int64 fixed point, indexed by sorted position
   double* epart;             // [ceil(max_ml/256)] block partial sums of E_i (K8)
   unsigned int* ticket;      // [1] last-block ticket of K8
+  long long* wcentre;        // [max_ml][9] per-centre strain derivative, 2^-32 fixed point (virial output on)
+  long long* wblk;           // [ceil(max_ml/256)][9] block partials of the above
+  double* d_virial;          // caller's DEVICE [9] output, or nullptr = virial off
   void* tc_ws;               // tensor-core path scratch
   int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
   cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end

@@ -459,3 +459,32 @@ def test_cuda_graph_capture_and_replay():
         torch.cuda.synchronize()
         assert ws.status() == 0
         assert torch.equal(E, E0) and torch.equal(F, F0)
+
+
+# ------------------------------------------------------------------ strain derivative / virial
+@pytest.mark.parametrize("k", [0, 1, 4])
+def test_virial_output(k):
+    """dE/d eps from the force kernel's pair partials (fixed point) against the oracle's fp64 pair sum; switching the
+    output on changes neither E nor F, and the result is bitwise reproducible."""
+    torch = _torch()
+    cfg = gen.get_config(k)
+    ml = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    n_ml = n if ml is None else len(ml)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate_virial(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nbr_mode=1 if n_ml > 2000 else 0)
+    m, ws = make(cfg)
+    E0, F0 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    W = torch.zeros(9, dtype=torch.float64, device="cuda")
+    ws.set_virial_output(W)
+    E1, F1 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    Wg = W.cpu().numpy().reshape(3, 3).copy()
+    E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert E1 == E0 and np.array_equal(F1, F0)
+    assert np.array_equal(W.cpu().numpy().reshape(3, 3), Wg)
+    scale = np.abs(ref["virial"]).max()
+    assert np.abs(Wg - ref["virial"]).max() <= 1e-3 * scale, (Wg, ref["virial"])     # same bar as the forces
+    assert np.abs(Wg - Wg.T).max() <= 1e-3 * scale
+    ws.set_virial_output(None)
+    E3, F3 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert E3 == E0 and np.array_equal(F3, F0)
