@@ -95,6 +95,11 @@ int nnp_workspace_set_mlp_mode(nnp_workspace*, int32_t mode);
  * 0 (default): only the column blocks that can be non-zero for the species present in the evaluation
  * (exact structural-zero compaction).  Results are identical up to summation order. */
 int nnp_workspace_set_dense_k(nnp_workspace*, int32_t dense);
+/* Unit conversion at the boundary (the MD engine's job in PAPER.md lines 75-77: GROMACS works in nm and kJ/mol).
+ * Positions and box are multiplied by angstrom_per_length_unit in fp64 and rounded to fp32 once; the model then runs
+ * in Angstrom / "eV" as always; E and the virial are multiplied by energy_units_per_ev, forces by
+ * energy_units_per_ev * angstrom_per_length_unit.  GROMACS: (10.0, 96.48533212).  Default (1, 1) = no conversion. */
+int nnp_workspace_set_units(nnp_workspace*, double angstrom_per_length_unit, double energy_units_per_ev);
 /* Strain derivative of the energy (the quantity a barostat needs; NPT runs in PAPER.md lines 92-94): with
  * d_virial9 != NULL every later nnp_eval also writes DEVICE d_virial9[3*a+b] = dE/d eps_ab for the homogeneous
  * deformation r -> (1 + eps) r of positions and box, accumulated from the pair partials of the force kernel,

@@ -16,7 +16,7 @@ NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
     "nnp_model_create", "nnp_model_create_ensemble", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
-    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_eval",
+    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
@@ -67,6 +67,7 @@ def lib():
         L.nnp_workspace_set_mlp_mode.argtypes = [vp, i32]
         L.nnp_workspace_set_dense_k.argtypes = [vp, i32]
         L.nnp_workspace_set_virial_output.argtypes = [vp, vp]
+        L.nnp_workspace_set_units.argtypes = [vp, C.c_double, C.c_double]
         L.nnp_eval.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_eval_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_status.argtypes = [vp]
@@ -127,6 +128,10 @@ def nnp_workspace_set_mlp_mode(ws, mode):
 
 def nnp_workspace_set_dense_k(ws, dense):
     return lib().nnp_workspace_set_dense_k(ws, int(dense))
+
+
+def nnp_workspace_set_units(ws, angstrom_per_length_unit, energy_units_per_ev):
+    return lib().nnp_workspace_set_units(ws, float(angstrom_per_length_unit), float(energy_units_per_ev))
 
 
 def nnp_workspace_set_virial_output(ws, d_virial9):
@@ -262,6 +267,9 @@ class Workspace:
 
     def set_mlp_mode(self, mode):
         _check(nnp_workspace_set_mlp_mode(self.handle, mode), "nnp_workspace_set_mlp_mode")
+
+    def set_units(self, angstrom_per_length_unit=1.0, energy_units_per_ev=1.0):
+        _check(nnp_workspace_set_units(self.handle, angstrom_per_length_unit, energy_units_per_ev), "nnp_workspace_set_units")
 
     def set_virial_output(self, virial):
         """virial: (9,) or (3,3) float64 cuda tensor that every later eval fills with dE/d eps, or None to switch off."""

@@ -163,7 +163,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
   void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
-                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->hd_pos, ws->hd_Z, ws->hd_ml,
+                  ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->pos_scaled, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_energy, ws->hd_forces};
   for (void* p : ptrs) if (p) cudaFree(p);
   cudaGetLastError();
@@ -184,6 +184,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
   ws->max_cells = (int)std::min<int64_t>(std::max<int64_t>(512, max_ml / 4), 1 << 21);
   ws->mlp_mode = m->tc ? NNP_MLP_F16X3 : NNP_MLP_FP32_SIMT;
   ws->dense_k = 0;
+  ws->len_scale = 1.0; ws->e_scale = 1.0;
   {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
@@ -204,7 +205,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
             dmalloc(&ws->hbuf[0], nr * HP) && dmalloc(&ws->hbuf[1], nr * HP) && dmalloc(&ws->hbuf[2], nr * HP) &&
             dmalloc(&ws->dbuf[0], nr * HP) && dmalloc(&ws->dbuf[1], nr * HP) && dmalloc(&ws->e_atom, nr) &&
             dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->epart, nm / 256 + 2) && dmalloc(&ws->ticket, 1) && dmalloc(&ws->wcentre, 9 * nm) &&
-            dmalloc(&ws->wblk, 9 * (nm / 256 + 2)) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
+            dmalloc(&ws->wblk, 9 * (nm / 256 + 2)) && dmalloc(&ws->pos_scaled, 3 * (size_t)max_atoms) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
             dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) && dmalloc(&ws->hd_energy, 1) &&
             dmalloc(&ws->hd_forces, 3 * (size_t)max_atoms);
   if (ok) ok = (tc_workspace_create(ws) == NNP_OK);
@@ -236,6 +237,20 @@ extern "C" int nnp_debug_stage_times(nnp_workspace* ws, float* ms) {
   if (!ws || !ms || !ws->profiling) return NNP_ERR_INVALID_ARG;
   CU_OK(cudaEventSynchronize(ws->ev[5]));
   for (int i = 0; i < 5; ++i) CU_OK(cudaEventElapsedTime(&ms[i], ws->ev[i], ws->ev[i + 1]));
+  return NNP_OK;
+}
+
+// positions in the caller's length unit -> Angstrom: converted in fp64 and rounded to fp32 ONCE; every later step
+// (cell binning and the pinned fp64 neighbour predicate included) works on the converted fp32 coordinates.
+__global__ void k_scale_pos(const float* __restrict__ in, float* __restrict__ out, long long n3, double s) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n3) out[i] = (float)((double)in[i] * s);
+}
+
+extern "C" int nnp_workspace_set_units(nnp_workspace* ws, double angstrom_per_length_unit, double energy_units_per_ev) {
+  if (!ws || !(angstrom_per_length_unit > 0.0) || !(energy_units_per_ev > 0.0)) return NNP_ERR_INVALID_ARG;
+  ws->len_scale = angstrom_per_length_unit;
+  ws->e_scale = energy_units_per_ev;
   return NNP_OK;
 }
 
@@ -274,7 +289,17 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   const float unit[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
   ws->n_atoms = n_atoms; ws->n_ml = n_ml; ws->d_ml_index = d_ml;
   prof_mark(ws, 0);
-  int nl = launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
+  int nl = 0;
+  float box_a[9];
+  if (ws->len_scale != 1.0) {   // unit conversion (GROMACS: nm -> Angstrom), see nnp_workspace_set_units
+    if (n_atoms > 0) {
+      k_scale_pos<<<(unsigned)((3 * n_atoms + 255) / 256), 256, 0, ws->stream>>>(d_pos, ws->pos_scaled, 3 * n_atoms, ws->len_scale);
+      ++nl;
+    }
+    d_pos = ws->pos_scaled;
+    if (pbc) { for (int i = 0; i < 9; ++i) box_a[i] = (float)((double)box[i] * ws->len_scale); box = box_a; }
+  }
+  nl += launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
   prof_mark(ws, 1);
   nl += launch_aev_forward(ws, n_ml);
   prof_mark(ws, 2);

@@ -327,7 +327,7 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
             const int32_t* __restrict__ ml, int n_ml, float* __restrict__ forces, const GroupInfo* __restrict__ grp,
             const float* __restrict__ e_atom, double* __restrict__ epart, unsigned int* __restrict__ ticket,
             double* __restrict__ energy, const long long* __restrict__ wcentre, long long* __restrict__ wblk,
-            double* __restrict__ virial) {
+            double* __restrict__ virial, double e_scale, double f_scale) {
   __shared__ double wsum[8];
   __shared__ long long vsum[8][9];
   __shared__ bool last;
@@ -338,7 +338,7 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
     const int w = __float_as_int(spos[ip].w);
     const int a = w & 0x0fffffff, slot = (w >> 28) & 7;
     const size_t o = ml ? (size_t)ml[a] : (size_t)a;
-    const double sc = 1.0 / 1099511627776.0;
+    const double sc = f_scale / 1099511627776.0;   // fixed point -> eV/Angstrom -> caller units
 #pragma unroll
     for (int d = 0; d < 3; ++d) forces[3 * o + d] = (float)((double)(long long)facc[3 * (size_t)ip + d] * sc);
     e = (double)e_atom[ip + grp->pad_shift[slot]];
@@ -376,9 +376,9 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
   if (virial && lane < 9) {
     long long v = 0;
     for (int i = 0; i < (int)gridDim.x; ++i) v += __ldcg(wblk + 9 * (size_t)i + lane);
-    virial[lane] = (double)v * (1.0 / 4294967296.0);
+    virial[lane] = (double)v * (e_scale / 4294967296.0);
   }
-  if (lane == 0) { *energy = t; *ticket = 0u; }
+  if (lane == 0) { *energy = t * e_scale; *ticket = 0u; }
 }
 
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
@@ -400,7 +400,8 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
     prof_mark(ws, 4);
     k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces,
                                                                    ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy,
-                                                                   ws->wcentre, ws->wblk, ws->d_virial);
+                                                                   ws->wcentre, ws->wblk, ws->d_virial, ws->e_scale,
+                                                                   ws->e_scale * ws->len_scale);
     nl += 2;
   } else {
     cudaMemsetAsync(d_energy, 0, sizeof(double), ws->stream);

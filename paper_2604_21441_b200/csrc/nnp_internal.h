@@ -150,6 +150,8 @@ struct nnp_workspace {
   long long* wcentre;        // [max_ml][9] per-centre strain derivative, 2^-32 fixed point (virial output on)
   long long* wblk;           // [ceil(max_ml/256)][9] block partials of the above
   double* d_virial;          // caller's DEVICE [9] output, or nullptr = virial off
+  float* pos_scaled;         // [max_atoms][3] positions converted to Angstrom (unit conversion on)
+  double len_scale, e_scale; // Angstrom per caller length unit; caller energy units per eV (1, 1 = off)
   void* tc_ws;               // tensor-core path scratch
   int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
   cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end

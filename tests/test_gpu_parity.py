@@ -488,3 +488,27 @@ def test_virial_output(k):
     ws.set_virial_output(None)
     E3, F3 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
     assert E3 == E0 and np.array_equal(F3, F0)
+
+
+def test_unit_conversion_nm_kjmol():
+    """GROMACS units at the boundary: positions/box in nm, energies in kJ/mol, forces in kJ/mol/nm.  Reading #33: the
+    conversion to Angstrom is one fp64 multiply rounded to fp32; the oracle is fed exactly those coordinates."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    pos_nm = (cfg["pos64"] / 10.0).astype(np.float32)
+    box_nm = (cfg["box"].astype(np.float64) / 10.0).astype(np.float32)
+    pos_a = (pos_nm.astype(np.float64) * 10.0).astype(np.float32)
+    box_a = (box_nm.astype(np.float64) * 10.0).astype(np.float32)
+    KJ = 96.48533212
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate_virial(om, pos_a, cfg["Z"], box_a, 1, None, nbr_mode=1)
+    m, ws = make(cfg)
+    ws.set_units(10.0, KJ)
+    W = torch.zeros(9, dtype=torch.float64, device="cuda")
+    ws.set_virial_output(W)
+    Eg, Fg = run_gpu(ws, pos_nm, cfg["Z"], box_nm)
+    check_lists(ws, dict(cfg, box=box_a), pos_a, n)
+    check_EF(Eg / KJ, Fg / (KJ * 10.0), ref, n)
+    Wg = W.cpu().numpy().reshape(3, 3) / KJ
+    assert np.abs(Wg - ref["virial"]).max() <= 1e-3 * np.abs(ref["virial"]).max()
