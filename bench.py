@@ -287,6 +287,50 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json's metric is quoted "vs water-box size": device-resident timing of every config (cfg 0-4), one JSON
+    line each (not the contract line; run explicitly with --sweep).  Positions cycle over 4 perturbed sets, L2 flushed."""
+    import torch
+    import paper_2604_21441_b200 as nnp
+    torch.cuda.set_device(0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for k in range(5):
+        cfg = gen.get_config(k)
+        n = cfg["pos"].shape[0]
+        ml = cfg["ml_index"]
+        n_ml = n if ml is None else len(ml)
+        P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 4)
+        model = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+        ws = nnp.Workspace(model, n, n_ml)
+        dpos = [torch.from_numpy(P[t]).cuda() for t in range(4)]
+        dZ = torch.from_numpy(cfg["Z"]).cuda()
+        dml = None if ml is None else torch.from_numpy(ml).cuda()
+        E = torch.zeros(1, dtype=torch.float64, device="cuda")
+        F = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
+        for t in range(5):
+            ws.eval(dpos[t % 4], dZ, cfg["box"], 1, dml, E, F)
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        ws.set_profiling(1)
+        steps = args.steps if k < 3 else max(10, args.steps // 4)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        stage = np.zeros(5)
+        for i in range(steps):
+            flush.zero_()
+            ev[i][0].record()
+            ws.eval(dpos[i % 4], dZ, cfg["box"], 1, dml, E, F)
+            ev[i][1].record()
+            stage += ws.stage_times()
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b in ev])
+        print(json.dumps({"sweep": True, "metric": METRIC, "unit": UNIT, "config": {"workload": cfg["name"], "n_atoms": n, "n_ml": n_ml},
+                          "value": n_ml / (ms.mean() * 1e-3), "ms_per_step": float(ms.mean()), "ms_per_step_min": float(ms.min()),
+                          "ns_per_day_2fs": 0.1728 / (ms.mean() * 1e-3), "steps": steps,
+                          "stage_ms": dict(zip(["neighbour", "aev_forward", "mlp", "aev_backward", "output"],
+                                               [float(x) for x in stage / steps]))}), flush=True)
+        del ws, model
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -297,12 +341,16 @@ def main():
     ap.add_argument("--ensemble", type=int, default=1, help="networks per element (ANI-2x: 8); E = mean over members")
     ap.add_argument("--dense-k", action="store_true", help="materialise all 1008 AEV columns (K = 1024 first layer)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="time every BASELINE.json config (cfg 0-4), one extra JSON line each")
     ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_ours(args, rank, world, local_rank)

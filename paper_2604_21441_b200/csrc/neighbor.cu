@@ -374,7 +374,7 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
     }
     __syncthreads();
     // ---- sweep: one warp per centre
-    for (int ci = warp; ci < nC; ci += 8) {
+    for (int ci = warp + 8 * blockIdx.y; ci < nC; ci += 8 * gridDim.y) {   // small systems: gridDim.y blocks share a cell
       int s = 0;
       while (s + 1 < MAX_S && ci >= cenOff[s + 1]) ++s;
       const int ip = cenStart[s] + (ci - cenOff[s]);
@@ -521,7 +521,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   int nl = 1;
   if (n_ml > 0) {
     // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside
-    k_neighbors<<<ws->max_cells, 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->bstart, d_pos, d_ml,
+    // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
+    const int ysplit = (n_ml <= 2048) ? 8 : 1;
+    k_neighbors<<<dim3(ws->max_cells, ysplit), 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->bstart, d_pos, d_ml,
                                                (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
                                                ws->flags);
     ++nl;
