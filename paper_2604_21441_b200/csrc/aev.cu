@@ -62,6 +62,8 @@ k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __res
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
               float* __restrict__ aev) {
   __shared__ WarpEnv env[AEV_WARPS];
+  pdl_trigger();
+  pdl_wait();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int ip = blockIdx.x * AEV_WARPS + w;
   if (ip >= n_ml) return;
@@ -152,8 +154,8 @@ int launch_aev_forward(nnp_workspace* ws, int64_t n_ml) {
   if (n_ml <= 0) return 0;
   const nnp_model* m = ws->model;
   const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
-  k_aev_forward<<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR, ws->nbrA,
-                                                       ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->aev);
+  launch_pdl(!ws->profiling, ws->stream, k_aev_forward, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid, ws->groups,
+             ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->aev);
   return 1;
 }
 

@@ -291,6 +291,9 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   prof_mark(ws, 0);
   int nl = 0;
   float box_a[9];
+  ws->tile_done = nullptr;
+  // rows of non-ML atoms are +0.0f; with no index subset every row is written by k_force_out
+  if (n_atoms > 0 && (d_ml || n_ml <= 0)) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
   if (ws->len_scale != 1.0) {   // unit conversion (GROMACS: nm -> Angstrom), see nnp_workspace_set_units
     if (n_atoms > 0) {
       k_scale_pos<<<(unsigned)((3 * n_atoms + 255) / 256), 256, 0, ws->stream>>>(d_pos, ws->pos_scaled, 3 * n_atoms, ws->len_scale);

@@ -21,7 +21,7 @@ __device__ __forceinline__ long long shfl_xor_ll(long long v, int o) {
 // Both shares of one unordered angular pair {j,k} of centre i: oj = dE_i/dr_j and ok = dE_i/dr_k contributions of the
 // 32 sub-features of the pair's species block (SURVEY.md Appendix A "Forces"; gb = this centre's dE/dAEV pieces).
 struct PairShares { float jx, jy, jz, kx, ky, kz; };
-__device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, const float4* __restrict__ gb, float4 uj,
+__device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, const float4* gb, float4 uj,
                                                   float fj, float dfj, float4 uk, float fk, float dfk) {
   const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
   const float cc = c.cTheta * u;
@@ -73,10 +73,13 @@ __global__ void __launch_bounds__(AEV_WARPS * 32, 4)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
-               const float* __restrict__ daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre) {
+               const float* daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre,
+               const int* tile_done, int done_target) {
   __shared__ WarpEnv env[AEV_WARPS];
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
   __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block, times TILE_M
+  pdl_trigger();
+  if (!tile_done) pdl_wait();   // with per-tile flags the MLP kernel is NOT awaited as a whole (see below)
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   if (threadIdx.x < MAX_S * MAX_S) {
     const int sa = threadIdx.x / MAX_S, sb = threadIdx.x % MAX_S;
@@ -84,6 +87,27 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     int off = 0;
     if (s2 < c.S) { const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)]; off = max(cp, 0) * (BLK / 4) * TILE_M; }
     pairoff[threadIdx.x] = off;
+  }
+  // Overlap with the MLP kernel (programmatic dependent launch): this grid may start while the persistent MLP CTAs
+  // are still on their last tiles; a centre only needs ITS OWN row of dE/dAEV, so the block waits for the completion
+  // flags of its centres' 128-row tiles (released by the MLP epilogue after the tile's last store) instead of the
+  // whole kernel.  Thread t looks after centre t and polls only where the tile changes (the rows of a block are
+  // contiguous: one poller per block almost always -- thousands of polling warps saturate the L2 slice that holds
+  // the flags and slow the MLP's weight stream down).  dE/dAEV is read through ordinary (coherent) loads.
+  if (tile_done && threadIdx.x < AEV_WARPS) {
+    const int ipw = blockIdx.x * AEV_WARPS + threadIdx.x;
+    if (ipw < n_ml) {
+      const int tw = (ipw + grp->pad_shift[(__float_as_int(spos[ipw].w) >> 28) & 7]) / TILE_M;
+      bool poll = true;
+      if (threadIdx.x > 0) poll = tw != (ipw - 1 + grp->pad_shift[(__float_as_int(spos[ipw - 1].w) >> 28) & 7]) / TILE_M;
+      if (poll) {
+        int seen;
+        do {
+          asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(tile_done + tw) : "memory");
+          if (seen < done_target) __nanosleep(500);
+        } while (seen < done_target);
+      }
+    }
   }
   __syncthreads();
   const int ip = blockIdx.x * AEV_WARPS + w;
@@ -96,7 +120,8 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   load_env(c, g, spos, rowR, nbrA + (size_t)ip * acap, nR, nA, ci, lane, e);
   const int Kc = grp->Kc;
   // row of dE/dAEV in the piece-major tile layout: float4 piece q of this row = gi4[q * TILE_M]
-  const float4* __restrict__ gi4 = reinterpret_cast<const float4*>(daev + daev_off((size_t)(ip + grp->pad_shift[si]), 0, Kc));
+  const size_t grow = (size_t)(ip + grp->pad_shift[si]);
+  const float4* gi4 = reinterpret_cast<const float4*>(daev + daev_off(grow, 0, Kc));
 
   // ---- angular: p_ij for the angular neighbours, staged in Pacc
   if (nA <= 32) {
@@ -204,7 +229,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const int sk = e.slotA[k];
         const int s1 = min(sj, sk), s2 = max(sj, sk);
         const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
-        const float4* __restrict__ gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
+        const float4* gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
         const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
         const float cc = c.cTheta * u;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
@@ -267,7 +292,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     if (q < nR) {
       const float4 uq = e.u[q];
       const int s = e.slotR[q];
-      const float4* __restrict__ gr = gi4 + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * TILE_M;
+      const float4* gr = gi4 + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * TILE_M;
       const float f = e.wR[q];   // c_R f_C
       float fc, dfc;
       cutoff(fminf(uq.w, c.Rcr), c.inv_Rcr, fc, dfc);
@@ -331,6 +356,8 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
   __shared__ double wsum[8];
   __shared__ long long vsum[8][9];
   __shared__ bool last;
+  pdl_trigger();
+  pdl_wait();
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
   double e = 0.0;
@@ -385,23 +412,24 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
                        float* d_forces) {
   const nnp_model* m = ws->model;
   int nl = 0;
-  // rows of non-ML atoms are +0.0f; with no index subset every row is written by k_force_out
-  if (d_ml || n_ml <= 0) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
+  // (rows of non-ML atoms are +0.0f: nnp_eval clears the force array before the first kernel when a subset is given)
   if (n_ml > 0) {
     const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
+    // after the tcgen05 MLP kernel the launch is a programmatic dependent launch: blocks start on the SMs the
+    // persistent MLP CTAs have left and wait per tile (see the kernel); stage profiling keeps the stages apart
+    const int* done = ws->profiling ? nullptr : ws->tile_done;
     if (ws->d_virial)
-      k_aev_backward<true><<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR,
-                                                                  ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap,
-                                                                  ws->acap, ws->daev, ws->facc, ws->wcentre);
+      launch_pdl(done != nullptr, ws->stream, k_aev_backward<true>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
+                 ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
+                 ws->facc, ws->wcentre, done, ws->tile_done_target);
     else
-      k_aev_backward<false><<<nb, AEV_WARPS * 32, 0, ws->stream>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->nbrR,
-                                                                   ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap,
-                                                                   ws->acap, ws->daev, ws->facc, nullptr);
+      launch_pdl(done != nullptr, ws->stream, k_aev_backward<false>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
+                 ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
+                 ws->facc, nullptr, done, ws->tile_done_target);
     prof_mark(ws, 4);
-    k_force_out<<<(int)((n_ml + 255) / 256), 256, 0, ws->stream>>>(ws->spos, ws->facc, d_ml, (int)n_ml, d_forces,
-                                                                   ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy,
-                                                                   ws->wcentre, ws->wblk, ws->d_virial, ws->e_scale,
-                                                                   ws->e_scale * ws->len_scale);
+    launch_pdl(!ws->profiling, ws->stream, k_force_out, dim3((unsigned)((n_ml + 255) / 256)), dim3(256), 0, ws->spos, ws->facc,
+               d_ml, (int)n_ml, d_forces, ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy, ws->wcentre, ws->wblk,
+               ws->d_virial, ws->e_scale, ws->e_scale * ws->len_scale);
     nl += 2;
   } else {
     cudaMemsetAsync(d_energy, 0, sizeof(double), ws->stream);

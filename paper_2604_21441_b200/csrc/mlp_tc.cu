@@ -23,9 +23,11 @@ namespace nnp {
 
 // ------------------------------------------------------------------------------------------------ image geometry
 // A B-operand matrix [N][K] (row n = output column, K contiguous) is cut into N-chunks of tc_chunk(N) rows
-// (<= 128, one MMA each) and K-panels of 64 columns.  Block (c, p) holds rows x 64 fp16 as rows x 128 bytes in
+// (<= 256, one MMA each: every layer width of the supported networks is ONE chunk, so the A operand is read from
+// shared memory once per k-step -- with two 128-row chunks the A re-read made the MMAs shared-memory bound) and
+// K-panels of 64 columns.  Block (c, p) holds rows x 64 fp16 as rows x 128 bytes in
 // the SWIZZLE_128B K-major layout (8-row atoms of 1024 B; 16-byte chunk index XOR row%8), hi half then lo half.
-__host__ __device__ inline int tc_nchunks(int N) { return (N + 127) / 128; }
+__host__ __device__ inline int tc_nchunks(int N) { return (N + 255) / 256; }
 __host__ __device__ inline int tc_chunk(int N) { const int nc = tc_nchunks(N); return (((N + nc - 1) / nc) + 15) & ~15; }
 __host__ __device__ inline int tc_npanels(int K) { return (K + 63) / 64; }
 __host__ __device__ inline size_t tc_img_bytes(int N, int K) {
@@ -102,22 +104,22 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
       "}\n" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
-// One k-step (K = 16) of the tile product, issued by one elected lane of a CONVERGED warp (predicated, so the
-// compiler emits straight-line code instead of a per-thread retry loop): hi*hi (+ lo*hi + hi*lo for the split).
-template <int NPASS>
-__device__ __forceinline__ void tc_mma_step(uint32_t d_tmem, uint64_t a_hi, uint64_t a_lo, uint64_t b_hi, uint64_t b_lo,
-                                            uint32_t idesc, uint32_t acc) {
-  if (NPASS == 3) {
+// One k-step (K = 16) against a B half-block, issued by one elected lane of a CONVERGED warp (predicated, so the
+// compiler emits straight-line code instead of a per-thread retry loop).  TWO = true: the B_hi block takes
+// A_hi * B_hi and A_lo * B_hi; TWO = false: one product (A_hi * B_hi of the single-pass mode, or A_hi * B_lo).
+template <bool TWO>
+__device__ __forceinline__ void tc_mma_step(uint32_t d_tmem, uint64_t a0, uint64_t a1, uint64_t b, uint32_t idesc,
+                                            uint32_t acc) {
+  if (TWO) {
     asm volatile(
         "{\n"
         ".reg .pred pe, pa, pt;\n"
         "elect.sync _|pe, 0xffffffff;\n"
-        "setp.ne.b32 pa, %6, 0;\n"
-        "setp.eq.b32 pt, %6, %6;\n"
-        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %3, %5, pa;\n"
-        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %2, %3, %5, pt;\n"
-        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %4, %5, pt;\n"
-        "}\n" ::"r"(d_tmem), "l"(a_hi), "l"(a_lo), "l"(b_hi), "l"(b_lo), "r"(idesc), "r"(acc) : "memory");
+        "setp.ne.b32 pa, %5, 0;\n"
+        "setp.eq.b32 pt, %5, %5;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %3, %4, pa;\n"
+        "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %2, %3, %4, pt;\n"
+        "}\n" ::"r"(d_tmem), "l"(a0), "l"(a1), "l"(b), "r"(idesc), "r"(acc) : "memory");
   } else {
     asm volatile(
         "{\n"
@@ -125,7 +127,7 @@ __device__ __forceinline__ void tc_mma_step(uint32_t d_tmem, uint64_t a_hi, uint
         "elect.sync _|pe, 0xffffffff;\n"
         "setp.ne.b32 pa, %4, 0;\n"
         "@pe tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, pa;\n"
-        "}\n" ::"r"(d_tmem), "l"(a_hi), "l"(b_hi), "r"(idesc), "r"(acc) : "memory");
+        "}\n" ::"r"(d_tmem), "l"(a0), "l"(b), "r"(idesc), "r"(acc) : "memory");
   }
 }
 __device__ __forceinline__ void tc_commit_elect(uint32_t bar) {
@@ -210,6 +212,8 @@ __device__ __forceinline__ void tc_store8(uint8_t* img, size_t blk_hi, size_t bl
 __global__ void __launch_bounds__(256)
 k_tc_pack_w1(const NetTable* __restrict__ all_nets, const GroupInfo* __restrict__ grp, TcPackAll all,
              unsigned long long* __restrict__ key, int* __restrict__ done, int max_tiles) {
+  pdl_trigger();
+  pdl_wait();
   {  // every call: clear the ensemble hand-over flags of the MLP kernel that follows
     const int nthr = gridDim.x * gridDim.y * gridDim.z * blockDim.x;
     const int gid = ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
@@ -256,9 +260,9 @@ constexpr uint32_t TC_P1 = 0, TC_P2 = 128;            // TMEM columns of the pac
 
 template <int NPASS> struct TcCfg {
   static constexpr int NH = (NPASS == 3) ? 2 : 1;
-  static constexpr int NST = (NPASS == 3) ? 3 : 6;
+  static constexpr int NST = (NPASS == 3) ? 3 : 4;
   static constexpr uint32_t ABUF = NH * 4 * TC_PANEL;
-  static constexpr uint32_t STAGE = NH * TC_PANEL;
+  static constexpr uint32_t STAGE = 2 * TC_PANEL;               // one half-block: <= 256 rows x 128 B
   static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], a_ready, acc_full
   static constexpr uint32_t TPTR = BARS + (2 * NST + 2) * 8;
   static constexpr uint32_t EPART = TPTR + 16;
@@ -271,8 +275,8 @@ struct TileNet {
 };
 
 // The six GEMMs of one tile as "rounds": a round reads the A operand resident in shared memory (<= 4 K-panels) and
-// fills <= 256 accumulator columns (<= 2 N-chunks).  F1 is K-streamed in rounds of 4 panels when Kc > 256, B1 is
-// N-streamed in rounds of 2 chunks when Kc > 256.  The producer and the MMA issuer walk the same table with ONE
+// fills <= 256 accumulator columns (one N-chunk).  F1 is K-streamed in rounds of 4 panels when Kc > 256, B1 is
+// N-streamed in rounds of one chunk when Kc > 256.  A ring stage holds one half-block (hi or lo) of B.  The producer and the MMA issuer walk the same table with ONE
 // copy of their block loop (an inlined copy per GEMM made the kernel overflow the instruction cache).
 struct TcRound {
   const uint8_t* img;   // B image [N][K]
@@ -290,8 +294,8 @@ __device__ __forceinline__ int tc_build_rounds(const TileNet& t, TcRound* r) {
   r[n++] = TcRound{t.w3t, t.N2, t.N3, 0, tc_nchunks(t.N2), 0, tc_npanels(t.N3), 0};
   r[n++] = TcRound{t.w2t, t.N1, t.N2, 0, tc_nchunks(t.N1), 0, tc_npanels(t.N2), 0};
   const int nc = tc_nchunks(t.Kc);
-  for (int c0 = 0; c0 < nc && n < TC_MAX_ROUNDS; c0 += 2)
-    r[n++] = TcRound{t.b1, t.Kc, t.N1, c0, min(nc, c0 + 2), 0, tc_npanels(t.N1), 0};
+  for (int c0 = 0; c0 < nc && n < TC_MAX_ROUNDS; ++c0)
+    r[n++] = TcRound{t.b1, t.Kc, t.N1, c0, c0 + 1, 0, tc_npanels(t.N1), 0};
   return n;
 }
 
@@ -326,7 +330,6 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
   volatile uint32_t* tptr = reinterpret_cast<volatile uint32_t*>(smem + C::TPTR);
   float* e_part = reinterpret_cast<float*>(smem + C::EPART);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_tiles = grp->n_tiles, Kc = grp->Kc;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::NST; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
@@ -342,6 +345,11 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tptr;
+  // barriers and TMEM are set up while the previous kernels drain; nothing they produce is read before this wait.
+  // The AEV backward kernel is this grid's programmatic dependent: it starts on the SMs this grid has left.
+  pdl_wait();
+  pdl_trigger();
+  const int n_tiles = grp->n_tiles, Kc = grp->Kc;
 
   // Work items are (member, tile) pairs in member-major order, dealt round-robin to the resident CTAs: with an
   // ensemble the 8 x 188 items fill the SMs evenly instead of 8 launches of 1.27 waves each.  Members of one tile
@@ -374,18 +382,18 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
           for (int c = c0; c < c1; ++c) {
             const uint32_t bytes = (uint32_t)min(ch, N - c * ch) * 128u;
             for (int p = p0; p < p1; ++p) {
-              mbar_wait(bar_empty + 8 * s, ph ^ 1);
-              mbar_expect_tx(bar_full + 8 * s, bytes * C::NH);
-              // each half-block goes out as four bulk copies: more requests in flight towards the L2 slices
+              // each half-block is a stage and goes out as four bulk copies: more requests in flight towards L2
               const uint32_t qb = bytes >> 2;
 #pragma unroll
               for (int h = 0; h < C::NH; ++h) {
+                mbar_wait(bar_empty + 8 * s, ph ^ 1);
+                mbar_expect_tx(bar_full + 8 * s, bytes);
                 const uint8_t* src = img + tc_blk_off(N, K, c, p, h);
-                const uint32_t dst = stage0 + s * C::STAGE + h * TC_PANEL;
+                const uint32_t dst = stage0 + s * C::STAGE;
 #pragma unroll
                 for (int u = 0; u < 4; ++u) bulk_g2s(dst + u * qb, src + u * qb, qb, bar_full + 8 * s);
+                if (++s == C::NST) { s = 0; ph ^= 1; }
               }
-              if (++s == C::NST) { s = 0; ph ^= 1; }
             }
           }
         }
@@ -412,21 +420,37 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             const int rows = min(ch, N - c * ch);
             const uint32_t idesc = tc_idesc(rows), d = tmem + TC_ACC + (uint32_t)((c - c0) * ch);
             for (int p = p0; p < p1; ++p) {
-              mbar_wait(bar_full + 8 * s, ph);
-              tc_fence_after();
               const int nks = min(4, (K - p * 64) >> 4);
-              const uint32_t a0 = abuf + (uint32_t)(p - p0) * TC_PANEL, b0 = stage0 + s * C::STAGE;
-              uint64_t ah = tc_desc(a0), al = tc_desc(a0 + TC_LO), bh = tc_desc(b0), bl = tc_desc(b0 + TC_PANEL);
-              uint32_t acc = (acc_first || p > p0) ? 1u : 0u;
+              const uint32_t a0 = abuf + (uint32_t)(p - p0) * TC_PANEL;
+              {   // B_hi block: A_hi * B_hi (+ A_lo * B_hi for the split)
+                mbar_wait(bar_full + 8 * s, ph);
+                tc_fence_after();
+                uint64_t ah = tc_desc(a0), al = tc_desc(a0 + TC_LO), b = tc_desc(stage0 + s * C::STAGE);
+                uint32_t acc = (acc_first || p > p0) ? 1u : 0u;
 #pragma unroll
-              for (int ks = 0; ks < 4; ++ks) {
-                if (ks < nks) {
-                  tc_mma_step<NPASS>(d, ah, al, bh, bl, idesc, acc);
-                  acc = 1u; ah += 2; al += 2; bh += 2; bl += 2;
+                for (int ks = 0; ks < 4; ++ks) {
+                  if (ks < nks) {
+                    tc_mma_step<NPASS == 3>(d, ah, al, b, idesc, acc);
+                    acc = 1u; ah += 2; al += 2; b += 2;
+                  }
                 }
+                tc_commit_elect(bar_empty + 8 * s);  // frees the stage when these MMAs have read it
+                if (++s == C::NST) { s = 0; ph ^= 1; }
               }
-              tc_commit_elect(bar_empty + 8 * s);  // frees the stage when these MMAs have read it
-              if (++s == C::NST) { s = 0; ph ^= 1; }
+              if (NPASS == 3) {   // B_lo block: A_hi * B_lo
+                mbar_wait(bar_full + 8 * s, ph);
+                tc_fence_after();
+                uint64_t ah = tc_desc(a0), b = tc_desc(stage0 + s * C::STAGE);
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) {
+                  if (ks < nks) {
+                    tc_mma_step<false>(d, ah, ah, b, idesc, 1u);
+                    ah += 2; b += 2;
+                  }
+                }
+                tc_commit_elect(bar_empty + 8 * s);
+                if (++s == C::NST) { s = 0; ph ^= 1; }
+              }
             }
           }
           tc_commit_elect(bar_acc);                // accumulator complete (and the A operand no longer read)
@@ -585,8 +609,8 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       // ---- B1 rounds: g = dE/dAEV columns [n0, n0 + ncols) -> global (fp32, compacted AEV column order)
       {
         const int nc = tc_nchunks(Kc), ch = tc_chunk(Kc);
-        for (int c0 = 0; c0 < nc; c0 += 2) {
-          const int n0 = c0 * ch, ncols = min(Kc, (c0 + 2) * ch) - n0;
+        for (int c0 = 0; c0 < nc; ++c0) {
+          const int n0 = c0 * ch, ncols = min(Kc, (c0 + 1) * ch) - n0;
           float* __restrict__ dst = daev + daev_off((size_t)(ti.row0 + row), n0, Kc);   // piece-major tile layout
 #pragma unroll 1
           for (int j = part; j * 16 < ncols; j += TC_NPART) {
@@ -603,10 +627,11 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
               }
             }
           }
-          if (c0 + 2 < nc) signal_and_wait();
+          if (c0 + 1 < nc) signal_and_wait();
         }
         // the first round of the next tile re-arms through its own signal_and_wait (program order: loads above done)
-        if (n_members > 1) {   // publish this member's updates of the tile to the CTA that holds the next member
+        {   // publish this member's updates of the tile: to the CTA that holds the next member, and (last member) to
+            // the AEV backward kernel, whose warps wait for their tile's flag
           __threadfence();
           asm volatile("bar.sync 2, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
           if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(done + t), "r"(mem + 1) : "memory");
@@ -787,22 +812,22 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   TcModel* tm = static_cast<TcModel*>(m->tc);
   TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
   if (!tm || !tw) return launch_mlp_simt(ws, n_ml);
+  ws->tile_done = tw->done; ws->tile_done_target = m->n_members;
   TcPackAll pall;
   for (int mem = 0; mem < MAX_MEMBERS; ++mem)
     for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
-  k_tc_pack_w1<<<dim3(32, m->aev.S, m->n_members), 256, 0, ws->stream>>>(tm->d_nets, ws->groups, pall, tw->key, tw->done,
-                                                                         ws->max_tiles);
+  const bool pdl = !ws->profiling;
+  launch_pdl(pdl, ws->stream, k_tc_pack_w1, dim3(32, m->aev.S, m->n_members), dim3(256), 0, tm->d_nets, ws->groups, pall,
+             tw->key, tw->done, ws->max_tiles);
   // one persistent CTA per SM over the (member, tile) work items (all CTAs are co-resident: 1 CTA/SM by shared memory)
   const int grid = (int)std::min<int64_t>((int64_t)ws->max_tiles * m->n_members, tw->num_sms);
   const float escale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members
   if (ws->mlp_mode == NNP_MLP_F16X1)
-    k_mlp_tc<1><<<grid, TC_THREADS, tw->smem_bytes[1], ws->stream>>>(tm->d_nets, tm->d_tabs, tw->d_pall, ws->groups, ws->tiles,
-                                                                     ws->aev, ws->daev, ws->e_atom, tw->key, tw->done,
-                                                                     m->n_members, escale);
+    launch_pdl(pdl, ws->stream, k_mlp_tc<1>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[1], tm->d_nets, tm->d_tabs,
+               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale);
   else
-    k_mlp_tc<3><<<grid, TC_THREADS, tw->smem_bytes[0], ws->stream>>>(tm->d_nets, tm->d_tabs, tw->d_pall, ws->groups, ws->tiles,
-                                                                     ws->aev, ws->daev, ws->e_atom, tw->key, tw->done,
-                                                                     m->n_members, escale);
+    launch_pdl(pdl, ws->stream, k_mlp_tc<3>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[0], tm->d_nets, tm->d_tabs,
+               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale);
   return 2;
 }
 

@@ -247,10 +247,12 @@ __device__ void d_scatter(int vb, const GridInfo* __restrict__ g, const float4* 
 }
 
 // K1c: the atomic ranks above are not reproducible; order every bucket by ML index so that the sorted order
-// (and with it every summation order downstream) is identical from run to run.  One warp per bucket: buckets of
-// <= 32 atoms are ranked by counting (all-pairs compare through shuffles); longer ones fall back to one lane.
-__device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S,
-                                                     const int* __restrict__ bstart, float4* __restrict__ spos) {
+// (and with it every summation order downstream) is identical from run to run.  One warp per bucket, ranking by
+// counting (keys = ML indices are distinct, so ranks are a permutation): buckets of <= 32 atoms compare through
+// shuffles in registers; longer ones (a box of one cell: cfg 0 holds 64 H in one bucket) count against the bucket
+// in global memory, permute into the free tmp4 scratch and copy back.
+__device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S, const int* __restrict__ bstart,
+                              float4* spos, float4* scratch) {
   const int k = (vb * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (k >= S * g->ncell) return;
   const int lo = bstart[k], n = bstart[k + 1] - lo;
@@ -262,15 +264,17 @@ __device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S,
     int rank = 0;
     for (int o = 0; o < n; ++o) rank += (__shfl_sync(0xffffffffu, key, o) < key) ? 1 : 0;
     __syncwarp();
-    if (lane < n) spos[lo + rank] = v;   // keys (ML indices) are distinct: ranks are a permutation
-  } else if (lane == 0) {
-    for (int p = lo + 1; p < lo + n; ++p) {
-      float4 v = spos[p];
-      int key = __float_as_int(v.w) & 0x0fffffff;
-      int q = p - 1;
-      while (q >= lo && (__float_as_int(spos[q].w) & 0x0fffffff) > key) { spos[q + 1] = spos[q]; --q; }
-      spos[q + 1] = v;
+    if (lane < n) spos[lo + rank] = v;
+  } else {
+    for (int e = lane; e < n; e += 32) {
+      const float4 v = spos[lo + e];
+      const int key = __float_as_int(v.w) & 0x0fffffff;
+      int rank = 0;
+      for (int o = 0; o < n; ++o) rank += ((__float_as_int(spos[lo + o].w) & 0x0fffffff) < key) ? 1 : 0;
+      scratch[lo + rank] = v;
     }
+    __syncwarp();
+    for (int e = lane; e < n; e += 32) spos[lo + e] = scratch[lo + e];
   }
 }
 
@@ -307,6 +311,8 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
   __shared__ int segStart[NB_SEG], segOff[NB_SEG + 1], segCode[NB_SEG];
   __shared__ int cenStart[MAX_S], cenOff[MAX_S + 1];
   __shared__ int wsum[8];
+  pdl_trigger();
+  pdl_wait();
   const int cell = blockIdx.x, ncell = g->ncell;
   if (cell >= ncell) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -468,7 +474,7 @@ __global__ void __launch_bounds__(1024, 1) k_prep(PrepArgs a) {
     d_scatter(vb, a.grid, a.tmp4, a.rank, a.bstart, a.n_ml, a.spos, a.scell);
   sync_all();
   const int nbS = (S * a.grid->ncell * 32 + (int)blockDim.x - 1) / (int)blockDim.x;
-  for (int vb = blockIdx.x; vb < nbS; vb += gridDim.x) d_bucket_sort(vb, a.grid, S, a.bstart, a.spos);
+  for (int vb = blockIdx.x; vb < nbS; vb += gridDim.x) d_bucket_sort(vb, a.grid, S, a.bstart, a.spos, a.tmp4);
 }
 
 // ---------------------------------------------------------------- host launcher
@@ -523,9 +529,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside
     // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
     const int ysplit = (n_ml <= 2048) ? 8 : 1;
-    k_neighbors<<<dim3(ws->max_cells, ysplit), 256, 0, st>>>(m->aev, ws->grid, ws->groups, ws->spos, ws->bstart, d_pos, d_ml,
-                                               (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
-                                               ws->flags);
+    launch_pdl(!ws->profiling, st, k_neighbors, dim3(ws->max_cells, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
+               ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
+               ws->flags);
     ++nl;
   }
   return nl;

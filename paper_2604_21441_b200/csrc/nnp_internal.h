@@ -153,6 +153,8 @@ struct nnp_workspace {
   float* pos_scaled;         // [max_atoms][3] positions converted to Angstrom (unit conversion on)
   double len_scale, e_scale; // Angstrom per caller length unit; caller energy units per eV (1, 1 = off)
   void* tc_ws;               // tensor-core path scratch
+  const int* tile_done;      // per-tile completion flags of the last MLP launch (tcgen05 path), or nullptr
+  int tile_done_target;      // value a finished tile's flag holds (= ensemble members)
   int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
   cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end
   // host-buffer entry point
@@ -160,6 +162,25 @@ struct nnp_workspace {
 };
 
 namespace nnp {
+// Programmatic dependent launch (PDL): every kernel of one evaluation after k_prep is launched with the
+// programmatic-stream-serialization attribute, triggers its dependents at its top and then waits for its
+// predecessor's completion (griddepcontrol.wait: full completion + memory flush), so launch latency and block
+// scheduling of kernel n+1 overlap the tail of kernel n.  k_aev_backward alone does not wait for the whole MLP
+// kernel but per tile (force.cu).  Stage profiling (events between the kernels) switches the attribute off.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+template <class... KArgs, class... Args>
+inline void launch_pdl(bool pdl, cudaStream_t st, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
 inline void prof_mark(nnp_workspace* ws, int i) { if (ws->profiling) cudaEventRecord(ws->ev[i], ws->stream); }
 // stage launchers (each returns the number of kernels it launched)
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
