@@ -316,6 +316,7 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
   const int cell = blockIdx.x, ncell = g->ncell;
   if (cell >= ncell) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (cell == 0 && tid == 0 && (int)gridDim.x < ncell) atomicOr(flags, FLAG_ARG);   // host / device cell counts differ
   const int nc0 = g->nc[0], nc1 = g->nc[1], nc2 = g->nc[2], pbc = g->pbc, S = c.S;
   const int cz = cell % nc2, cy = (cell / nc2) % nc1, cx = cell / (nc1 * nc2);
   const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
@@ -526,10 +527,27 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   }
   int nl = 1;
   if (n_ml > 0) {
-    // the cell count is only known on the device: one block per cell of the capacity, guard on ncell inside
+    // one block per cell, guard on ncell inside.  Periodic boxes: the host repeats d_grid_setup's cell-count
+    // arithmetic (same doubles, same shrink loop), so no empty blocks are launched; open boundaries: the extent is
+    // only known on the device, one block per cell of the capacity.
+    int ncell_host = ws->max_cells;
+    if (pbc) {
+      const double cutoff = (double)m->aev.Rcr * (1.0 + 1e-4);
+      const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]};
+      int nc[3];
+      for (int d = 0; d < 3; ++d) { int n = (int)floor(ext[d] / cutoff); if (n < 3) n = 1; nc[d] = n; }
+      while ((long long)nc[0] * nc[1] * nc[2] > (long long)ws->max_cells) {
+        int d = 0;
+        if (nc[1] > nc[d]) d = 1;
+        if (nc[2] > nc[d]) d = 2;
+        nc[d] -= 1;
+        if (nc[d] < 3) nc[d] = 1;
+      }
+      ncell_host = nc[0] * nc[1] * nc[2];
+    }
     // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
     const int ysplit = (n_ml <= 2048) ? 8 : 1;
-    launch_pdl(!ws->profiling, st, k_neighbors, dim3(ws->max_cells, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
+    launch_pdl(!ws->profiling, st, k_neighbors, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
                ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
                ws->flags);
     ++nl;
