@@ -107,6 +107,19 @@ int nnp_workspace_set_units(nnp_workspace*, double angstrom_per_length_unit, dou
  * in 2^-32 fixed point (reproducible).  NULL (default) switches it off; the pointer must stay valid while set. */
 int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
 
+/* External pair list ("The 2026 version adds the internal pair-list built by GROMACS ... as
+ * available inputs").  With d_pairs != NULL every later nnp_eval takes its neighbour
+ * candidates from this list instead of its own cell search:
+ *   d_pairs  DEVICE [n_pairs][2] int32 GLOBAL atom indices (i, j), i != j, in any order; every unordered pair at most
+ *            once; it must contain every ML-ML pair within the radial cut-off under the minimum-image convention and
+ *            may contain more (a Verlet-buffered list): each pair is decided by the same pinned fp64 predicate as the
+ *            cell search, so the neighbour rows -- and E, F -- are those of nnp_eval without a list.  Pairs with a
+ *            non-ML end are ignored.  Read during every evaluation: the buffer must stay valid and unchanged while set.
+ * A pair listed twice or with i == j raises NNP_ERR_INVALID_ARG through nnp_status().  d_pairs = NULL (default)
+ * returns to the built-in cell search.  The list may be replaced between evaluations (list reuse over several MD
+ * steps is the caller's choice of buffer width). */
+int nnp_workspace_set_pair_list(nnp_workspace*, const int32_t* d_pairs, int64_t n_pairs);
+
 /* One energy+force evaluation.  Asynchronous on the workspace stream.
  *   d_pos      DEVICE [n_atoms][3] fp32, Angstrom, any periodic image
  *   d_Z        DEVICE [n_atoms] int32 atomic numbers (only ML atoms' entries are read)

@@ -260,6 +260,13 @@ extern "C" int nnp_workspace_set_virial_output(nnp_workspace* ws, double* d_viri
   return NNP_OK;
 }
 
+extern "C" int nnp_workspace_set_pair_list(nnp_workspace* ws, const int32_t* d_pairs, int64_t n_pairs) {
+  if (!ws || n_pairs < 0 || (n_pairs > 0 && !d_pairs)) return NNP_ERR_INVALID_ARG;
+  ws->ext_pairs = d_pairs;
+  ws->n_ext_pairs = d_pairs ? n_pairs : 0;
+  return NNP_OK;
+}
+
 extern "C" int nnp_workspace_set_dense_k(nnp_workspace* ws, int32_t dense) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   ws->dense_k = dense ? 1 : 0;

@@ -279,8 +279,8 @@ __device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S, con
 }
 
 // ---------------------------------------------------------------- K2: neighbour rows, one warp per centre
-__device__ __noinline__ double exact_d2(const float* __restrict__ pos, int oi, int oj, const GridInfo* g) {
-  double d[3];
+// minimum-image displacement r_oj - r_oi and its squared length, the pinned fp64 expression of reading #6
+__device__ __forceinline__ double exact_disp(const float* __restrict__ pos, int oi, int oj, const GridInfo* g, double d[3]) {
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     double x = (double)pos[3 * (size_t)oj + a] - (double)pos[3 * (size_t)oi + a];
@@ -288,6 +288,10 @@ __device__ __noinline__ double exact_d2(const float* __restrict__ pos, int oi, i
     d[a] = x;
   }
   return __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
+}
+__device__ __noinline__ double exact_d2(const float* __restrict__ pos, int oi, int oj, const GridInfo* g) {
+  double d[3];
+  return exact_disp(pos, oi, oj, g, d);
 }
 
 constexpr float GUARD_BAND = 2.0e-3f;  // Angstrom^2; >> fp32 error of d2 (~1e-5), reading #6
@@ -478,6 +482,112 @@ __global__ void __launch_bounds__(1024, 1) k_prep(PrepArgs a) {
   for (int vb = blockIdx.x; vb < nbS; vb += gridDim.x) d_bucket_sort(vb, a.grid, S, a.bstart, a.spos, a.tmp4);
 }
 
+// ---------------------------------------------------------------- external pair list
+// "The 2026 version adds the internal pair-list built by GROMACS ... as available inputs."  With a
+// list set (nnp_workspace_set_pair_list) K2's cell sweep is replaced by a filter over the engine's candidate pairs:
+// every pair is decided by the pinned fp64 predicate on the original coordinates (so a Verlet-buffered superset gives
+// exactly the rows of the cell search), appended to both rows, and the rows are then put in sorted-index order
+// (species-major, reproducible) with the angular subset marked.  K0-K1 still run: the sort groups atoms by element.
+
+// inv[ML-local index] = sorted position; row counters cleared
+__global__ void __launch_bounds__(256) k_pair_index(const float4* __restrict__ spos, int n_ml, int* __restrict__ inv,
+                                                    int* __restrict__ cntR) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ip >= n_ml) return;
+  inv[__float_as_int(spos[ip].w) & 0x0fffffff] = ip;
+  cntR[ip] = 0;
+}
+
+__device__ __forceinline__ int ml_local(const int32_t* __restrict__ ml, int n_ml, int gidx) {
+  if (!ml) return (gidx >= 0 && gidx < n_ml) ? gidx : -1;
+  int lo = 0, hi = n_ml - 1;
+  while (lo < hi) { const int mid = (lo + hi) >> 1; if (ml[mid] < gidx) lo = mid + 1; else hi = mid; }
+  return (n_ml > 0 && ml[lo] == gidx) ? lo : -1;
+}
+
+// one thread per candidate pair
+__global__ void __launch_bounds__(256)
+k_pair_fill(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const int* __restrict__ inv,
+            const float* __restrict__ pos, const int32_t* __restrict__ ml, int n_ml, const int32_t* __restrict__ pairs,
+            long long n_pairs, int rcap, uint32_t* __restrict__ nbrR, int* __restrict__ cntR, int* __restrict__ flags) {
+  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= n_pairs) return;
+  const int gi = pairs[2 * p], gj = pairs[2 * p + 1];
+  const int ai = ml_local(ml, n_ml, gi), aj = ml_local(ml, n_ml, gj);
+  if (ai < 0 || aj < 0) return;             // a pair with a non-ML end does not feed the AEV
+  if (ai == aj) { atomicOr(flags, FLAG_ARG); return; }
+  double d[3];
+  const double e2 = exact_disp(pos, gi, gj, g, d);
+  if (!(e2 <= c.Rcr2_d)) return;
+  if (e2 == 0.0) atomicOr(flags, FLAG_COINCIDENT);
+  const int ip = inv[ai], jp = inv[aj];
+  const float4 pi = spos[ip], pj = spos[jp];
+  // rows store the neighbour's cell offset: displacement = (local_j - local_i) + off * edge  (aev_common.cuh)
+  const float li[3] = {pi.x, pi.y, pi.z}, lj[3] = {pj.x, pj.y, pj.z};
+  uint32_t ci = 0u, cj = 0u;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const int off = (int)rint((d[a] - ((double)lj[a] - (double)li[a])) * g->inv_edge_d[a]);
+    if (off < -1 || off > 1) { atomicOr(flags, FLAG_ARG); return; }
+    ci |= (uint32_t)(off + 1) << (2 * a);
+    cj |= (uint32_t)(1 - off) << (2 * a);
+  }
+  const int qi = atomicAdd(&cntR[ip], 1), qj = atomicAdd(&cntR[jp], 1);
+  if (qi < rcap) nbrR[(size_t)ip * rcap + qi] = (uint32_t)jp | (ci << JBITS);
+  if (qj < rcap) nbrR[(size_t)jp * rcap + qj] = (uint32_t)ip | (cj << JBITS);
+  if (qi >= rcap || qj >= rcap) atomicOr(flags, FLAG_CAP);
+}
+
+// one warp per centre: order the row by sorted index (ranking by counting; a neighbour appears once), then the angular
+// subset by the pinned predicate, in row order
+__global__ void __launch_bounds__(256)
+k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const float* __restrict__ pos,
+            const int32_t* __restrict__ ml, int n_ml, int rcap, int acap, uint32_t* __restrict__ nbrR,
+            uint8_t* __restrict__ nbrA, int* __restrict__ cntR, int* __restrict__ cntA, int* __restrict__ flags) {
+  __shared__ uint32_t raw[8][RCAP_MAX], srt[8][RCAP_MAX];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int ip = blockIdx.x * 8 + w;
+  if (ip >= n_ml) return;
+  const int n = min(cntR[ip], rcap);
+  uint32_t* row = nbrR + (size_t)ip * rcap;
+  for (int q = lane; q < n; q += 32) raw[w][q] = row[q];
+  __syncwarp();
+  int dup = 0;
+  for (int q = lane; q < n; q += 32) {
+    const uint32_t e = raw[w][q], key = e & JMASK;
+    int rank = 0;
+    for (int o = 0; o < n; ++o) {
+      const uint32_t ko = raw[w][o] & JMASK;
+      rank += (ko < key || (ko == key && o < q)) ? 1 : 0;   // a permutation even for a (faulty) repeated pair
+      dup |= (ko == key && o != q) ? 1 : 0;
+    }
+    srt[w][rank] = e;
+  }
+  if (dup) atomicOr(flags, FLAG_ARG);   // a pair listed twice
+  __syncwarp();
+  const int a_i = __float_as_int(spos[ip].w) & 0x0fffffff;
+  const int o_i = ml ? ml[a_i] : a_i;
+  int nA = 0;
+  for (int q0 = 0; q0 < n; q0 += 32) {
+    const int q = q0 + lane;
+    bool inA = false;
+    if (q < n) {
+      const uint32_t e = srt[w][q];
+      row[q] = e;
+      const int a_j = __float_as_int(spos[e & JMASK].w) & 0x0fffffff;
+      inA = exact_d2(pos, o_i, ml ? ml[a_j] : a_j, g) <= c.Rca2_d;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, inA);
+    const int pA = nA + __popc(m & lanemask_lt());
+    if (inA && pA < acap) nbrA[(size_t)ip * acap + pA] = (uint8_t)q;
+    nA += __popc(m);
+  }
+  if (lane == 0) {
+    cntR[ip] = n; cntA[ip] = min(nA, acap);
+    if (nA > acap) atomicOr(flags, FLAG_CAP);
+  }
+}
+
 // ---------------------------------------------------------------- host launcher
 // Largest cluster (16, else the portable 8) that can hold k_prep's 1024-thread CTAs on this device; 0 = none.
 int prep_cluster_size() {
@@ -526,6 +636,17 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     cudaLaunchCooperativeKernel((const void*)k_prep<false>, dim3(grid), dim3(1024), args, 0, st);
   }
   int nl = 1;
+  if (n_ml > 0 && ws->ext_pairs) {
+    // external candidate pairs instead of the cell sweep (plain launches: fully ordered behind k_prep)
+    k_pair_index<<<(unsigned)((n_ml + 255) / 256), 256, 0, st>>>(ws->spos, (int)n_ml, ws->rank, ws->cntR);
+    if (ws->n_ext_pairs > 0)
+      k_pair_fill<<<(unsigned)((ws->n_ext_pairs + 255) / 256), 256, 0, st>>>(m->aev, ws->grid, ws->spos, ws->rank, d_pos, d_ml,
+                                                                            (int)n_ml, ws->ext_pairs, (long long)ws->n_ext_pairs,
+                                                                            ws->rcap, ws->nbrR, ws->cntR, ws->flags);
+    k_pair_rows<<<(unsigned)((n_ml + 7) / 8), 256, 0, st>>>(m->aev, ws->grid, ws->spos, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap,
+                                                           ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->flags);
+    return nl + 3;
+  }
   if (n_ml > 0) {
     // one block per cell, guard on ncell inside.  Periodic boxes: the host repeats d_grid_setup's cell-count
     // arithmetic (same doubles, same shrink loop), so no empty blocks are launched; open boundaries: the extent is

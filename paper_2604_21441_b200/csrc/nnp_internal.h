@@ -152,6 +152,8 @@ struct nnp_workspace {
   double* d_virial;          // caller's DEVICE [9] output, or nullptr = virial off
   float* pos_scaled;         // [max_atoms][3] positions converted to Angstrom (unit conversion on)
   double len_scale, e_scale; // Angstrom per caller length unit; caller energy units per eV (1, 1 = off)
+  const int32_t* ext_pairs;  // caller's DEVICE [n_ext_pairs][2] candidate pair list, or nullptr = own cell search
+  int64_t n_ext_pairs;
   void* tc_ws;               // tensor-core path scratch
   const int* tile_done;      // per-tile completion flags of the last MLP launch (tcgen05 path), or nullptr
   int tile_done_target;      // value a finished tile's flag holds (= ensemble members)

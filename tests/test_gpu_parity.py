@@ -512,3 +512,63 @@ def test_unit_conversion_nm_kjmol():
     check_EF(Eg / KJ, Fg / (KJ * 10.0), ref, n)
     Wg = W.cpu().numpy().reshape(3, 3) / KJ
     assert np.abs(Wg - ref["virial"]).max() <= 1e-3 * np.abs(ref["virial"]).max()
+
+
+# ------------------------------------------------------------------ external pair list
+def _buffered_pairs(pos, box, pbc, atoms, cutoff, seed):
+    """Candidate pairs as an MD engine's Verlet-buffered list would hold them: every unordered pair of `atoms` within
+    `cutoff` under the minimum image (numpy fp64, all pairs), in shuffled order with random (i, j) orientation."""
+    x = pos[atoms].astype(np.float64)
+    d = x[None, :, :] - x[:, None, :]
+    if pbc:
+        L = np.array([box[0], box[4], box[8]], dtype=np.float64)
+        d -= L * np.rint(d / L)
+    r2 = (d ** 2).sum(-1)
+    i, j = np.nonzero(np.triu(r2 <= cutoff * cutoff, k=1))
+    rng = np.random.default_rng(seed)
+    swap = rng.random(len(i)) < 0.5
+    a, b = np.where(swap, j, i), np.where(swap, i, j)
+    perm = rng.permutation(len(i))
+    return np.stack([atoms[a[perm]], atoms[b[perm]]], axis=1).astype(np.int32)
+
+
+@pytest.mark.parametrize("k,pbc", [(0, 1), (1, 1), (1, 0), (4, 1)])
+def test_external_pair_list(k, pbc):
+    """PAPER.md line 77 (2026 nnpot: the engine's pair list as a model input): with a buffered candidate list set, the
+    neighbour rows are bit-identical to the oracle's lists and E, F meet the same bars as the built-in cell search."""
+    torch = _torch()
+    cfg = gen.get_config(k)
+    ml = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    n_ml = n if ml is None else len(ml)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)
+    if ml is None:
+        atoms = np.arange(n)
+    else:   # the engine's list also holds pairs with MM ends: they must be ignored
+        mm = np.setdiff1d(np.arange(n), ml)
+        atoms = np.sort(np.concatenate([ml, np.random.default_rng(5).choice(mm, 400, replace=False)]))
+    pairs = _buffered_pairs(cfg["pos"], cfg["box"], pbc, atoms, cfg["aev"]["Rcr"] + 0.8, seed=11 + k)
+    m, ws = make(cfg)
+    E0, F0 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)        # built-in search
+    dpairs = torch.from_numpy(pairs).cuda()
+    ws.set_pair_list(dpairs)
+    E1, F1 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)
+    check_lists(ws, cfg, cfg["pos"], n_ml, ml, pbc)
+    check_EF(E1, F1, ref, n_ml, rows=ml)
+    assert abs(E1 - E0) / n_ml < 1e-6 and np.abs(F1 - F0).max() < 1e-4     # same rows, another summation order
+    E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)
+    assert E2 == E1 and np.array_equal(F2, F1)                             # reproducible despite the atomic row fill
+    # a pair listed twice is an argument error
+    dd = cfg["pos"][pairs[:, 1]].astype(np.float64) - cfg["pos"][pairs[:, 0]].astype(np.float64)
+    if pbc:
+        Lb = np.array([cfg["box"][0], cfg["box"][4], cfg["box"][8]], dtype=np.float64)
+        dd -= Lb * np.rint(dd / Lb)
+    inside = np.nonzero(((dd ** 2).sum(1) < 9.0) & np.isin(pairs, atoms if ml is None else ml).all(1))[0][:1]
+    ws.set_pair_list(torch.from_numpy(np.concatenate([pairs, pairs[inside, ::-1]]).copy()).cuda())
+    ws.eval(torch.from_numpy(cfg["pos"]).cuda(), torch.from_numpy(cfg["Z"]).cuda(), cfg["box"], pbc,
+            None if ml is None else torch.from_numpy(ml).cuda())
+    assert ws.status() != 0
+    ws.set_pair_list(None)
+    E3, F3 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)
+    assert E3 == E0 and np.array_equal(F3, F0)
