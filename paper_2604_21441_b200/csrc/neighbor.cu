@@ -621,7 +621,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
   a.dense_k = ws->dense_k;
   void* args[] = {&a};
-  if (ws->prep_cluster > 0 && n_ml <= 8192) {   // small systems: barrier latency dominates, a few SMs suffice
+  if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ws->prep_cluster); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = 0; cfg.stream = st;
     cudaLaunchAttribute at[1];

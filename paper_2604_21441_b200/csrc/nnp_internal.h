@@ -117,6 +117,7 @@ struct nnp_workspace {
   int max_cells;
   int num_sms;               // multiprocessor count of the device (cooperative grid size)
   int prep_cluster;          // CTAs of the single-cluster prep kernel (0: cooperative grid only)
+  int prep_cluster_max;      // largest n_ml the single-cluster variant takes
   int mlp_mode;
   int dense_k;               // 1: materialise every column block (no structural-zero compaction)
   int64_t max_rows;          // padded AEV rows
