@@ -534,7 +534,7 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
             const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
             const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
-            cp[i >> 1] = pack_c(z0 > 0.f ? 1.f : e0, z1 > 0.f ? 1.f : e1);
+            cp[i >> 1] = pack_c(e0, e1);   // CELU'(z) = exp(min(z, 0) / alpha): ex2(0) = 1 exactly, no select needed
             split2(h0, h1, hi[i >> 1], lo[i >> 1]);
           }
           tmem_st8(tlane + pcol + j * 8, cp);
@@ -566,7 +566,7 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
             const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
             e = fmaf(h0, wa, e); e = fmaf(h1, wb, e);
-            split2(escale * wa * (z0 > 0.f ? 1.f : e0), escale * wb * (z1 > 0.f ? 1.f : e1), hi[i >> 1], lo[i >> 1]);
+            split2(escale * wa * e0, escale * wb * e1, hi[i >> 1], lo[i >> 1]);   // e = CELU'(z) (1 for z > 0)
           }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
         }
