@@ -33,8 +33,8 @@ FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's main kernel, from the committed ncu full-set
-# capture profiles/r01d_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
-NCU_TRAFFIC_BYTES = {"neighbour": 0.563e6 + 58.1e3, "aev_forward": 8.08e6, "mlp": 18.3e6 + 2.05e3, "aev_backward": 21.0e6,
+# capture profiles/r01e_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
+NCU_TRAFFIC_BYTES = {"neighbour": 0.502e6 + 0.489e6, "aev_forward": 8.08e6, "mlp": 18.3e6, "aev_backward": 20.98e6,
                      "output": 1.07e6}
 
 
@@ -48,7 +48,7 @@ def peaks():
 
 
 class ClockSampler:
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -56,11 +56,19 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(dev), f"--query-gpu={self.Q}", "--format=csv,noheader",
-                                       "-lms", "25"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "10"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
-    def stop(self):
+    @staticmethod
+    def now():
+        import datetime
+        return datetime.datetime.now()
+
+    def stop(self, t0=None, t1=None):
+        """Median SM clock and throttle reasons over the samples whose nvidia-smi timestamp lies in [t0, t1] (the timed
+        region; the sampler is started earlier because nvidia-smi needs ~0.1 s to deliver its first line)."""
+        import datetime
         out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
         if self.p is None:
             return out
@@ -74,6 +82,20 @@ class ClockSampler:
         os.unlink(self.f.name)
         if not rows:
             return out
+        if t0 is not None:
+            sel = []
+            for r in rows:
+                try:
+                    ts = datetime.datetime.strptime(r[0].strip(), "%Y/%m/%d %H:%M:%S.%f")
+                except ValueError:
+                    continue
+                if t0 <= ts <= t1:
+                    sel.append(r)
+            out["samples_total"] = len(rows)
+            if sel:
+                rows = sel
+            else:
+                out["note"] = "no sample fell inside the timed region; all samples of the run are used"
         mhz = [float(r[1].split()[0]) for r in rows]
         reasons = set()
         for r in rows:
@@ -173,7 +195,9 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- warm-up (also collects the workload statistics used for the algorithmic work)
+    # ---- warm-up (also collects the workload statistics used for the algorithmic work).  The clock sampler starts
+    # here: nvidia-smi delivers its first line after ~0.1 s, longer than a short timed region.
+    clocks = ClockSampler(local_rank)
     for t in range(max(args.warmup, 3)):
         ws.eval(dpos[t % N_POS_SETS], dZ, box, 1, None, E, F)
     torch.cuda.synchronize()
@@ -190,9 +214,9 @@ def run_ours(args, rank, world, local_rank):
     # every stage boundary (which serialises the stages: their sum exceeds ms_per_step by the overlap).
     ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    clocks = ClockSampler(local_rank)
     barrier()
     wall0 = time.perf_counter()
+    ts0 = ClockSampler.now()
     for k in range(args.steps):
         flush.zero_()
         ev0[k].record()
@@ -200,7 +224,7 @@ def run_ours(args, rank, world, local_rank):
         ev1[k].record()
     barrier()
     wall = time.perf_counter() - wall0
-    clk = clocks.stop()
+    clk = clocks.stop(ts0, ClockSampler.now())
     assert ws.status() == 0
     ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
     total_s = float(ms.sum()) * 1e-3
@@ -262,7 +286,7 @@ def run_ours(args, rank, world, local_rank):
     default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1
     roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
                 traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
-                traffic_source="profiles/r01d_launches.md (ncu --set full, per launch)")
+                traffic_source="profiles/r01e_launches.md (ncu --set full, per launch)")
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline and args.ensemble == 1:
