@@ -101,11 +101,11 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
       bool poll = true;
       if (threadIdx.x > 0) poll = tw != (ipw - 1 + grp->pad_shift[(__float_as_int(spos[ipw - 1].w) >> 28) & 7]) / TILE_M;
       if (poll) {
-        int seen;
+        int seen, spins = 0;
         do {
           asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(tile_done + tw) : "memory");
           if (seen < done_target) __nanosleep(500);
-        } while (seen < done_target);
+        } while (seen < done_target && ++spins < (1 << 22));   // ~2 s: a flag that never comes must not hang the GPU
       }
     }
   }
