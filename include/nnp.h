@@ -107,6 +107,13 @@ int nnp_workspace_set_units(nnp_workspace*, double angstrom_per_length_unit, dou
  * in 2^-32 fixed point (reproducible).  NULL (default) switches it off; the pointer must stay valid while set. */
 int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
 
+/* Small-system front end (the ML/MM regime of PAPER.md lines 108, 140, 154, 164: 14-107
+ * ML atoms, where per-step latency is what counts).  on != 0 (default): a periodic evaluation with at most 256 ML atoms,
+ * box lengths <= 64 Angstrom and no external pair list runs species map, ordering, all-pairs neighbour search in shared
+ * memory and the AEV as ONE kernel (no grid-wide barriers, no cell list); rows, E and F are those of the general path
+ * up to fp32 summation order of the positions' frame.  0: always the general cell-list path. */
+int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
+
 /* External pair list ("The 2026 version adds the internal pair-list built by GROMACS ... as
  * available inputs").  With d_pairs != NULL every later nnp_eval takes its neighbour
  * candidates from this list instead of its own cell search:

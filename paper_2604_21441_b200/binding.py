@@ -16,7 +16,7 @@ NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
     "nnp_model_create", "nnp_model_create_ensemble", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
-    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_eval",
+    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
@@ -69,6 +69,7 @@ def lib():
         L.nnp_workspace_set_virial_output.argtypes = [vp, vp]
         L.nnp_workspace_set_units.argtypes = [vp, C.c_double, C.c_double]
         L.nnp_workspace_set_pair_list.argtypes = [vp, vp, i64]
+        L.nnp_workspace_set_small_path.argtypes = [vp, i32]
         L.nnp_eval.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_eval_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_status.argtypes = [vp]
@@ -133,6 +134,10 @@ def nnp_workspace_set_dense_k(ws, dense):
 
 def nnp_workspace_set_units(ws, angstrom_per_length_unit, energy_units_per_ev):
     return lib().nnp_workspace_set_units(ws, float(angstrom_per_length_unit), float(energy_units_per_ev))
+
+
+def nnp_workspace_set_small_path(ws, on):
+    return lib().nnp_workspace_set_small_path(ws, int(on))
 
 
 def nnp_workspace_set_pair_list(ws, d_pairs, n_pairs):
@@ -281,6 +286,9 @@ class Workspace:
         self._virial = virial
         _check(nnp_workspace_set_virial_output(self.handle, None if virial is None else virial.data_ptr()),
                "nnp_workspace_set_virial_output")
+
+    def set_small_path(self, on):
+        _check(nnp_workspace_set_small_path(self.handle, on), "nnp_workspace_set_small_path")
 
     def set_pair_list(self, pairs):
         """pairs: (n_pairs, 2) int32 cuda tensor of candidate pairs (global atom indices), or None for the cell search."""

@@ -192,6 +192,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
     }
     ws->num_sms = sms;
     ws->prep_cluster = prep_cluster_size();
+    ws->small_path = 1;
     ws->prep_cluster_max = 8192;   // measured: 24 000 atoms run 4 us slower in one cluster than on the cooperative grid
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
@@ -268,6 +269,12 @@ extern "C" int nnp_workspace_set_pair_list(nnp_workspace* ws, const int32_t* d_p
   return NNP_OK;
 }
 
+extern "C" int nnp_workspace_set_small_path(nnp_workspace* ws, int32_t on) {
+  if (!ws) return NNP_ERR_INVALID_ARG;
+  ws->small_path = on ? 1 : 0;
+  return NNP_OK;
+}
+
 extern "C" int nnp_workspace_set_dense_k(nnp_workspace* ws, int32_t dense) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   ws->dense_k = dense ? 1 : 0;
@@ -310,10 +317,17 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
     d_pos = ws->pos_scaled;
     if (pbc) { for (int i = 0; i < 9; ++i) box_a[i] = (float)((double)box[i] * ws->len_scale); box = box_a; }
   }
-  nl += launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
-  prof_mark(ws, 1);
-  nl += launch_aev_forward(ws, n_ml);
-  prof_mark(ws, 2);
+  if (small_front_applicable(ws, box, pbc, n_ml)) {
+    // small periodic ML region: K0-K3 in one kernel (stage profiling books it under "neighbour", AEV forward = 0)
+    nl += launch_small_front(ws, d_pos, d_Z, box, d_ml, n_atoms, n_ml);
+    prof_mark(ws, 1);
+    prof_mark(ws, 2);
+  } else {
+    nl += launch_neighbor_stage(ws, d_pos, d_Z, pbc ? box : unit, pbc ? 1 : 0, d_ml, n_atoms, n_ml);
+    prof_mark(ws, 1);
+    nl += launch_aev_forward(ws, n_ml);
+    prof_mark(ws, 2);
+  }
   nl += (ws->mlp_mode == NNP_MLP_FP32_SIMT) ? launch_mlp_simt(ws, n_ml) : launch_mlp_tc(ws, n_ml);
   prof_mark(ws, 3);
   if (n_ml <= 0) prof_mark(ws, 4);

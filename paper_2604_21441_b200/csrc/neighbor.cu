@@ -13,16 +13,12 @@
 #include <cooperative_groups.h>
 #include <algorithm>
 #include "nnp_internal.h"
+#include "groups.cuh"
+#include "neighbor_common.cuh"
 
 namespace cg = cooperative_groups;
 
 namespace nnp {
-
-__device__ __forceinline__ unsigned lanemask_lt() {
-  unsigned m;
-  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
-  return m;
-}
 
 // ---------------------------------------------------------------- grid setup (1 block)
 __device__ void d_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, float Ly, float Lz, float Rcr,
@@ -174,61 +170,9 @@ __device__ void d_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
   if (threadIdx.x == 0) { bstart[n] = total; gs[S] = total; if (total != n_ml) atomicOr(flags, FLAG_ARG); }
   __syncthreads();
   __shared__ int pshift[MAX_S];
-  if (threadIdx.x == 0) {
-    int rows = 0, nt = 0, cnt[MAX_S];
-    for (int q = 0; q < MAX_S; ++q) {
-      cnt[q] = (q < S) ? gs[q + 1] - gs[q] : 0;
-      grp->count[q] = cnt[q];
-      grp->start[q] = (q < S) ? gs[q] : n_ml;
-      pshift[q] = rows - ((q < S) ? gs[q] : 0);
-      grp->pad_shift[q] = pshift[q];
-      tb[q] = nt;
-      int t = (cnt[q] + TILE_M - 1) / TILE_M;
-      nt += t; rows += t * TILE_M;
-    }
-    grp->start[MAX_S] = n_ml;
-    tb[MAX_S] = nt;
-    grp->n_tiles = min(nt, max_tiles);
-    grp->n_rows = rows;
-    if (nt > max_tiles) atomicOr(flags, FLAG_CAP);
-    // compacted AEV column blocks: a radial block holds species (2b, 2b+1), an angular block one pair p(s1,s2)
-    const int nRB = (S + 1) / 2;
-    int nb = 0;
-    for (int b = 0; b < nRB; ++b) {
-      bool on = dense_k || cnt[2 * b] > 0 || (2 * b + 1 < S && cnt[2 * b + 1] > 0);
-      grp->cpos[b] = on ? nb : -1;
-      if (on) grp->blkmap[nb++] = b;
-    }
-    int p = 0;
-    for (int s1 = 0; s1 < S; ++s1)
-      for (int s2 = s1; s2 < S; ++s2, ++p) {
-        bool on = dense_k || (cnt[s1] > 0 && cnt[s2] > 0);
-        grp->cpos[nRB + p] = on ? nb : -1;
-        if (on) grp->blkmap[nb++] = nRB + p;
-      }
-    for (int b = nRB + p; b < MAX_BLK; ++b) grp->cpos[b] = -1;
-    for (int b = nb; b < MAX_BLK; ++b) grp->blkmap[b] = 0;
-    grp->nblk = nb;
-    grp->Kc = nb * BLK;
-    int npres = 0;
-    for (int q = 0; q < MAX_S; ++q) { if (cnt[q] > 0) grp->pres[npres++] = q; }
-    for (int q = npres; q < MAX_S; ++q) grp->pres[q] = 0;
-    grp->npres = npres;
-    unsigned long long key = 1ull << 63;
-    for (int b = 0; b < nb; ++b) key |= 1ull << grp->blkmap[b];
-    grp->colkey = key;
-  }
+  if (threadIdx.x == 0) d_groups(gs, S, n_ml, max_tiles, dense_k, grp, pshift, tb, flags);
   __syncthreads();
-  const int nt = min(tb[MAX_S], max_tiles);
-  for (int t = threadIdx.x; t < nt; t += 1024) {
-    int q = 0;
-    while (q + 1 < MAX_S && t >= tb[q + 1]) ++q;
-    int r = t - tb[q];
-    int cnt = gs[min(q + 1, S)] - gs[min(q, S)];
-    TileInfo ti;
-    ti.slot = q; ti.row0 = pshift[q] + gs[q] + r * TILE_M; ti.nvalid = min(TILE_M, cnt - r * TILE_M); ti.pad = 0;
-    tiles[t] = ti;
-  }
+  d_tiles(gs, pshift, tb, S, max_tiles, tiles);
 }
 
 // ---------------------------------------------------------------- K1b: scatter into slot-major cell order
@@ -279,23 +223,6 @@ __device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S, con
 }
 
 // ---------------------------------------------------------------- K2: neighbour rows, one warp per centre
-// minimum-image displacement r_oj - r_oi and its squared length, the pinned fp64 expression of reading #6
-__device__ __forceinline__ double exact_disp(const float* __restrict__ pos, int oi, int oj, const GridInfo* g, double d[3]) {
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    double x = (double)pos[3 * (size_t)oj + a] - (double)pos[3 * (size_t)oi + a];
-    if (g->pbc) x -= g->L_d[a] * rint(x / g->L_d[a]);
-    d[a] = x;
-  }
-  return __fma_rn(d[2], d[2], __fma_rn(d[1], d[1], __dmul_rn(d[0], d[0])));
-}
-__device__ __noinline__ double exact_d2(const float* __restrict__ pos, int oi, int oj, const GridInfo* g) {
-  double d[3];
-  return exact_disp(pos, oi, oj, g, d);
-}
-
-constexpr float GUARD_BAND = 2.0e-3f;  // Angstrom^2; >> fp32 error of d2 (~1e-5), reading #6
-
 constexpr int NB_CAP = 1024;            // candidates staged in shared memory per chunk
 constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of one centre cell
 

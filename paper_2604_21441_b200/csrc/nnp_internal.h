@@ -120,6 +120,7 @@ struct nnp_workspace {
   int prep_cluster_max;      // largest n_ml the single-cluster variant takes
   int mlp_mode;
   int dense_k;               // 1: materialise every column block (no structural-zero compaction)
+  int small_path;            // 1 (default): small periodic ML regions take the single-kernel front end (small.cu)
   int64_t max_rows;          // padded AEV rows
   int max_tiles;
   // last evaluation
@@ -190,6 +191,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
 int prep_cluster_size();
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);
+bool small_front_applicable(const nnp_workspace* ws, const float* box, int pbc, int64_t n_ml);
+int launch_small_front(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, const int32_t* d_ml,
+                       int64_t n_atoms, int64_t n_ml);
 int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,

@@ -572,3 +572,38 @@ def test_external_pair_list(k, pbc):
     ws.set_pair_list(None)
     E3, F3 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], pbc, ml)
     assert E3 == E0 and np.array_equal(F3, F0)
+
+
+# ------------------------------------------------------------------ small-system front end
+@pytest.mark.parametrize("k,layout", [(0, "A"), (4, "A"), (4, "B")])
+def test_small_path_and_general_path(k, layout):
+    """<= 256 ML atoms in a periodic box take the single-kernel front end by default; the general cell-list path must
+    give the same rows (bit-exact, both against the oracle) and the same E, F up to fp32 rounding of the positions' frame."""
+    cfg = gen.get_config(k, layout=layout) if k == 4 else gen.get_config(k)
+    ml = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    n_ml = n if ml is None else len(ml)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, want_aev=True)
+    m, ws = make(cfg)
+    out = {}
+    for on in (1, 0):
+        ws.set_small_path(on)
+        E, F = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+        assert ws.launches() == (5 if on else 7)
+        check_lists(ws, cfg, cfg["pos"], n_ml, ml)
+        G = ws.aev(n_ml).astype(np.float64)
+        assert np.all(np.abs(G - ref["aev"]) <= 2e-5 * (1 + np.abs(ref["aev"]))), np.abs(G - ref["aev"]).max()
+        check_EF(E, F, ref, n_ml, rows=ml)
+        E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+        assert E2 == E and np.array_equal(F2, F)
+        out[on] = (E, F)
+    assert abs(out[1][0] - out[0][0]) / n_ml < 1e-6 and np.abs(out[1][1] - out[0][1]).max() < 1e-4
+    # atoms shifted by whole box vectors: same rows
+    ws.set_small_path(1)
+    shift = np.random.default_rng(3).integers(-2, 3, size=cfg["pos"].shape).astype(np.float32)
+    pos2 = (cfg["pos"] + shift * np.array([cfg["box"][0], cfg["box"][4], cfg["box"][8]], dtype=np.float32)).astype(np.float32)
+    ref2 = oracle.evaluate(om, pos2, cfg["Z"], cfg["box"], 1, ml)
+    E3, F3 = run_gpu(ws, pos2, cfg["Z"], cfg["box"], 1, ml)
+    check_lists(ws, cfg, pos2, n_ml, ml)
+    check_EF(E3, F3, ref2, n_ml, rows=ml)
