@@ -59,6 +59,7 @@ struct TcWorkspace {
   unsigned long long* key; // [2]: column-set key the images were packed for / scratch
   TcPackAll* d_pall;       // device copy of the layer-1 image pointer table
   int* done;               // [max_tiles] ensemble hand-over: members of a tile already accumulated (reset every call)
+  uint32_t* cscr;          // [num_sms][TC_CSCR_WORDS] packed CELU' of the tile in flight, per CTA
   int num_sms;
   int smem_bytes[2];
 };
@@ -255,16 +256,17 @@ constexpr int TC_NPART = TC_EPI_WARPS / 4;            // warps sharing a lane qu
 constexpr int TC_THREADS = (TC_EPI_WARPS + 2) * 32;   // + weight producer warp + MMA issuer warp
 constexpr uint32_t TC_PANEL = 16384;                  // 128 rows x 128 B
 constexpr uint32_t TC_LO = 4 * TC_PANEL;              // lo half of the A buffer
-constexpr uint32_t TC_ACC = 256;                      // TMEM column of the 256-column accumulator
-constexpr uint32_t TC_P1 = 0, TC_P2 = 128;            // TMEM columns of the packed CELU' of layers 1 and 2
+constexpr uint32_t TC_ACCW = 256;                     // TMEM: two 256-column accumulators (columns 0 and 256), used alternately
+constexpr int TC_CW1 = 128, TC_CW2 = 128;             // words per row of the packed CELU' of layers 1 and 2 (global scratch)
+constexpr int TC_CSCR_WORDS = (TC_CW1 + TC_CW2) * 128;  // per CTA
 
 template <int NPASS> struct TcCfg {
   static constexpr int NH = (NPASS == 3) ? 2 : 1;
   static constexpr int NST = (NPASS == 3) ? 3 : 4;
   static constexpr uint32_t ABUF = NH * 4 * TC_PANEL;
   static constexpr uint32_t STAGE = 2 * TC_PANEL;               // one half-block: <= 256 rows x 128 B
-  static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], a_ready, acc_full
-  static constexpr uint32_t TPTR = BARS + (2 * NST + 2) * 8;
+  static constexpr uint32_t BARS = ABUF + NST * STAGE;          // full[NST], empty[NST], panel[4], acc_full
+  static constexpr uint32_t TPTR = BARS + (2 * NST + 5) * 8;
   static constexpr uint32_t EPART = TPTR + 16;
   static constexpr uint32_t TOTAL = EPART + (TC_NPART - 1) * 128 * 4;
 };
@@ -320,20 +322,20 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
          const TcPackAll* __restrict__ w1all, const GroupInfo* __restrict__ grp,
          const TileInfo* __restrict__ tiles, const float* __restrict__ aev, float* __restrict__ daev,
          float* __restrict__ e_atom, unsigned long long* __restrict__ key, int* __restrict__ done, int n_members,
-         float escale) {
+         float escale, uint32_t* cscr) {
   using C = TcCfg<NPASS>;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   const uint32_t abuf = sbase, stage0 = sbase + C::ABUF;
   const uint32_t bar_full = sbase + C::BARS, bar_empty = bar_full + 8 * C::NST;
-  const uint32_t bar_aready = bar_empty + 8 * C::NST, bar_acc = bar_aready + 8;
+  const uint32_t bar_panel = bar_empty + 8 * C::NST, bar_acc = bar_panel + 32;
   volatile uint32_t* tptr = reinterpret_cast<volatile uint32_t*>(smem + C::TPTR);
   float* e_part = reinterpret_cast<float*>(smem + C::EPART);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < C::NST; ++i) { mbar_init(bar_full + 8 * i, 1); mbar_init(bar_empty + 8 * i, 1); }
-    mbar_init(bar_aready, TC_EPI_WARPS * 32);
+    for (int i = 0; i < 4; ++i) mbar_init(bar_panel + 8 * i, TC_EPI_WARPS * 32);
     mbar_init(bar_acc, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -404,7 +406,7 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
     // built once per block and advanced by 32 B (+2 in the address field) per k-step: the issue loop must stay a
     // handful of instructions per MMA, or the single issuing warp, not the tensor core, paces the GEMM. =====
     {
-      int s = 0; uint32_t ph = 0, aph = 0;
+      int s = 0; uint32_t ph = 0, pph = 0, buf = 1;
       for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
         int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
         TcRound rd[TC_MAX_ROUNDS];
@@ -413,13 +415,15 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
         for (int ir = 0; ir < nrd; ++ir) {
           const int N = rd[ir].N, K = rd[ir].K, c0 = rd[ir].c0, c1 = rd[ir].c1, p0 = rd[ir].p0, p1 = rd[ir].p1;
           const bool acc_first = rd[ir].acc_first != 0;
-          mbar_wait(bar_aready, aph); aph ^= 1;   // A operand in place, accumulator columns drained
-          tc_fence_after();
+          if (!acc_first) buf ^= 1;               // a new accumulation takes the other accumulator
           const int ch = tc_chunk(N);
           for (int c = c0; c < c1; ++c) {
             const int rows = min(ch, N - c * ch);
-            const uint32_t idesc = tc_idesc(rows), d = tmem + TC_ACC + (uint32_t)((c - c0) * ch);
+            const uint32_t idesc = tc_idesc(rows), d = tmem + buf * TC_ACCW;
             for (int p = p0; p < p1; ++p) {
+              // the previous epilogue hands the A operand over panel by panel (every panel barrier completes once a round)
+              mbar_wait(bar_panel + 8 * (p - p0), pph);
+              tc_fence_after();
               const int nks = min(4, (K - p * 64) >> 4);
               const uint32_t a0 = abuf + (uint32_t)(p - p0) * TC_PANEL;
               {   // B_hi block: A_hi * B_hi (+ A_lo * B_hi for the split)
@@ -454,6 +458,7 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             }
           }
           tc_commit_elect(bar_acc);                // accumulator complete (and the A operand no longer read)
+          pph ^= 1;
         }
       }
     }
@@ -462,13 +467,27 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
     // 16-column chunks round-robin =====
     const int q = warp & 3, part = warp >> 2, row = q * 32 + lane;
     const uint32_t tlane = tmem + ((uint32_t)(q * 32) << 16);
-    uint32_t fph = 0;
+    uint32_t fph = 0, buf = 1;
     int tl = 0;   // timeline slot (block 0, thread 0 only): even = operand handed to the MMA warp, odd = accumulator back
-    auto signal_and_wait = [&]() {
+    // Hand-over protocol.  The A operand goes to the MMA warp PANEL BY PANEL (64 columns): every thread arrives once a
+    // round on each of the four panel barriers, as soon as its share of the panel is in shared memory, so the MMAs of
+    // the next GEMM start on panel 0 while this epilogue is still producing panels 1-3.  That GEMM accumulates into the
+    // OTHER 256-column TMEM accumulator (the epilogue is still reading this one); CELU' therefore waits for the
+    // backward pass in a per-CTA global scratch (L2-resident) instead of TMEM.
+    auto arrive_panel = [&](int i) {
+      tc_fence_before();
+      fence_proxy_async();
+      if (i == 3 && blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
+      mbar_arrive(bar_panel + 8 * i);
+    };
+    auto arrive_all = [&]() {
       tc_fence_before();
       fence_proxy_async();
       if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
-      mbar_arrive(bar_aready);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) mbar_arrive(bar_panel + 8 * i);
+    };
+    auto wait_acc = [&]() {
       // ONE thread polls the mbarrier; the other 511 sleep in a hardware named barrier.  (512 threads spinning on
       // try_wait flood the shared-memory pipe that feeds the tensor core's operand reads.)
       if (threadIdx.x == 0) mbar_wait(bar_acc, fph);
@@ -477,6 +496,8 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       tc_fence_after();
       if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
     };
+    uint32_t* const cs1 = cscr + (size_t)blockIdx.x * TC_CSCR_WORDS;   // CELU' of layer 1: [chunk j][2][128 rows][4 words]
+    uint32_t* const cs2 = cs1 + TC_CW1 * 128;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
       const Net& net = all_nets[mem].net[ti.slot];
@@ -488,41 +509,51 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       for (int p0 = 0; p0 < np; p0 += 4) {
         const int k0 = p0 * 64, kw = min(Kc, k0 + 256) - k0, n16 = kw >> 3;
         constexpr int NT = TC_EPI_WARPS * 32;
-        for (int base = threadIdx.x; base < 128 * n16; base += 4 * NT) {
+        static_assert(NT == 512, "two batches of two 1024-item panels");
+        // panel-major: a 64-column panel is 128 rows x 8 chunks of 8 floats = 1024 items, two per thread; a batch of two
+        // panels keeps four loads per thread in flight, and each panel is handed to the MMA warp as soon as it is in place
+#pragma unroll 1
+        for (int pb = 0; pb < 4; pb += 2) {
           float4 x0[4], x1[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {   // all loads of the batch in flight before the first use
-            const int idx = base + u * NT, r = idx / n16, chn = idx - r * n16;
+            const int within = (int)threadIdx.x + (u & 1) * NT, r = within >> 3, chn = (pb + (u >> 1)) * 8 + (within & 7);
             x0[u] = make_float4(0.f, 0.f, 0.f, 0.f); x1[u] = x0[u];
-            if (idx < 128 * n16 && r < ti.nvalid) {
+            if (chn < n16 && r < ti.nvalid) {
               const float4* src = reinterpret_cast<const float4*>(aev + (size_t)(ti.row0 + r) * Kc + k0 + chn * 8);
               x0[u] = __ldg(src); x1[u] = __ldg(src + 1);
             }
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int idx = base + u * NT, r = idx / n16, chn = idx - r * n16;
-            if (idx >= 128 * n16) break;
-            uint32_t hi[4], lo[4];
-            split2(x0[u].x, x0[u].y, hi[0], lo[0]); split2(x0[u].z, x0[u].w, hi[1], lo[1]);
-            split2(x1[u].x, x1[u].y, hi[2], lo[2]); split2(x1[u].z, x1[u].w, hi[3], lo[3]);
-            const uint32_t dst = abuf + (uint32_t)(chn >> 3) * TC_PANEL + (uint32_t)r * 128u + (uint32_t)(((chn & 7) ^ (r & 7)) << 4);
-            sts128(dst, hi[0], hi[1], hi[2], hi[3]);
-            if (NPASS == 3) sts128(dst + TC_LO, lo[0], lo[1], lo[2], lo[3]);
+            const int within = (int)threadIdx.x + (u & 1) * NT, r = within >> 3, chn = (pb + (u >> 1)) * 8 + (within & 7);
+            if (chn < n16) {
+              uint32_t hi[4], lo[4];
+              split2(x0[u].x, x0[u].y, hi[0], lo[0]); split2(x0[u].z, x0[u].w, hi[1], lo[1]);
+              split2(x1[u].x, x1[u].y, hi[2], lo[2]); split2(x1[u].z, x1[u].w, hi[3], lo[3]);
+              const uint32_t dst = abuf + (uint32_t)(chn >> 3) * TC_PANEL + (uint32_t)r * 128u + (uint32_t)(((chn & 7) ^ (r & 7)) << 4);
+              sts128(dst, hi[0], hi[1], hi[2], hi[3]);
+              if (NPASS == 3) sts128(dst + TC_LO, lo[0], lo[1], lo[2], lo[3]);
+            }
+            if (u & 1) arrive_panel(pb + (u >> 1));
           }
         }
-        signal_and_wait();
+        if (p0 == 0) buf ^= 1;   // mirrors the MMA warp: a new accumulation takes the other accumulator
+        wait_acc();
       }
-      // ---- forward hidden layers 1, 2: h = CELU(z + b) -> A operand of the next layer; CELU' packed into TMEM
+      // ---- forward hidden layers 1, 2: h = CELU(z + b) -> A operand of the next layer; CELU' packed to the scratch
 #pragma unroll 1
       for (int l = 1; l <= 2; ++l) {
         const int N = (l == 1) ? tn.N1 : tn.N2;
         const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[l - 1]);
-        const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
+        uint32_t* const cs = (l == 1) ? cs1 : cs2;
+        const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
-        for (int j = part; j * 16 < N; j += TC_NPART) {
+        for (int pi4 = 0; pi4 < 4; ++pi4) {
+          const int j = part + TC_NPART * pi4;
+          if (j * 16 < N) {
           uint32_t v[16], hi[8], lo[8], cp[8];
-          tmem_ld16(tlane + TC_ACC + j * 16, v);
+          tmem_ld16(tacc + j * 16, v);
           float4 bv[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) bv[i] = __ldg(bias4 + j * 4 + i);
@@ -537,11 +568,14 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             cp[i >> 1] = pack_c(e0, e1);   // CELU'(z) = exp(min(z, 0) / alpha): ex2(0) = 1 exactly, no select needed
             split2(h0, h1, hi[i >> 1], lo[i >> 1]);
           }
-          tmem_st8(tlane + pcol + j * 8, cp);
+          __stcg(reinterpret_cast<uint4*>(cs + ((size_t)(2 * j) * 128 + row) * 4), make_uint4(cp[0], cp[1], cp[2], cp[3]));
+          __stcg(reinterpret_cast<uint4*>(cs + ((size_t)(2 * j + 1) * 128 + row) * 4), make_uint4(cp[4], cp[5], cp[6], cp[7]));
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
+          }
+          arrive_panel(pi4);
         }
-        tmem_wait_st();
-        signal_and_wait();
+        buf ^= 1;
+        wait_acc();
       }
       // ---- layer 3 + output layer: E_i = h3 . w4 + b4;  dl3 = w4 * CELU'(z3) -> A operand of B3
       {
@@ -549,10 +583,13 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
         const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[2]);
         const float4* __restrict__ w44 = reinterpret_cast<const float4*>(net.W[nl - 1]);
         float e = 0.f;
+        const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
-        for (int j = part; j * 16 < tn.N3; j += TC_NPART) {
+        for (int pi4 = 0; pi4 < 4; ++pi4) {
+          const int j = part + TC_NPART * pi4;
+          if (j * 16 < tn.N3) {
           uint32_t v[16], hi[8], lo[8];
-          tmem_ld16(tlane + TC_ACC + j * 16, v);
+          tmem_ld16(tacc + j * 16, v);
           float4 bv[4], wv[4];
 #pragma unroll
           for (int i = 0; i < 4; ++i) { bv[i] = __ldg(bias4 + j * 4 + i); wv[i] = __ldg(w44 + j * 4 + i); }
@@ -569,6 +606,8 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
             split2(escale * wa * e0, escale * wb * e1, hi[i >> 1], lo[i >> 1]);   // e = CELU'(z) (1 for z > 0)
           }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
+          }
+          arrive_panel(pi4);
         }
         if (part > 0) e_part[(part - 1) * 128 + row] = e;
         if (accumulate && threadIdx.x == 0) {   // the previous member of this tile must have finished its updates
@@ -585,37 +624,57 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
           const float ev = valid ? escale * (e + __ldg(net.b[nl - 1])) : 0.f;
           e_atom[ti.row0 + row] = accumulate ? e_atom[ti.row0 + row] + ev : ev;   // ensemble: mean over members
         }
-        signal_and_wait();
+        buf ^= 1;   // (the wait for B3 sits at the top of the backward loop, behind the CELU' prefetch)
       }
-      // ---- backward through layers 2, 1: dl_l = d_l * CELU'(z_l) -> A operand of the next backward GEMM
+      // ---- backward through layers 2, 1: dl_l = d_l * CELU'(z_l) -> A operand of the next backward GEMM.  The packed
+      // CELU' words come back from the scratch one chunk ahead of their use (the first ones while the GEMM still runs).
 #pragma unroll 1
       for (int l = 2; l >= 1; --l) {
         const int N = (l == 1) ? tn.N1 : tn.N2;
-        const uint32_t pcol = (l == 1) ? TC_P1 : TC_P2;
+        const uint32_t* const cs = (l == 1) ? cs1 : cs2;
+        uint4 cn0 = make_uint4(0u, 0u, 0u, 0u), cn1 = cn0;   // this thread wrote these words itself in the forward pass
+        if (part * 16 < N) {
+          cn0 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * part) * 128 + row) * 4));
+          cn1 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * part + 1) * 128 + row) * 4));
+        }
+        wait_acc();   // B3 (l = 2) / B2 (l = 1) complete
+        const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
-        for (int j = part; j * 16 < N; j += TC_NPART) {
-          uint32_t v[16], cp[8], hi[8], lo[8];
-          tmem_ld16(tlane + TC_ACC + j * 16, v);
-          tmem_ld8(tlane + pcol + j * 8, cp);
+        for (int pi4 = 0; pi4 < 4; ++pi4) {
+          const int j = part + TC_NPART * pi4;
+          if (j * 16 < N) {
+          uint32_t v[16], hi[8], lo[8];
+          tmem_ld16(tacc + j * 16, v);
+          const uint32_t cp[8] = {cn0.x, cn0.y, cn0.z, cn0.w, cn1.x, cn1.y, cn1.z, cn1.w};
+          if ((j + TC_NPART) * 16 < N) {
+            cn0 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * (j + TC_NPART)) * 128 + row) * 4));
+            cn1 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * (j + TC_NPART) + 1) * 128 + row) * 4));
+          }
           tmem_wait_ld();
 #pragma unroll
           for (int i = 0; i < 16; i += 2)
             split2(__uint_as_float(v[i]) * unpack_c_lo(cp[i >> 1]), __uint_as_float(v[i + 1]) * unpack_c_hi(cp[i >> 1]),
                    hi[i >> 1], lo[i >> 1]);
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
+          }
+          arrive_panel(pi4);
         }
-        signal_and_wait();
+        buf ^= 1;
       }
+      wait_acc();   // B1, first column chunk
       // ---- B1 rounds: g = dE/dAEV columns [n0, n0 + ncols) -> global (fp32, compacted AEV column order)
       {
         const int nc = tc_nchunks(Kc), ch = tc_chunk(Kc);
         for (int c0 = 0; c0 < nc; ++c0) {
           const int n0 = c0 * ch, ncols = min(Kc, (c0 + 1) * ch) - n0;
           float* __restrict__ dst = daev + daev_off((size_t)(ti.row0 + row), n0, Kc);   // piece-major tile layout
+          const uint32_t tacc = tlane + buf * TC_ACCW;
+          // the A operand (dl1) is unchanged: the MMAs of the next column chunk start now, into the other accumulator
+          if (c0 + 1 < nc) { arrive_all(); buf ^= 1; }
 #pragma unroll 1
           for (int j = part; j * 16 < ncols; j += TC_NPART) {
             uint32_t v[16];
-            tmem_ld16(tlane + TC_ACC + j * 16, v);
+            tmem_ld16(tacc + j * 16, v);
             tmem_wait_ld();
             if (valid) {
 #pragma unroll
@@ -627,9 +686,9 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
               }
             }
           }
-          if (c0 + 1 < nc) signal_and_wait();
+          if (c0 + 1 < nc) wait_acc();
         }
-        // the first round of the next tile re-arms through its own signal_and_wait (program order: loads above done)
+        // the next tile's first round re-arms the panel barriers after its own loads (program order: the reads above are done)
         {   // publish this member's updates of the tile: to the CTA that holds the next member, and (last member) to
             // the AEV backward kernel, whose warps wait for their tile's flag
           __threadfence();
@@ -783,6 +842,7 @@ int tc_workspace_create(nnp_workspace* ws) {
       cudaMalloc(&tw->done, sizeof(int) * (size_t)std::max(ws->max_tiles, 1)) != cudaSuccess)
     return NNP_ERR_CUDA;
   cudaMemset(tw->done, 0, sizeof(int) * (size_t)std::max(ws->max_tiles, 1));
+  if (cudaMalloc(&tw->cscr, sizeof(uint32_t) * (size_t)TC_CSCR_WORDS * tw->num_sms) != cudaSuccess) return NNP_ERR_CUDA;
   return NNP_OK;
 }
 
@@ -797,6 +857,7 @@ void tc_workspace_destroy(nnp_workspace* ws) {
   if (tw->key) cudaFree(tw->key);
   if (tw->d_pall) cudaFree(tw->d_pall);
   if (tw->done) cudaFree(tw->done);
+  if (tw->cscr) cudaFree(tw->cscr);
   cudaGetLastError();
   delete tw;
   ws->tc_ws = nullptr;
@@ -824,10 +885,10 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   const float escale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members
   if (ws->mlp_mode == NNP_MLP_F16X1)
     launch_pdl(pdl, ws->stream, k_mlp_tc<1>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[1], tm->d_nets, tm->d_tabs,
-               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale);
+               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale, tw->cscr);
   else
     launch_pdl(pdl, ws->stream, k_mlp_tc<3>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[0], tm->d_nets, tm->d_tabs,
-               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale);
+               tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale, tw->cscr);
   return 2;
 }
 
