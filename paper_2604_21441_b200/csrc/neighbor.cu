@@ -20,6 +20,37 @@ namespace cg = cooperative_groups;
 
 namespace nnp {
 
+// Cell grid from the extent of the system (thread 0 of the prep kernel; for periodic boxes also the HOST, which passes
+// the result to the kernel by value and saves the set-up phase and one grid-wide barrier -- same doubles, same code).
+__host__ __device__ inline void grid_from_extent(GridInfo* g, int pbc, const double ext[3], const double org[3], float Lx,
+                                                 float Ly, float Lz, double cutoff, int max_cells) {
+  int nc[3];
+  for (int d = 0; d < 3; ++d) {
+    int n = (int)floor(ext[d] / cutoff);
+    if (pbc) { if (n < 3) n = 1; } else { if (n < 1) n = 1; }
+    nc[d] = n;
+  }
+  // respect the workspace's cell capacity: shrink the largest dimension (cells only get bigger)
+  while ((long long)nc[0] * nc[1] * nc[2] > (long long)max_cells) {
+    int d = 0;
+    if (nc[1] > nc[d]) d = 1;
+    if (nc[2] > nc[d]) d = 2;
+    nc[d] -= 1;
+    if (pbc && nc[d] < 3) nc[d] = 1;
+  }
+  for (int d = 0; d < 3; ++d) {
+    double e = ext[d] / nc[d];
+    if (!pbc && e < cutoff) e = cutoff;
+    g->nc[d] = nc[d];
+    g->edge_d[d] = e; g->inv_edge_d[d] = 1.0 / e; g->edge[d] = (float)e;
+    g->origin_d[d] = org[d];
+  }
+  g->L_d[0] = (double)Lx; g->L_d[1] = (double)Ly; g->L_d[2] = (double)Lz;
+  g->L[0] = Lx; g->L[1] = Ly; g->L[2] = Lz;
+  g->ncell = nc[0] * nc[1] * nc[2];
+  g->pbc = pbc;
+}
+
 // ---------------------------------------------------------------- grid setup (1 block)
 __device__ void d_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, float Ly, float Lz, float Rcr,
                              int max_cells, const float* __restrict__ pos, const int32_t* __restrict__ ml,
@@ -54,31 +85,7 @@ __device__ void d_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, flo
     }
   }
   if (threadIdx.x != 0) return;
-  int nc[3];
-  for (int d = 0; d < 3; ++d) {
-    int n = (int)floor(ext[d] / cutoff);
-    if (pbc) { if (n < 3) n = 1; } else { if (n < 1) n = 1; }
-    nc[d] = n;
-  }
-  // respect the workspace's cell capacity: shrink the largest dimension (cells only get bigger)
-  while ((long long)nc[0] * nc[1] * nc[2] > (long long)max_cells) {
-    int d = 0;
-    if (nc[1] > nc[d]) d = 1;
-    if (nc[2] > nc[d]) d = 2;
-    nc[d] -= 1;
-    if (pbc && nc[d] < 3) nc[d] = 1;
-  }
-  for (int d = 0; d < 3; ++d) {
-    double e = ext[d] / nc[d];
-    if (!pbc && e < cutoff) e = cutoff;
-    g->nc[d] = nc[d];
-    g->edge_d[d] = e; g->inv_edge_d[d] = 1.0 / e; g->edge[d] = (float)e;
-    g->origin_d[d] = org[d];
-  }
-  g->L_d[0] = (double)Lx; g->L_d[1] = (double)Ly; g->L_d[2] = (double)Lz;
-  g->L[0] = Lx; g->L[1] = Ly; g->L[2] = Lz;
-  g->ncell = nc[0] * nc[1] * nc[2];
-  g->pbc = pbc;
+  grid_from_extent(g, pbc, ext, org, Lx, Ly, Lz, cutoff, max_cells);
   (void)grp;
 }
 
@@ -381,23 +388,31 @@ struct PrepArgs {
   unsigned long long* facc; int* flags;
   float Lx, Ly, Lz;
   int pbc, n_atoms, n_ml, max_cells, max_tiles, dense_k;
+  int host_grid;   // 1: hg holds the cell grid (periodic boxes: computed on the host), no set-up phase
+  GridInfo hg;
 };
 
 // CLUSTER = true: the whole grid is ONE thread-block cluster (<= 16 CTAs) and the phases are separated by the
 // hardware cluster barrier (~0.2 us) -- these steps are latency-bound, a few SMs are plenty up to ~1e5 atoms.
 // CLUSTER = false: cooperative launch over up to one CTA per SM with grid-wide barriers (larger systems).
 template <bool CLUSTER>
-__global__ void __launch_bounds__(1024, 1) k_prep(PrepArgs a) {
+__global__ void __launch_bounds__(1024, 1) k_prep(const __grid_constant__ PrepArgs a) {
   auto sync_all = [&]() {
     if (CLUSTER) cg::this_cluster().sync(); else cg::this_grid().sync();
   };
   const int S = a.c.S;
-  if (blockIdx.x == 0)
-    d_grid_setup(a.grid, a.groups, a.pbc, a.Lx, a.Ly, a.Lz, a.c.Rcr, a.max_cells, a.pos, a.ml, a.n_ml);
-  sync_all();
+  const GridInfo* gbin = a.grid;
+  if (a.host_grid) {   // binning reads the by-value copy; everybody else reads a.grid after the next barrier
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.grid = a.hg;
+    gbin = &a.hg;
+  } else {
+    if (blockIdx.x == 0)
+      d_grid_setup(a.grid, a.groups, a.pbc, a.Lx, a.Ly, a.Lz, a.c.Rcr, a.max_cells, a.pos, a.ml, a.n_ml);
+    sync_all();
+  }
   const int nbA = (a.n_ml + (int)blockDim.x - 1) / (int)blockDim.x;
   for (int vb = blockIdx.x; vb < nbA; vb += gridDim.x)
-    d_bin(vb, a.c, a.grid, a.pos, a.Z, a.ml, a.n_atoms, a.n_ml, a.tmp4, a.rank, a.cell_count, a.facc, a.flags);
+    d_bin(vb, a.c, gbin, a.pos, a.Z, a.ml, a.n_atoms, a.n_ml, a.tmp4, a.rank, a.cell_count, a.facc, a.flags);
   sync_all();
   if (blockIdx.x == 0)
     d_scan(a.grid, a.cell_count, a.bstart, a.groups, a.tiles, S, a.n_ml, a.max_tiles, a.dense_k, a.flags);
@@ -547,6 +562,12 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.Lx = box[0]; a.Ly = box[4]; a.Lz = box[8];
   a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
   a.dense_k = ws->dense_k;
+  a.host_grid = 0;
+  if (pbc) {   // the cell grid of a periodic box needs no device data
+    const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]}, org[3] = {0.0, 0.0, 0.0};
+    grid_from_extent(&a.hg, 1, ext, org, box[0], box[4], box[8], (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);
+    a.host_grid = 1;
+  }
   void* args[] = {&a};
   if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
     cudaLaunchConfig_t cfg = {};
@@ -575,24 +596,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     return nl + 3;
   }
   if (n_ml > 0) {
-    // one block per cell, guard on ncell inside.  Periodic boxes: the host repeats d_grid_setup's cell-count
-    // arithmetic (same doubles, same shrink loop), so no empty blocks are launched; open boundaries: the extent is
-    // only known on the device, one block per cell of the capacity.
-    int ncell_host = ws->max_cells;
-    if (pbc) {
-      const double cutoff = (double)m->aev.Rcr * (1.0 + 1e-4);
-      const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]};
-      int nc[3];
-      for (int d = 0; d < 3; ++d) { int n = (int)floor(ext[d] / cutoff); if (n < 3) n = 1; nc[d] = n; }
-      while ((long long)nc[0] * nc[1] * nc[2] > (long long)ws->max_cells) {
-        int d = 0;
-        if (nc[1] > nc[d]) d = 1;
-        if (nc[2] > nc[d]) d = 2;
-        nc[d] -= 1;
-        if (nc[d] < 3) nc[d] = 1;
-      }
-      ncell_host = nc[0] * nc[1] * nc[2];
-    }
+    // one block per cell, guard on ncell inside.  Periodic boxes: the host knows the cell count; open boundaries: the
+    // extent is only known on the device, one block per cell of the capacity.
+    const int ncell_host = a.host_grid ? a.hg.ncell : ws->max_cells;
     // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
     const int ysplit = (n_ml <= 2048) ? 8 : 1;
     launch_pdl(!ws->profiling, st, k_neighbors, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
