@@ -9,7 +9,9 @@
 // (AEV tile, then each layer's activations / deltas) lives in shared memory in the canonical K-major
 // SWIZZLE_128B layout and is rewritten in place by the epilogue warps; the B operand (weights) is streamed from
 // L2 by the bulk-copy engine (cp.async.bulk, UBLKCP) through an mbarrier ring from images pre-tiled in exactly the
-// shared-memory layout.  CELU' of layers 1-2 waits for the backward pass in TMEM, packed to 16 bits.
+// shared-memory layout.  The operand is handed to the MMA warp panel by panel (64 columns), so a GEMM runs while the
+// epilogue that feeds it is still at work; consecutive GEMMs alternate between two 256-column TMEM accumulators, and
+// CELU' of layers 1-2 (packed to 16 bits) waits for the backward pass in a per-CTA, L2-resident global scratch.
 //
 // Arithmetic (NNP_MLP_F16X3): every operand x is split x = hi + lo with hi = fp16(x), lo = fp16(x - hi) and the
 // product is hi*hi + lo*hi + hi*lo (three MMAs, fp32 accumulate): ~2^-21 relative operand error, i.e. fp32-grade
@@ -148,31 +150,12 @@ __device__ __forceinline__ uint64_t tc_desc(uint32_t saddr) {
 __device__ __forceinline__ uint32_t tc_idesc(int N) { return (1u << 4) | ((uint32_t)(N >> 3) << 17) | (8u << 24); }
 
 #define TC_R8(v, o) "=r"(v[o]), "=r"(v[o + 1]), "=r"(v[o + 2]), "=r"(v[o + 3]), "=r"(v[o + 4]), "=r"(v[o + 5]), "=r"(v[o + 6]), "=r"(v[o + 7])
-#define TC_W8(v, o) "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]), "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), "r"(v[o + 7])
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* v) {  // 32 lanes x 32 columns: lane = thread
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,"
-      "%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-      : TC_R8(v, 0), TC_R8(v, 8), TC_R8(v, 16), TC_R8(v, 24) : "r"(taddr) : "memory");
-}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
       : TC_R8(v, 0), TC_R8(v, 8) : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
-      TC_W8(v, 0), TC_W8(v, 8) : "memory");
-}
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];" : TC_R8(v, 0) : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), TC_W8(v, 0) : "memory");
-}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }

@@ -447,41 +447,61 @@ __device__ __forceinline__ int ml_local(const int32_t* __restrict__ ml, int n_ml
   return (n_ml > 0 && ml[lo] == gidx) ? lo : -1;
 }
 
-// one thread per candidate pair
+// one thread per candidate pair.  Like the cell sweep, the pair is decided in fp32 from the cell-local coordinates
+// (displacement = local_j - local_i + cell offset * edge, the form the AEV kernels rebuild) and only a pair inside a
+// guard band of the cut-off goes through the pinned fp64 predicate: no fp64 division for > 99 % of the candidates.
 __global__ void __launch_bounds__(256)
-k_pair_fill(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const int* __restrict__ inv,
-            const float* __restrict__ pos, const int32_t* __restrict__ ml, int n_ml, const int32_t* __restrict__ pairs,
-            long long n_pairs, int rcap, uint32_t* __restrict__ nbrR, int* __restrict__ cntR, int* __restrict__ flags) {
+k_pair_fill(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const int* __restrict__ scell,
+            const int* __restrict__ inv, const float* __restrict__ pos, const int32_t* __restrict__ ml, int n_ml,
+            const int32_t* __restrict__ pairs, long long n_pairs, int rcap, uint32_t* __restrict__ nbrR,
+            int* __restrict__ cntR, int* __restrict__ flags) {
   const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n_pairs) return;
   const int gi = pairs[2 * p], gj = pairs[2 * p + 1];
   const int ai = ml_local(ml, n_ml, gi), aj = ml_local(ml, n_ml, gj);
   if (ai < 0 || aj < 0) return;             // a pair with a non-ML end does not feed the AEV
   if (ai == aj) { atomicOr(flags, FLAG_ARG); return; }
-  double d[3];
-  const double e2 = exact_disp(pos, gi, gj, g, d);
-  if (!(e2 <= c.Rcr2_d)) return;
-  if (e2 == 0.0) atomicOr(flags, FLAG_COINCIDENT);
   const int ip = inv[ai], jp = inv[aj];
   const float4 pi = spos[ip], pj = spos[jp];
-  // rows store the neighbour's cell offset: displacement = (local_j - local_i) + off * edge  (aev_common.cuh)
+  const int ci = scell[ip], cj = scell[jp];
+  const int nc[3] = {g->nc[0], g->nc[1], g->nc[2]};
+  const int ic[3] = {ci / (nc[1] * nc[2]), (ci / nc[2]) % nc[1], ci % nc[2]};
+  const int jc[3] = {cj / (nc[1] * nc[2]), (cj / nc[2]) % nc[1], cj % nc[2]};
   const float li[3] = {pi.x, pi.y, pi.z}, lj[3] = {pj.x, pj.y, pj.z};
-  uint32_t ci = 0u, cj = 0u;
+  float dd[3];
+  uint32_t code_i = 0u, code_j = 0u;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    const int off = (int)rint((d[a] - ((double)lj[a] - (double)li[a])) * g->inv_edge_d[a]);
-    if (off < -1 || off > 1) { atomicOr(flags, FLAG_ARG); return; }
-    ci |= (uint32_t)(off + 1) << (2 * a);
-    cj |= (uint32_t)(1 - off) << (2 * a);
+    const float e = g->edge[a];
+    float dl = lj[a] - li[a];
+    int off;
+    if (nc[a] == 1) {
+      off = g->pbc ? -(int)rintf(dl / e) : 0;      // one cell: the minimum image of the pair
+    } else {
+      off = jc[a] - ic[a];
+      if (g->pbc) { if (off == nc[a] - 1) off = -1; else if (off == 1 - nc[a]) off = 1; }
+      if (off < -1 || off > 1) return;             // two cells apart: farther than the cut-off (edge >= Rcr)
+    }
+    dd[a] = dl + (float)off * e;
+    code_i |= (uint32_t)(off + 1) << (2 * a);
+    code_j |= (uint32_t)(1 - off) << (2 * a);
   }
+  const float d2 = fmaf(dd[2], dd[2], fmaf(dd[1], dd[1], dd[0] * dd[0]));
+  bool in = d2 < c.Rcr2 - GUARD_BAND;
+  if (fabsf(d2 - c.Rcr2) <= GUARD_BAND || d2 < 1e-6f) {
+    const double e2 = exact_d2(pos, gi, gj, g);
+    if (fabsf(d2 - c.Rcr2) <= GUARD_BAND) in = e2 <= c.Rcr2_d;
+    if (e2 == 0.0) atomicOr(flags, FLAG_COINCIDENT);
+  }
+  if (!in) return;
   const int qi = atomicAdd(&cntR[ip], 1), qj = atomicAdd(&cntR[jp], 1);
-  if (qi < rcap) nbrR[(size_t)ip * rcap + qi] = (uint32_t)jp | (ci << JBITS);
-  if (qj < rcap) nbrR[(size_t)jp * rcap + qj] = (uint32_t)ip | (cj << JBITS);
+  if (qi < rcap) nbrR[(size_t)ip * rcap + qi] = (uint32_t)jp | (code_i << JBITS);
+  if (qj < rcap) nbrR[(size_t)jp * rcap + qj] = (uint32_t)ip | (code_j << JBITS);
   if (qi >= rcap || qj >= rcap) atomicOr(flags, FLAG_CAP);
 }
 
 // one warp per centre: order the row by sorted index (ranking by counting; a neighbour appears once), then the angular
-// subset by the pinned predicate, in row order
+// subset (fp32 decision on the row's own displacement, pinned fp64 predicate inside the guard band), in row order
 __global__ void __launch_bounds__(256)
 k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const float* __restrict__ pos,
             const int32_t* __restrict__ ml, int n_ml, int rcap, int acap, uint32_t* __restrict__ nbrR,
@@ -494,21 +514,21 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
   uint32_t* row = nbrR + (size_t)ip * rcap;
   for (int q = lane; q < n; q += 32) raw[w][q] = row[q];
   __syncwarp();
-  int dup = 0;
+  // keys below position q count with <=, keys above with <: a permutation even for a (faulty) repeated pair
   for (int q = lane; q < n; q += 32) {
     const uint32_t e = raw[w][q], key = e & JMASK;
     int rank = 0;
-    for (int o = 0; o < n; ++o) {
-      const uint32_t ko = raw[w][o] & JMASK;
-      rank += (ko < key || (ko == key && o < q)) ? 1 : 0;   // a permutation even for a (faulty) repeated pair
-      dup |= (ko == key && o != q) ? 1 : 0;
-    }
+    for (int o = 0; o < q; ++o) rank += ((raw[w][o] & JMASK) <= key) ? 1 : 0;
+    for (int o = q + 1; o < n; ++o) rank += ((raw[w][o] & JMASK) < key) ? 1 : 0;
     srt[w][rank] = e;
   }
-  if (dup) atomicOr(flags, FLAG_ARG);   // a pair listed twice
   __syncwarp();
-  const int a_i = __float_as_int(spos[ip].w) & 0x0fffffff;
-  const int o_i = ml ? ml[a_i] : a_i;
+  int dup = 0;   // a pair listed twice shows up as equal neighbours in the ordered row
+  for (int q = lane + 1; q < n; q += 32) dup |= ((srt[w][q] & JMASK) == (srt[w][q - 1] & JMASK)) ? 1 : 0;
+  if (dup) atomicOr(flags, FLAG_ARG);
+  const float4 pi = spos[ip];
+  const int a_i = __float_as_int(pi.w) & 0x0fffffff;
+  const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
   int nA = 0;
   for (int q0 = 0; q0 < n; q0 += 32) {
     const int q = q0 + lane;
@@ -516,8 +536,17 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
     if (q < n) {
       const uint32_t e = srt[w][q];
       row[q] = e;
-      const int a_j = __float_as_int(spos[e & JMASK].w) & 0x0fffffff;
-      inA = exact_d2(pos, o_i, ml ? ml[a_j] : a_j, g) <= c.Rca2_d;
+      const float4 pj = spos[e & JMASK];
+      const int oc = (int)(e >> JBITS);
+      const float dx = (pj.x - pi.x) + (float)((oc & 3) - 1) * ex;
+      const float dy = (pj.y - pi.y) + (float)(((oc >> 2) & 3) - 1) * ey;
+      const float dz = (pj.z - pi.z) + (float)(((oc >> 4) & 3) - 1) * ez;
+      const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+      inA = d2 < c.Rca2 - GUARD_BAND;
+      if (fabsf(d2 - c.Rca2) <= GUARD_BAND) {
+        const int a_j = __float_as_int(pj.w) & 0x0fffffff;
+        inA = exact_d2(pos, ml ? ml[a_i] : a_i, ml ? ml[a_j] : a_j, g) <= c.Rca2_d;
+      }
     }
     const unsigned m = __ballot_sync(0xffffffffu, inA);
     const int pA = nA + __popc(m & lanemask_lt());
@@ -588,7 +617,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     // external candidate pairs instead of the cell sweep (plain launches: fully ordered behind k_prep)
     k_pair_index<<<(unsigned)((n_ml + 255) / 256), 256, 0, st>>>(ws->spos, (int)n_ml, ws->rank, ws->cntR);
     if (ws->n_ext_pairs > 0)
-      k_pair_fill<<<(unsigned)((ws->n_ext_pairs + 255) / 256), 256, 0, st>>>(m->aev, ws->grid, ws->spos, ws->rank, d_pos, d_ml,
+      k_pair_fill<<<(unsigned)((ws->n_ext_pairs + 255) / 256), 256, 0, st>>>(m->aev, ws->grid, ws->spos, ws->scell, ws->rank, d_pos, d_ml,
                                                                             (int)n_ml, ws->ext_pairs, (long long)ws->n_ext_pairs,
                                                                             ws->rcap, ws->nbrR, ws->cntR, ws->flags);
     k_pair_rows<<<(unsigned)((n_ml + 7) / 8), 256, 0, st>>>(m->aev, ws->grid, ws->spos, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap,
