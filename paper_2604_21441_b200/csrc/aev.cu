@@ -12,16 +12,16 @@
 
 namespace nnp {
 
-__global__ void __launch_bounds__(AEV_WARPS * 32, 4)
+__global__ void __launch_bounds__(AEV_FWD_WARPS * 32, 32 / AEV_FWD_WARPS)
 k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
               const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
               float* __restrict__ aev) {
-  __shared__ WarpEnv env[AEV_WARPS];
+  __shared__ WarpEnv env[AEV_FWD_WARPS];
   pdl_trigger();
   pdl_wait();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int ip = blockIdx.x * AEV_WARPS + w;
+  const int ip = blockIdx.x * AEV_FWD_WARPS + w;
   if (ip >= n_ml) return;
   aev_forward_centre(c, g, grp, spos, nbrR + (size_t)ip * rcap, nbrA + (size_t)ip * acap, cntR[ip], cntA[ip], ip, aev, lane,
                      env[w]);
@@ -30,8 +30,8 @@ k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __res
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml) {
   if (n_ml <= 0) return 0;
   const nnp_model* m = ws->model;
-  const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
-  launch_pdl(!ws->profiling, ws->stream, k_aev_forward, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid, ws->groups,
+  const int nb = (int)((n_ml + AEV_FWD_WARPS - 1) / AEV_FWD_WARPS);
+  launch_pdl(!ws->profiling, ws->stream, k_aev_forward, dim3(nb), dim3(AEV_FWD_WARPS * 32), 0, m->aev, ws->grid, ws->groups,
              ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->aev);
   return 1;
 }

@@ -69,7 +69,7 @@ __device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, 
 }
 
 template <bool VIRIAL>
-__global__ void __launch_bounds__(AEV_WARPS * 32, 4)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 32 / AEV_WARPS)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
