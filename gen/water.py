@@ -100,3 +100,21 @@ def perturbed_positions(pos64, seed, T, sigma=0.01):
     rng = np.random.default_rng(seed)
     eps = rng.normal(0.0, sigma, size=(T,) + pos64.shape)
     return (pos64[None] + eps).astype(np.float32)
+
+
+def sheared_water_box(cfg, bx, cx, cy):
+    """Triclinic stand-in (GROMACS lower-triangular box): the molecules of an orthorhombic
+    water configuration `cfg` are moved with their oxygen to the same FRACTIONAL position of the box with rows
+    a = (Lx, 0, 0), b = (bx*Lx, Ly, 0), c = (cx*Lx, cy*Ly, Lz) (bx, cx, cy in box-length units, |.| <= 0.5); molecules stay
+    rigid.  Returns (pos float32 (N,3), box float32 (9,)).  Input generation only: no model arithmetic."""
+    pos = cfg["pos"].astype(np.float64)
+    Lx, Ly, Lz = float(cfg["box"][0]), float(cfg["box"][4]), float(cfg["box"][8])
+    H = np.array([[Lx, 0.0, 0.0], [bx * Lx, Ly, 0.0], [cx * Lx, cy * Ly, Lz]])
+    out = pos.copy()
+    n_mol = pos.shape[0] // 3
+    for m in range(n_mol):            # atoms are stored molecule by molecule: O, H, H
+        o = pos[3 * m]
+        s = o / np.array([Lx, Ly, Lz])
+        shift = s @ H - o
+        out[3 * m: 3 * m + 3] += shift
+    return out.astype(np.float32), H.astype(np.float32).reshape(9)

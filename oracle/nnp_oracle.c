@@ -58,25 +58,54 @@ static double celu_prime(double x, double a) { return x > 0.0 ? 1.0 : exp(x / a)
 
 /* Minimum-image displacement and the pinned neighbour predicate (section 8.c step 2, readings #6, #7):
  * d = r_j - r_i on fp32 inputs promoted to fp64; d_a -= L_a * rint(d_a / L_a);
- * d2 = fma(dz,dz, fma(dy,dy, dx*dx)). */
-static double disp(const float* pos, int64_t i, int64_t j, const double L[3], int pbc, double d[3]) {
-  for (int a = 0; a < 3; ++a) {
-    double x = (double)pos[3 * j + a] - (double)pos[3 * i + a];
-    if (pbc) x -= L[a] * rint(x / L[a]);
-    d[a] = x;
+ * d2 = fma(dz,dz, fma(dy,dy, dx*dx)).
+ * Triclinic boxes (reading #35) in the GROMACS convention: rows
+ * a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz) with |bx| <= ax/2, |cx| <= ax/2, |cy| <= by/2.  The box is held as
+ * L[6] = {ax, by, cz, bx, cx, cy}; the image is first reduced row by row, c first, then b, then a:
+ *     n = rint(dz/cz): d -= n c;   n = rint(dy/by): d -= n b;   n = rint(dx/ax): d -= n a
+ * which lands in the brick |dz| <= cz/2, ... but is NOT always the nearest image of a skewed box; the nearest one is
+ * then searched among the 27 images d + nc c + nb b + na a, n in {-1,0,1} (loops nc, nb, na outermost to innermost,
+ * first strict minimum of d2 wins).  Pinned against a 343-image brute force in tests/test_oracle_pins.py.  With
+ * bx = cx = cy = 0 no search is made and the arithmetic is the orthorhombic expression above, bit for bit. */
+static double disp(const float* pos, int64_t i, int64_t j, const double L[6], int pbc, double d[3]) {
+  for (int a = 0; a < 3; ++a) d[a] = (double)pos[3 * j + a] - (double)pos[3 * i + a];
+  if (pbc) {
+    double n = rint(d[2] / L[2]);
+    d[2] -= L[2] * n; d[1] -= L[5] * n; d[0] -= L[4] * n;
+    n = rint(d[1] / L[1]);
+    d[1] -= L[1] * n; d[0] -= L[3] * n;
+    n = rint(d[0] / L[0]);
+    d[0] -= L[0] * n;
+    if (L[3] != 0.0 || L[4] != 0.0 || L[5] != 0.0) {
+      double best = fma(d[2], d[2], fma(d[1], d[1], d[0] * d[0])), b[3] = {d[0], d[1], d[2]};
+      for (int nc = -1; nc <= 1; ++nc)
+        for (int nb = -1; nb <= 1; ++nb)
+          for (int na = -1; na <= 1; ++na) {
+            double v[3] = {d[0], d[1], d[2]};
+            v[2] += L[2] * nc; v[1] += L[5] * nc; v[0] += L[4] * nc;
+            v[1] += L[1] * nb; v[0] += L[3] * nb;
+            v[0] += L[0] * na;
+            const double v2 = fma(v[2], v[2], fma(v[1], v[1], v[0] * v[0]));
+            if (v2 < best) { best = v2; b[0] = v[0]; b[1] = v[1]; b[2] = v[2]; }
+          }
+      d[0] = b[0]; d[1] = b[1]; d[2] = b[2];
+    }
   }
   return fma(d[2], d[2], fma(d[1], d[1], d[0] * d[0]));
 }
 
-static int check_box(const float* box, double L[3]) {
+static int check_box(const float* box, double L[6]) {
   for (int r = 0; r < 3; ++r)
     for (int c = 0; c < 3; ++c) {
       double v = (double)box[3 * r + c];
       if (r == c) { if (!(v > 0.0)) return ORC_ERR_BOX; L[r] = v; }
-      else if (v != 0.0) return ORC_ERR_BOX; /* orthorhombic only (reading #9) */
+      else if (c > r && v != 0.0) return ORC_ERR_BOX; /* lower-triangular rows only (readings #9, #35) */
     }
+  L[3] = (double)box[3]; L[4] = (double)box[6]; L[5] = (double)box[7];
+  if (fabs(L[3]) > 0.5 * L[0] || fabs(L[4]) > 0.5 * L[0] || fabs(L[5]) > 0.5 * L[1]) return ORC_ERR_BOX;
   return ORC_OK;
 }
+static int box_is_triclinic(const double L[6]) { return L[3] != 0.0 || L[4] != 0.0 || L[5] != 0.0; }
 
 /* ---------------------------------------------------------------------------------------------
  * Neighbour lists.  mode 0: the definition -- every ordered pair (i,j) of active atoms (O(N^2)).
@@ -91,9 +120,10 @@ typedef struct { int32_t* start; int32_t* col; int64_t n_pairs; } nbr_list;
 
 static void nbr_free(nbr_list* nl) { free(nl->start); free(nl->col); nl->start = nl->col = NULL; }
 
-static int build_neighbors(int64_t n_atoms, const float* pos, const double L[3], int pbc,
+static int build_neighbors(int64_t n_atoms, const float* pos, const double L[6], int pbc,
                            const int32_t* act, int64_t n_ml, double Rc, int mode, nbr_list* out) {
   const double Rc2 = Rc * Rc;
+  if (pbc && box_is_triclinic(L)) mode = 0;   /* the simple cell list below is orthorhombic: use the definition */
   int32_t* count = (int32_t*)calloc((size_t)n_ml + 1, sizeof(int32_t));
   int32_t** rows = (int32_t**)calloc((size_t)n_ml, sizeof(int32_t*));
   int coincident = 0;
@@ -210,7 +240,7 @@ static int32_t* active_set(int64_t n_atoms, const int32_t* ml_index, int64_t n_m
 int64_t orc_neighbors(int64_t n_atoms, const float* pos, const float* box, int32_t pbc,
                       const int32_t* ml_index, int64_t n_ml, double Rc, int32_t mode,
                       int32_t* row_start, int32_t* col, int64_t cap) {
-  double L[3];
+  double L[6];
   int rc = check_box(box, L);
   if (rc) return rc;
   if (!ml_index) n_ml = n_atoms;
@@ -384,7 +414,7 @@ static int eval_impl(const orc_aev_params* p, const orc_mlp* nets /* [S] */, int
              const int32_t* Z, const float* box, int32_t pbc, const int32_t* ml_index, int64_t n_ml,
              int32_t nbr_mode, int32_t want_forces, double* energy, double* forces,
              double* aev_out, double* e_atom, double* daev_out, double* virial9) {
-  double L3[3];
+  double L3[6];
   int rc = check_box(box, L3);
   if (rc) return rc;
   if (!ml_index) n_ml = n_atoms;
@@ -529,11 +559,16 @@ void orc_set_num_threads(int n) {
  * --------------------------------------------------------------------------------------------- */
 static void link_bond(const float* pos, const float* box, int32_t pbc, int32_t a, int32_t b, double* u, double* l) {
   double v[3], s = 0.0;
-  for (int k = 0; k < 3; ++k) {
-    v[k] = (double)pos[3 * (size_t)b + k] - (double)pos[3 * (size_t)a + k];
-    if (pbc) { const double L = (double)box[4 * k]; v[k] -= L * rint(v[k] / L); }
-    s += v[k] * v[k];
+  for (int k = 0; k < 3; ++k) v[k] = (double)pos[3 * (size_t)b + k] - (double)pos[3 * (size_t)a + k];
+  if (pbc) {   /* row-by-row image reduction as in disp(): c, then b, then a (orthorhombic: per component) */
+    double n = rint(v[2] / (double)box[8]);
+    v[2] -= (double)box[8] * n; v[1] -= (double)box[7] * n; v[0] -= (double)box[6] * n;
+    n = rint(v[1] / (double)box[4]);
+    v[1] -= (double)box[4] * n; v[0] -= (double)box[3] * n;
+    n = rint(v[0] / (double)box[0]);
+    v[0] -= (double)box[0] * n;
   }
+  for (int k = 0; k < 3; ++k) s += v[k] * v[k];
   *l = sqrt(s);
   for (int k = 0; k < 3; ++k) u[k] = v[k] / *l;
 }

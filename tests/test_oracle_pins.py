@@ -569,3 +569,89 @@ def test_virial_shear_and_force_moment_open_boundaries():
     for a, b in ((0, 1), (2, 0), (1, 2), (1, 1)):
         fd = _fd_strain(m, pos64, Z, cfg["box"], 0, a, b, 2e-4)
         assert abs(fd - W[a, b]) < 2e-3 * (1 + abs(W[a, b])), (a, b, fd, W[a, b])
+
+
+# ------------------------------------------------------------------ triclinic boxes (reading #35)
+def _tric_water(shear=(0.3, -0.2, 0.4), n=5, L=16.0, seed=41):
+    """125 rigid waters in a sheared box; coordinates and box entries on a 1/1024 grid (exact in fp32, also after
+    shifts by box vectors)."""
+    from gen import water_box, sheared_water_box
+    pos, Z, box, _ = water_box(n, n, n, L, seed)
+    cfg = {"pos": pos, "box": box}
+    p, H = sheared_water_box(cfg, *shear)
+    q = lambda x: (np.round(np.asarray(x, np.float64) * 1024) / 1024)
+    return q(p), Z, q(H).astype(np.float32)
+
+
+def test_triclinic_minimum_image_is_the_brute_force_image_search():
+    """The reduction + 27-image search of the oracle's disp() against the definition: a pair is a neighbour iff SOME lattice
+    image lies within Rc (all 343 images n in {-3..3}^3 tried), on random boxes inside the GROMACS shape limits."""
+    rng = np.random.default_rng(5)
+    Rc = 5.2
+    for trial in range(6):
+        ax, by, cz = rng.uniform(11.0, 16.0, 3)
+        bx, cx, cy = rng.uniform(-0.5, 0.5) * ax, rng.uniform(-0.5, 0.5) * ax, rng.uniform(-0.5, 0.5) * by
+        H = np.array([[ax, 0, 0], [bx, by, 0], [cx, cy, cz]], dtype=np.float32)
+        H64 = H.astype(np.float64)
+        # Rc must not exceed half the smallest box width (distance between opposite faces)
+        vol = abs(np.linalg.det(H64))
+        widths = [vol / np.linalg.norm(np.cross(H64[(k + 1) % 3], H64[(k + 2) % 3])) for k in range(3)]
+        if min(widths) < 2 * Rc + 0.2:
+            continue
+        n = 60
+        pos = (rng.uniform(-0.5, 1.5, (n, 3)) @ H64).astype(np.float32)     # also outside the unit cell
+        s, c = oracle.neighbors(pos, H.reshape(9), Rc)
+        p64 = pos.astype(np.float64)
+        imgs = np.array([[i, j, k] for i in range(-3, 4) for j in range(-3, 4) for k in range(-3, 4)], dtype=np.float64) @ H64
+        ref_cols = []
+        for i in range(n):
+            d = p64[None, :, :] - p64[i][None, None, :] + imgs[:, None, :]
+            near = ((d ** 2).sum(-1) <= Rc * Rc).any(0)
+            near[i] = False
+            ref_cols.append(np.nonzero(near)[0])
+        assert np.array_equal(s, np.concatenate([[0], np.cumsum([len(r) for r in ref_cols])]))
+        assert np.array_equal(c, np.concatenate(ref_cols))
+
+
+def test_triclinic_invariances_and_finite_differences():
+    pos, Z, H = _tric_water()
+    cfg = get_config(0, bias_scale=0.1)
+    model = oracle.Model(cfg["aev"], cfg["nets"])
+    out = oracle.evaluate(model, pos, Z, H)
+    F, scale = out["forces"], np.abs(out["forces"]).max()
+    assert np.abs(F.sum(0)).max() < 1e-9 * scale
+    # atoms moved by whole box vectors (any integer combination): same lists, same energy and forces
+    rng = np.random.default_rng(9)
+    n_int = rng.integers(-2, 3, size=pos.shape).astype(np.float64)
+    pos2 = pos + n_int @ H.astype(np.float64).reshape(3, 3)
+    assert np.array_equal(pos2, pos2.astype(np.float32).astype(np.float64))    # exact in fp32
+    out2 = oracle.evaluate(model, pos2, Z, H)
+    for Rc in (cfg["aev"]["Rcr"], cfg["aev"]["Rca"]):
+        a, b = oracle.neighbors(pos, H, Rc), oracle.neighbors(pos2, H, Rc)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    assert abs(out2["energy"] - out["energy"]) < 1e-9 * abs(out["energy"])
+    assert np.abs(out2["forces"] - F).max() < 1e-9 * scale
+    # rigid translation
+    out3 = oracle.evaluate(model, pos + np.array([1.25, -2.5, 0.75]), Z, H)
+    assert abs(out3["energy"] - out["energy"]) < 1e-9 * abs(out["energy"])
+    # analytic forces against central differences
+    atoms = [0, 1, 2, 200, 374]
+    Ffd = fd_forces(model, pos, Z, H, 1, atoms, 2.0 ** -14)
+    assert np.abs(F[atoms] - Ffd).max() < 5e-6 * scale
+    # zero shear is the orthorhombic arithmetic, bit for bit
+    H0 = np.diag(np.diag(H.reshape(3, 3))).astype(np.float32).reshape(9)
+    a = oracle.evaluate(model, pos, Z, H0)
+    H0b = H0.copy(); H0b[3] = 0.0
+    assert oracle.evaluate(model, pos, Z, H0b)["energy"] == a["energy"]
+
+
+def test_triclinic_box_shape_limits():
+    pos, Z, H = _tric_water()
+    cfg = get_config(0)
+    model = oracle.Model(cfg["aev"], cfg["nets"])
+    bad = H.copy(); bad[3] = 0.6 * H[0]          # |bx| > ax / 2
+    with pytest.raises(RuntimeError):
+        oracle.evaluate(model, pos, Z, bad)
+    bad = H.copy(); bad[2] = 0.1                  # an upper-triangular entry
+    with pytest.raises(RuntimeError):
+        oracle.evaluate(model, pos, Z, bad)
