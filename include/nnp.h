@@ -130,7 +130,10 @@ int nnp_workspace_set_pair_list(nnp_workspace*, const int32_t* d_pairs, int64_t 
 /* One energy+force evaluation.  Asynchronous on the workspace stream.
  *   d_pos      DEVICE [n_atoms][3] fp32, Angstrom, any periodic image
  *   d_Z        DEVICE [n_atoms] int32 atomic numbers (only ML atoms' entries are read)
- *   box        HOST   [9] row vectors a,b,c in Angstrom; orthorhombic only (read during the call)
+ *   box        HOST   [9] row vectors a,b,c in Angstrom (read during the call): orthorhombic, or triclinic in the
+ *                     GROMACS convention a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz) with |bx| <= ax/2, |cx| <= ax/2,
+ *                     |cy| <= by/2 and at least three cut-off wide cells between every pair of opposite faces
+ *                     (face distance >= 3.0003 Rcr); a triclinic evaluation always takes the cell-list path
  *   pbc        1 = xyz periodic (minimum image), 0 = open boundaries (box ignored)
  *   d_ml_index DEVICE [n_ml] int32 strictly ascending atom indices, or NULL => all atoms are ML (n_ml ignored)
  *   d_energy   DEVICE [1] fp64

@@ -48,7 +48,9 @@ __device__ __forceinline__ void load_env(const AevConst& c, const GridInfo* __re
                                          const float4* __restrict__ spos, const uint32_t* __restrict__ rowR,
                                          const uint8_t* __restrict__ rowA, int nR, int nA, float4 ci, int lane,
                                          WarpEnv& e) {
-  const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
+  float ev[9];   // cell edge vectors (orthorhombic: diagonal)
+#pragma unroll
+  for (int k = 0; k < 9; ++k) ev[k] = g->ev[k];
   int seg[MAX_S];
 #pragma unroll
   for (int s = 0; s < MAX_S; ++s) seg[s] = 0;
@@ -60,9 +62,9 @@ __device__ __forceinline__ void load_env(const AevConst& c, const GridInfo* __re
       const int jp = (int)(ent & JMASK);
       const int oc = (int)(ent >> JBITS);
       const float4 pj = spos[jp];
-      const float dx = (pj.x - ci.x) + (float)((oc & 3) - 1) * ex;
-      const float dy = (pj.y - ci.y) + (float)(((oc >> 2) & 3) - 1) * ey;
-      const float dz = (pj.z - ci.z) + (float)(((oc >> 4) & 3) - 1) * ez;
+      float sx, sy, sz;
+      cell_shift(ev, (oc & 3) - 1, ((oc >> 2) & 3) - 1, ((oc >> 4) & 3) - 1, sx, sy, sz);
+      const float dx = (pj.x - ci.x) + sx, dy = (pj.y - ci.y) + sy, dz = (pj.z - ci.z) + sz;
       const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
       const float rinv = rsqrtf(d2);
       const float R = d2 * rinv;

@@ -289,8 +289,10 @@ static int check_box(const float* box, int pbc) {
     for (int c = 0; c < 3; ++c) {
       const float v = box[3 * r + c];
       if (r == c) { if (!(v > 0.f) || !isfinite(v)) return NNP_ERR_BOX_UNSUPPORTED; }
-      else if (v != 0.f) return NNP_ERR_BOX_UNSUPPORTED;
+      else if (c > r ? v != 0.f : !isfinite(v)) return NNP_ERR_BOX_UNSUPPORTED;   // GROMACS rows: lower triangular
     }
+  // triclinic shape limits of the minimum-image reduction (reading #35)
+  if (fabsf(box[3]) > 0.5f * box[0] || fabsf(box[6]) > 0.5f * box[0] || fabsf(box[7]) > 0.5f * box[4]) return NNP_ERR_BOX_UNSUPPORTED;
   return NNP_OK;
 }
 
@@ -302,6 +304,11 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   int rc = check_box(box, pbc);
   if (rc) return rc;
   const float unit[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+  if (pbc) {   // a triclinic box must hold >= 3 cut-off wide cells between every pair of faces
+    float bs[9];
+    for (int i = 0; i < 9; ++i) bs[i] = (float)((double)box[i] * ws->len_scale);
+    if (!neighbor_box_ok(ws, bs)) return NNP_ERR_BOX_UNSUPPORTED;
+  }
   ws->n_atoms = n_atoms; ws->n_ml = n_ml; ws->d_ml_index = d_ml;
   prof_mark(ws, 0);
   int nl = 0;

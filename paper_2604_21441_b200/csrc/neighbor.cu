@@ -49,6 +49,56 @@ __host__ __device__ inline void grid_from_extent(GridInfo* g, int pbc, const dou
   g->L[0] = Lx; g->L[1] = Ly; g->L[2] = Lz;
   g->ncell = nc[0] * nc[1] * nc[2];
   g->pbc = pbc;
+  g->tric = 0;
+  for (int k = 0; k < 9; ++k) { g->ev[k] = 0.f; g->ev_d[k] = 0.0; }
+  for (int d = 0; d < 3; ++d) { g->ev[4 * d] = g->edge[d]; g->ev_d[4 * d] = g->edge_d[d]; }
+  g->H_d[0] = (double)Lx; g->H_d[1] = (double)Ly; g->H_d[2] = (double)Lz; g->H_d[3] = g->H_d[4] = g->H_d[5] = 0.0;
+}
+
+// Periodic triclinic box (HOST; GROMACS rows, reading #35): cells are cut in fractional coordinates, nc[d] =
+// floor(width_d / cutoff) with width_d the distance between the box faces normal to reciprocal direction d, so that
+// neighbours within the cut-off always sit in adjacent cells.  Every dimension needs >= 3 cells (the one-cell
+// minimum-image sweep is orthorhombic only): returns false otherwise.
+inline bool grid_triclinic(GridInfo* g, const float* box, double cutoff, int max_cells) {
+  const double a[3] = {(double)box[0], 0.0, 0.0}, b[3] = {(double)box[3], (double)box[4], 0.0},
+               c[3] = {(double)box[6], (double)box[7], (double)box[8]};
+  auto cross_norm = [](const double* u, const double* v) {
+    const double x = u[1] * v[2] - u[2] * v[1], y = u[2] * v[0] - u[0] * v[2], z = u[0] * v[1] - u[1] * v[0];
+    return sqrt(x * x + y * y + z * z);
+  };
+  const double vol = a[0] * b[1] * c[2];
+  const double width[3] = {vol / cross_norm(b, c), vol / cross_norm(c, a), vol / cross_norm(a, b)};
+  int nc[3];
+  for (int d = 0; d < 3; ++d) { nc[d] = (int)floor(width[d] / cutoff); if (nc[d] < 3) return false; }
+  while ((long long)nc[0] * nc[1] * nc[2] > (long long)max_cells) {
+    int d = 0;
+    if (nc[1] > nc[d]) d = 1;
+    if (nc[2] > nc[d]) d = 2;
+    nc[d] -= 1;
+    if (nc[d] < 3) return false;
+  }
+  const double* rows[3] = {a, b, c};
+  for (int d = 0; d < 3; ++d) {
+    g->nc[d] = nc[d];
+    for (int k = 0; k < 3; ++k) { g->ev_d[3 * d + k] = rows[d][k] / nc[d]; g->ev[3 * d + k] = (float)g->ev_d[3 * d + k]; }
+    g->edge_d[d] = width[d] / nc[d]; g->inv_edge_d[d] = 1.0 / g->edge_d[d]; g->edge[d] = (float)g->edge_d[d];
+    g->origin_d[d] = 0.0;
+    g->L_d[d] = rows[d][d]; g->L[d] = (float)rows[d][d];
+  }
+  g->H_d[0] = a[0]; g->H_d[1] = b[1]; g->H_d[2] = c[2]; g->H_d[3] = b[0]; g->H_d[4] = c[0]; g->H_d[5] = c[1];
+  g->ncell = nc[0] * nc[1] * nc[2];
+  g->pbc = 1;
+  g->tric = 1;
+  return true;
+}
+
+bool box_is_triclinic(const float* box) { return box[3] != 0.f || box[6] != 0.f || box[7] != 0.f; }
+
+// the box of a periodic evaluation can be gridded (orthorhombic: always)
+bool neighbor_box_ok(const nnp_workspace* ws, const float* box) {
+  if (!box_is_triclinic(box)) return true;
+  GridInfo g;
+  return grid_triclinic(&g, box, (double)ws->model->aev.Rcr * (1.0 + 1e-4), ws->max_cells);
 }
 
 // ---------------------------------------------------------------- grid setup (1 block)
@@ -107,6 +157,29 @@ __device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g,
   if (slot < 0) { atomicOr(flags, FLAG_SPECIES); slot = 0; }
   int cc[3];
   float loc[3];
+  if (g->tric) {
+    // fractional coordinates of the lower-triangular box (fp64), wrapped into [0, 1); local position = the fractional
+    // remainder inside the cell times the cell's edge vectors
+    const double x = (double)pos[3 * (size_t)i], y = (double)pos[3 * (size_t)i + 1], z = (double)pos[3 * (size_t)i + 2];
+    double s[3];
+    s[2] = z / g->H_d[2];
+    s[1] = (y - s[2] * g->H_d[5]) / g->H_d[1];
+    s[0] = (x - s[1] * g->H_d[3] - s[2] * g->H_d[4]) / g->H_d[0];
+    double f[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      double t = s[d] - floor(s[d]);
+      if (!(t < 1.0)) t = 0.0;
+      t *= (double)g->nc[d];
+      int ci = (int)t;
+      if (ci >= g->nc[d]) ci = g->nc[d] - 1;
+      cc[d] = ci;
+      f[d] = t - (double)ci;
+    }
+    loc[0] = (float)(f[0] * g->ev_d[0] + f[1] * g->ev_d[3] + f[2] * g->ev_d[6]);
+    loc[1] = (float)(f[1] * g->ev_d[4] + f[2] * g->ev_d[7]);
+    loc[2] = (float)(f[2] * g->ev_d[8]);
+  } else {
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     double x = (double)pos[3 * (size_t)i + d];
@@ -124,6 +197,7 @@ __device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g,
     if (ci >= g->nc[d]) ci = g->nc[d] - 1;
     cc[d] = ci;
     loc[d] = (float)((t - (double)ci) * g->edge_d[d]);
+  }
   }
   int cell = (cc[0] * g->nc[1] + cc[1]) * g->nc[2] + cc[2];
   int key = slot * g->ncell + cell;
@@ -237,6 +311,7 @@ constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of
 // staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
 // cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
 // warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
+template <bool TRIC>
 __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
                                                    const float4* __restrict__ spos,
@@ -247,6 +322,7 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
                                                    int* __restrict__ flags) {
   __shared__ float4 cand[NB_CAP];
   __shared__ int segStart[NB_SEG], segOff[NB_SEG + 1], segCode[NB_SEG];
+  __shared__ float segSx[NB_SEG], segSy[NB_SEG], segSz[NB_SEG];   // Cartesian shift of the segment's cell offset
   __shared__ int cenStart[MAX_S], cenOff[MAX_S + 1];
   __shared__ int wsum[8];
   pdl_trigger();
@@ -291,7 +367,12 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
   __syncthreads();
   int base = 0;
   for (int w = 0; w < warp; ++w) base += wsum[w];
-  if (tid < NB_SEG) { segStart[tid] = b0; segOff[tid] = base + incl - len; segCode[tid] = code; }
+  if (tid < NB_SEG) {
+    segStart[tid] = b0; segOff[tid] = base + incl - len; segCode[tid] = code;
+    float sx, sy, sz;
+    cell_shift(g->ev, (code & 3) - 1, ((code >> 2) & 3) - 1, ((code >> 4) & 3) - 1, sx, sy, sz);
+    segSx[tid] = sx; segSy[tid] = sy; segSz[tid] = sz;
+  }
   int total = 0;
   for (int w = 0; w < 8; ++w) total += wsum[w];
   if (tid == 0) segOff[NB_SEG] = total;
@@ -311,7 +392,7 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
       while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (segOff[mid] <= gq) lo = mid; else hi = mid - 1; }
       const int jp = segStart[lo] + (gq - segOff[lo]), cd = segCode[lo];
       float4 pj = spos[jp];
-      pj.x += (float)((cd & 3) - 1) * ex; pj.y += (float)(((cd >> 2) & 3) - 1) * ey; pj.z += (float)(((cd >> 4) & 3) - 1) * ez;
+      pj.x += segSx[lo]; pj.y += segSy[lo]; pj.z += segSz[lo];
       const int a_j = __float_as_int(pj.w) & 0x0fffffff;
       pj.w = __int_as_float(jp | (cd << JBITS));
       cand[idx] = pj;
@@ -356,7 +437,7 @@ __global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo
           if (near) {
             const int a_j = __float_as_int(spos[ent & JMASK].w) & 0x0fffffff;
             const int o_j = ml ? ml[a_j] : a_j;
-            const double e2 = exact_d2(pos, o_i, o_j, g);
+            const double e2 = TRIC ? exact_d2_tric(pos, o_i, o_j, g) : exact_d2(pos, o_i, o_j, g);
             if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
             if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
             if (e2 == 0.0) bad |= FLAG_COINCIDENT;
@@ -469,6 +550,7 @@ k_pair_fill(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
   const int jc[3] = {cj / (nc[1] * nc[2]), (cj / nc[2]) % nc[1], cj % nc[2]};
   const float li[3] = {pi.x, pi.y, pi.z}, lj[3] = {pj.x, pj.y, pj.z};
   float dd[3];
+  int offs[3];
   uint32_t code_i = 0u, code_j = 0u;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -482,14 +564,20 @@ k_pair_fill(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
       if (g->pbc) { if (off == nc[a] - 1) off = -1; else if (off == 1 - nc[a]) off = 1; }
       if (off < -1 || off > 1) return;             // two cells apart: farther than the cut-off (edge >= Rcr)
     }
-    dd[a] = dl + (float)off * e;
+    dd[a] = dl;
+    offs[a] = off;
     code_i |= (uint32_t)(off + 1) << (2 * a);
     code_j |= (uint32_t)(1 - off) << (2 * a);
+  }
+  {
+    float sx, sy, sz;
+    cell_shift(g->ev, offs[0], offs[1], offs[2], sx, sy, sz);
+    dd[0] += sx; dd[1] += sy; dd[2] += sz;
   }
   const float d2 = fmaf(dd[2], dd[2], fmaf(dd[1], dd[1], dd[0] * dd[0]));
   bool in = d2 < c.Rcr2 - GUARD_BAND;
   if (fabsf(d2 - c.Rcr2) <= GUARD_BAND || d2 < 1e-6f) {
-    const double e2 = exact_d2(pos, gi, gj, g);
+    const double e2 = exact_d2_any(pos, gi, gj, g);
     if (fabsf(d2 - c.Rcr2) <= GUARD_BAND) in = e2 <= c.Rcr2_d;
     if (e2 == 0.0) atomicOr(flags, FLAG_COINCIDENT);
   }
@@ -528,7 +616,6 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
   if (dup) atomicOr(flags, FLAG_ARG);
   const float4 pi = spos[ip];
   const int a_i = __float_as_int(pi.w) & 0x0fffffff;
-  const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
   int nA = 0;
   for (int q0 = 0; q0 < n; q0 += 32) {
     const int q = q0 + lane;
@@ -538,14 +625,14 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
       row[q] = e;
       const float4 pj = spos[e & JMASK];
       const int oc = (int)(e >> JBITS);
-      const float dx = (pj.x - pi.x) + (float)((oc & 3) - 1) * ex;
-      const float dy = (pj.y - pi.y) + (float)(((oc >> 2) & 3) - 1) * ey;
-      const float dz = (pj.z - pi.z) + (float)(((oc >> 4) & 3) - 1) * ez;
+      float sx, sy, sz;
+      cell_shift(g->ev, (oc & 3) - 1, ((oc >> 2) & 3) - 1, ((oc >> 4) & 3) - 1, sx, sy, sz);
+      const float dx = (pj.x - pi.x) + sx, dy = (pj.y - pi.y) + sy, dz = (pj.z - pi.z) + sz;
       const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
       inA = d2 < c.Rca2 - GUARD_BAND;
       if (fabsf(d2 - c.Rca2) <= GUARD_BAND) {
         const int a_j = __float_as_int(pj.w) & 0x0fffffff;
-        inA = exact_d2(pos, ml ? ml[a_i] : a_i, ml ? ml[a_j] : a_j, g) <= c.Rca2_d;
+        inA = exact_d2_any(pos, ml ? ml[a_i] : a_i, ml ? ml[a_j] : a_j, g) <= c.Rca2_d;
       }
     }
     const unsigned m = __ballot_sync(0xffffffffu, inA);
@@ -592,7 +679,10 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
   a.dense_k = ws->dense_k;
   a.host_grid = 0;
-  if (pbc) {   // the cell grid of a periodic box needs no device data
+  if (pbc && box_is_triclinic(box)) {
+    grid_triclinic(&a.hg, box, (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);   // nnp_eval checked neighbor_box_ok
+    a.host_grid = 1;
+  } else if (pbc) {   // the cell grid of a periodic box needs no device data
     const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]}, org[3] = {0.0, 0.0, 0.0};
     grid_from_extent(&a.hg, 1, ext, org, box[0], box[4], box[8], (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);
     a.host_grid = 1;
@@ -630,9 +720,14 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     const int ncell_host = a.host_grid ? a.hg.ncell : ws->max_cells;
     // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
     const int ysplit = (n_ml <= 2048) ? 8 : 1;
-    launch_pdl(!ws->profiling, st, k_neighbors, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
-               ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
-               ws->flags);
+    if (a.host_grid && a.hg.tric)
+      launch_pdl(!ws->profiling, st, k_neighbors<true>, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
+                 ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
+                 ws->flags);
+    else
+      launch_pdl(!ws->profiling, st, k_neighbors<false>, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
+                 ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
+                 ws->flags);
     ++nl;
   }
   return nl;

@@ -55,7 +55,22 @@ struct GridInfo {
   double origin_d[3];  // 0 for pbc; bounding-box minimum for open boundaries
   double L_d[3];       // box lengths (fp32 inputs promoted), for the exact predicate
   float L[3];
+  // Triclinic boxes (GROMACS rows a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz); reading #35).  The cell of
+  // index (i,j,k) has its origin at i ea + j eb + k ec with the edge VECTORS ea = a / nc[0], eb = b / nc[1],
+  // ec = c / nc[2] (ev rows; orthorhombic: the diagonal holds edge[]), and the displacement of a stored neighbour is
+  // (local_j - local_i) + ox ea + oy eb + oz ec.
+  int tric;
+  float ev[9];
+  double ev_d[9];
+  double H_d[6];       // {ax, by, cz, bx, cx, cy}
 };
+
+// Cartesian shift of a cell offset (ox, oy, oz)
+__host__ __device__ inline void cell_shift(const float* __restrict__ ev, int ox, int oy, int oz, float& sx, float& sy, float& sz) {
+  sx = (float)ox * ev[0] + (float)oy * ev[3] + (float)oz * ev[6];
+  sy = (float)oy * ev[4] + (float)oz * ev[7];
+  sz = (float)oz * ev[8];
+}
 
 // Species groups, MLP tiles and the compacted AEV column map of one evaluation (device resident; k_scan).
 // Internal AEV column order: radial species s at s*16 (padded to nRB*32 columns), angular pair p at
@@ -190,6 +205,8 @@ inline void prof_mark(nnp_workspace* ws, int i) { if (ws->profiling) cudaEventRe
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
 int prep_cluster_size();
+bool box_is_triclinic(const float* box);
+bool neighbor_box_ok(const nnp_workspace* ws, const float* box);
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);
 bool small_front_applicable(const nnp_workspace* ws, const float* box, int pbc, int64_t n_ml);
 int launch_small_front(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, const int32_t* d_ml,

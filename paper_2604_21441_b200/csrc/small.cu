@@ -83,10 +83,13 @@ __global__ void __launch_bounds__(SMALL_WARPS * 32, 1) k_small_front(SmallArgs a
     for (int q = 0; q <= MAX_S; ++q) { if (q <= S) gs[q] = run; if (q < S) run += cnt_s[q]; }
     for (int q = S + 1; q <= MAX_S; ++q) gs[q] = run;
     d_groups(gs, S, n, a.max_tiles, a.dense_k, &grp_s, pshift, tb, a.flags);
-    g_s.nc[0] = g_s.nc[1] = g_s.nc[2] = 1; g_s.ncell = 1; g_s.pbc = 1;
+    g_s.nc[0] = g_s.nc[1] = g_s.nc[2] = 1; g_s.ncell = 1; g_s.pbc = 1; g_s.tric = 0;
+    for (int k = 0; k < 9; ++k) { g_s.ev[k] = 0.f; g_s.ev_d[k] = 0.0; }
+    for (int k = 0; k < 6; ++k) g_s.H_d[k] = (k < 3) ? L[k] : 0.0;
     for (int d = 0; d < 3; ++d) {
       g_s.edge[d] = (float)L[d]; g_s.edge_d[d] = L[d]; g_s.inv_edge_d[d] = 1.0 / L[d]; g_s.origin_d[d] = 0.0;
       g_s.L_d[d] = L[d]; g_s.L[d] = (float)L[d];
+      g_s.ev[4 * d] = (float)L[d]; g_s.ev_d[4 * d] = L[d];
     }
   }
   __syncthreads();
@@ -165,7 +168,7 @@ __global__ void __launch_bounds__(SMALL_WARPS * 32, 1) k_small_front(SmallArgs a
 }
 
 bool small_front_applicable(const nnp_workspace* ws, const float* box, int pbc, int64_t n_ml) {
-  return ws->small_path && pbc && n_ml > 0 && n_ml <= SMALL_MAX && !ws->ext_pairs && ws->rcap <= RCAP_MAX &&
+  return ws->small_path && pbc && !box_is_triclinic(box) && n_ml > 0 && n_ml <= SMALL_MAX && !ws->ext_pairs && ws->rcap <= RCAP_MAX &&
          ws->acap <= ACAP_MAX && box[0] <= SMALL_MAX_BOX && box[4] <= SMALL_MAX_BOX && box[8] <= SMALL_MAX_BOX;
 }
 

@@ -607,3 +607,69 @@ def test_small_path_and_general_path(k, layout):
     E3, F3 = run_gpu(ws, pos2, cfg["Z"], cfg["box"], 1, ml)
     check_lists(ws, cfg, pos2, n_ml, ml)
     check_EF(E3, F3, ref2, n_ml, rows=ml)
+
+
+# ------------------------------------------------------------------ triclinic boxes (reading #35)
+@pytest.mark.parametrize("shear", [(0.3, -0.2, 0.4), (-0.5, 0.5, -0.5), (0.0, 0.0, 0.25)])
+def test_triclinic_box(shear):
+    """GROMACS lower-triangular box: cfg 1's waters at the same fractional positions of a sheared box.  Lists bit-exact,
+    E and F within the bars, against the oracle (whose triclinic minimum image is pinned to a brute-force image search)."""
+    import paper_2604_21441_b200 as nnp
+    torch = _torch()
+    cfg = gen.get_config(1)
+    pos, H = gen.sheared_water_box(cfg, *shear)
+    n = pos.shape[0]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, pos, cfg["Z"], H, 1, None, want_aev=True)
+    tcfg = dict(cfg); tcfg["box"] = H
+    m, ws = make(cfg)
+    E, F = run_gpu(ws, pos, cfg["Z"], H)
+    check_lists(ws, tcfg, pos, n)
+    G = ws.aev(n).astype(np.float64)
+    assert np.all(np.abs(G - ref["aev"]) <= 2e-5 * (1 + np.abs(ref["aev"]))), np.abs(G - ref["aev"]).max()
+    check_EF(E, F, ref, n)
+    assert abs(F.sum(0)).max() < 1e-3
+    # atoms moved by whole box vectors: same rows, same results within fp32 rounding of the inputs
+    k = np.random.default_rng(4).integers(-2, 3, size=pos.shape).astype(np.float64)
+    pos2 = (pos.astype(np.float64) + k @ H.astype(np.float64).reshape(3, 3)).astype(np.float32)
+    ref2 = oracle.evaluate(om, pos2, cfg["Z"], H)
+    E2, F2 = run_gpu(ws, pos2, cfg["Z"], H)
+    check_lists(ws, tcfg, pos2, n)
+    check_EF(E2, F2, ref2, n)
+    # the engine's pair list in a triclinic box (candidates from the oracle's own buffered list)
+    s_o, c_o = oracle.neighbors(pos, H, cfg["aev"]["Rcr"] + 0.5)
+    rows = np.repeat(np.arange(n), np.diff(s_o))
+    keep = rows < c_o
+    pairs = np.stack([rows[keep], c_o[keep]], 1).astype(np.int32)
+    ws.set_pair_list(torch.from_numpy(pairs).cuda())
+    E3, F3 = run_gpu(ws, pos, cfg["Z"], H)
+    check_lists(ws, tcfg, pos, n)
+    check_EF(E3, F3, ref, n)
+    ws.set_pair_list(None)
+    # virial against the oracle's strain derivative
+    W = torch.zeros(9, dtype=torch.float64, device="cuda")
+    ws.set_virial_output(W)
+    run_gpu(ws, pos, cfg["Z"], H)
+    Wo = np.asarray(oracle.evaluate_virial(om, pos, cfg["Z"], H)["virial"]).reshape(9)
+    assert np.abs(W.cpu().numpy() - Wo).max() <= 1e-3 * np.abs(Wo).max()
+    ws.set_virial_output(None)
+
+
+def test_triclinic_box_limits():
+    import paper_2604_21441_b200 as nnp
+    torch = _torch()
+    cfg = gen.get_config(1)
+    pos, H = gen.sheared_water_box(cfg, 0.3, -0.2, 0.4)
+    m, ws = make(cfg)
+    dpos, dZ = torch.from_numpy(pos).cuda(), torch.from_numpy(cfg["Z"]).cuda()
+    bad = H.copy(); bad[3] = 0.6 * H[0]                       # |bx| > ax / 2
+    with pytest.raises(nnp.NNPError) as e:
+        ws.eval(dpos, dZ, bad, 1)
+    assert e.value.code == -3
+    bad = H.copy(); bad[1] = 0.5                              # not lower-triangular
+    with pytest.raises(nnp.NNPError):
+        ws.eval(dpos, dZ, bad, 1)
+    small = (H * 0.45).astype(np.float32)                     # < 3 cut-off wide cells between the faces
+    with pytest.raises(nnp.NNPError) as e:
+        ws.eval(dpos, dZ, small, 1)
+    assert e.value.code == -3
