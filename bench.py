@@ -33,8 +33,8 @@ FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's main kernel, from the committed ncu full-set
-# capture profiles/r01g_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
-NCU_TRAFFIC_BYTES = {"neighbour": 0.565e6 + 0.061e6 + 0.490e6, "aev_forward": 8.08e6, "mlp": 18.33e6 + 0.286e6, "aev_backward": 20.98e6,
+# capture profiles/r01h_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
+NCU_TRAFFIC_BYTES = {"neighbour": 0.565e6 + 0.061e6 + 0.490e6, "aev_forward": 8.08e6, "mlp": 18.33e6 + 0.341e6, "aev_backward": 20.98e6,
                      "output": 1.07e6}
 
 
@@ -286,7 +286,7 @@ def run_ours(args, rank, world, local_rank):
     default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1
     roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
                 traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
-                traffic_source="profiles/r01g_launches.md (ncu --set full, per launch)")
+                traffic_source="profiles/r01h_launches.md (ncu --set full, per launch)")
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline and args.ensemble == 1:
