@@ -158,7 +158,7 @@ int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int
  *   nnp_link_spread: adds the chain-rule shares of the link rows of d_forces onto the bonded atoms and zeroes the
  *                    link rows (call after nnp_eval): F_ML += F_L - (d/l)(F_L - u(u.F_L)), F_MM += (d/l)(F_L - u(u.F_L))
  * d = link distance in Angstrom (PAPER.md default 1.0); bond vectors take the minimum image when pbc != 0 (box as in
- * nnp_eval, HOST).  d_link_ml / d_link_mm: DEVICE [n_links] int32 atom indices < n_atoms.  Asynchronous on the given
+ * nnp_eval, HOST: orthorhombic or GROMACS-style triclinic).  d_link_ml / d_link_mm: DEVICE [n_links] int32 atom indices < n_atoms.  Asynchronous on the given
  * cudaStream_t; out-of-range indices and zero-length bonds are skipped.  Returns NNP_ERR_INVALID_ARG / _BOX_UNSUPPORTED
  * for bad arguments. */
 int nnp_link_place(void* cuda_stream, int64_t n_atoms, int64_t n_links, const int32_t* d_link_ml,

@@ -673,3 +673,40 @@ def test_triclinic_box_limits():
     with pytest.raises(nnp.NNPError) as e:
         ws.eval(dpos, dZ, small, 1)
     assert e.value.code == -3
+
+
+def test_link_atoms_triclinic_box():
+    """Link-atom placement and force spread with bonds crossing the faces of a sheared box, against the oracle."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    pos, H = gen.sheared_water_box(cfg, 0.3, -0.2, 0.4)
+    H64 = H.astype(np.float64).reshape(3, 3)
+    n, nl = 60, 12
+    rng = np.random.default_rng(21)
+    p = pos[:n].astype(np.float64)
+    lm = rng.choice(n, nl, replace=False).astype(np.int32)
+    lb = np.array([(a + 1 + rng.integers(0, n - 1)) % n for a in lm], dtype=np.int32)
+    for a, b in zip(lm, lb):     # MM partner 1.2-1.6 A from the ML atom, then moved to another periodic image
+        v = rng.normal(size=3); v *= rng.uniform(1.2, 1.6) / np.linalg.norm(v)
+        p[b] = p[a] + v + rng.integers(-1, 2, 3) @ H64
+    pos_ext = np.concatenate([p, np.zeros((nl, 3))]).astype(np.float32)
+    ref_pos = pos_ext.copy()
+    oracle.link_place(ref_pos, n, lm, lb, H, d=1.0, pbc=1)
+    cfg4 = gen.get_config(0)
+    m, ws = make(cfg4, max_atoms=n + nl)
+    dpos = torch.from_numpy(pos_ext).cuda()
+    dlm, dlb = torch.from_numpy(lm).cuda(), torch.from_numpy(lb).cuda()
+    ws.link_place(dpos, n, dlm, dlb, H, d=1.0, pbc=1)
+    torch.cuda.synchronize()
+    got = dpos.cpu().numpy()
+    assert np.abs(got - ref_pos).max() < 1e-5
+    d = got[n:] - got[lm]
+    assert np.allclose(np.linalg.norm(d, axis=1), 1.0, atol=1e-5)        # the bond's nearest image was taken
+    F = rng.normal(size=(n + nl, 3)).astype(np.float32)
+    refF = F.astype(np.float64)
+    oracle.link_spread(refF, ref_pos, n, lm, lb, H, d=1.0, pbc=1)
+    dF = torch.from_numpy(F.copy()).cuda()
+    ws.link_spread(dF, dpos, n, dlm, dlb, H, d=1.0, pbc=1)
+    torch.cuda.synchronize()
+    assert np.abs(dF.cpu().numpy() - refF).max() < 1e-5
+    assert np.all(dF.cpu().numpy()[n:] == 0.0)
