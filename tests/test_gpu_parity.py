@@ -710,3 +710,24 @@ def test_link_atoms_triclinic_box():
     torch.cuda.synchronize()
     assert np.abs(dF.cpu().numpy() - refF).max() < 1e-5
     assert np.all(dF.cpu().numpy()[n:] == 0.0)
+
+
+@pytest.mark.parametrize("n_sub", [90, 600])
+def test_triclinic_box_ml_subset(n_sub):
+    """An index-listed ML subset in a sheared box (90 ML atoms would take the small-system front end in an orthorhombic
+    box; a triclinic evaluation must fall back to the cell-list path), MM rows +0.0f."""
+    cfg = gen.get_config(1)
+    pos, H = gen.sheared_water_box(cfg, -0.4, 0.3, 0.2)
+    n = pos.shape[0]
+    ml = np.sort(np.random.default_rng(8).choice(n // 3, n_sub // 3, replace=False))
+    ml = (3 * ml[:, None] + np.arange(3)[None, :]).reshape(-1).astype(np.int32)     # whole molecules
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, pos, cfg["Z"], H, 1, ml)
+    tcfg = dict(cfg); tcfg["box"] = H; tcfg["ml_index"] = ml
+    m, ws = make(tcfg)
+    E, F = run_gpu(ws, pos, cfg["Z"], H, 1, ml)
+    assert ws.launches() == 7
+    check_lists(ws, tcfg, pos, len(ml), ml)
+    check_EF(E, F, ref, len(ml), rows=ml)
+    mm = np.setdiff1d(np.arange(n), ml)
+    assert np.all(F[mm] == 0.0) and not np.any(np.signbit(F[mm]))
