@@ -312,7 +312,7 @@ constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of
 // cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
 // warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
 template <bool TRIC>
-__global__ void __launch_bounds__(256, 3) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
+__global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
                                                    const float4* __restrict__ spos,
                                                    const int* __restrict__ bstart, const float* __restrict__ pos,
