@@ -34,7 +34,7 @@ FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's main kernel, from the committed ncu full-set
 # capture profiles/r01h_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
-NCU_TRAFFIC_BYTES = {"neighbour": 0.565e6 + 0.061e6 + 0.490e6, "aev_forward": 8.08e6, "mlp": 18.33e6 + 0.341e6, "aev_backward": 20.98e6,
+NCU_TRAFFIC_BYTES = {"neighbour": 0.502e6 + 0.491e6, "aev_forward": 8.08e6, "mlp": 18.33e6 + 0.413e6, "aev_backward": 20.98e6,
                      "output": 1.07e6}
 
 
