@@ -79,7 +79,9 @@ typedef struct {
 int nnp_model_create(const nnp_aev_params* aev, const nnp_mlp_desc* nets /* HOST [n_species] */, nnp_model** out);
 /* Ensemble of n_members (1..8) networks per element, E = mean of the members' energies -- ANI-2x "is an ensemble of 8
  * networks".  nets: HOST [n_members][n_species], member-major; every member must have the same
- * layer widths per species.  nnp_model_create is the n_members = 1 case.  All members share one AEV. */
+ * layer widths per species.  nnp_model_create is the n_members = 1 case.  All members share one AEV.
+ * The members of a tile hand over in order between the co-resident CTAs of ONE persistent kernel: an ensemble evaluation
+ * needs the device to itself while its MLP kernel runs (do not run ensemble workspaces concurrently on several streams). */
 int nnp_model_create_ensemble(const nnp_aev_params* aev, const nnp_mlp_desc* nets, int32_t n_members, nnp_model** out);
 int nnp_model_destroy(nnp_model*);
 int nnp_model_aev_length(const nnp_model*);

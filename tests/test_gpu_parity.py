@@ -731,3 +731,42 @@ def test_triclinic_box_ml_subset(n_sub):
     check_EF(E, F, ref, len(ml), rows=ml)
     mm = np.setdiff1d(np.arange(n), ml)
     assert np.all(F[mm] == 0.0) and not np.any(np.signbit(F[mm]))
+
+
+def test_two_workspaces_on_two_streams():
+    """Two workspaces of one model on two CUDA streams, evaluations interleaved without synchronisation in between:
+    every result bitwise equal to the same evaluation run alone (the launch chain, tile flags and scratch are per
+    workspace)."""
+    torch = _torch()
+    import paper_2604_21441_b200 as nnp
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 4)
+    m = nnp.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    dpos = [torch.from_numpy(P[t]).cuda() for t in range(4)]
+    ws0 = nnp.Workspace(m, n)
+    alone = []
+    for t in range(4):
+        E, F = ws0.eval(dpos[t], dZ, cfg["box"], 1)
+        torch.cuda.synchronize()
+        alone.append((float(E.cpu()[0]), F.cpu().numpy().copy()))
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s1):
+        w1 = nnp.Workspace(m, n)
+    with torch.cuda.stream(s2):
+        w2 = nnp.Workspace(m, n)
+    outs = []
+    for rep in range(3):
+        for t in range(4):
+            ws, st = (w1, s1) if t % 2 == 0 else (w2, s2)
+            with torch.cuda.stream(st):
+                E = torch.empty(1, dtype=torch.float64, device="cuda")
+                F = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+                ws.eval(dpos[t], dZ, cfg["box"], 1, None, E, F)
+                outs.append((t, E, F))
+    torch.cuda.synchronize()
+    assert w1.status() == 0 and w2.status() == 0
+    for t, E, F in outs:
+        assert float(E.cpu()[0]) == alone[t][0] and np.array_equal(F.cpu().numpy(), alone[t][1])
