@@ -183,6 +183,8 @@ def run_ours(args, rank, world, local_rank):
         ws.set_mlp_mode({"simt": nnp.NNP_MLP_FP32_SIMT, "f16x3": nnp.NNP_MLP_F16X3, "f16x1": nnp.NNP_MLP_F16X1}[args.mlp_mode])
     if args.dense_k:
         ws.set_dense_k(1)
+    if args.bin_reuse > 1:      # not the contract workload: SURVEY.md section 8.d rebuilds everything every step
+        ws.set_bin_reuse(args.bin_reuse, args.skin)
     dpos = [torch.from_numpy(P[t]).cuda() for t in range(N_POS_SETS)]
     dZ = torch.from_numpy(cfg["Z"]).cuda()
     E = torch.zeros(1, dtype=torch.float64, device="cuda")
@@ -283,7 +285,7 @@ def run_ours(args, rank, world, local_rank):
     dom = names[int(np.argmax(stage_ms))]
     roof = dict(stages[dom])
     roof.pop("ms")
-    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1
+    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1 and args.bin_reuse <= 1
     roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
                 traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
                 traffic_source="profiles/r01h_launches.md (ncu --set full, per launch)")
@@ -308,6 +310,7 @@ def run_ours(args, rank, world, local_rank):
                    "l2": "flushed between timed steps (256 MiB write)",
                    "stage_timing": "second pass of the same steps with stage events (serialises the PDL-overlapped kernels)",
                    "mlp_mode": args.mlp_mode, "dense_k": bool(args.dense_k), "ensemble": args.ensemble,
+                   "bin_reuse": args.bin_reuse,
                    "radial_pairs": pairs_R, "triplets": triplets, "parallelism": f"replicas x{world}"},
         "ns_per_day_2fs": 0.1728 * args.steps / total_s,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 12 * n + 8,
@@ -377,6 +380,8 @@ def main():
     ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
     ap.add_argument("--ensemble", type=int, default=1, help="networks per element (ANI-2x: 8); E = mean over members")
     ap.add_argument("--dense-k", action="store_true", help="materialise all 1008 AEV columns (K = 1024 first layer)")
+    ap.add_argument("--bin-reuse", type=int, default=0, help="reuse the cell binning for N-1 of every N steps (0 = rebuild every step)")
+    ap.add_argument("--skin", type=float, default=0.5, help="cell-width buffer in Angstrom for --bin-reuse")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="time every BASELINE.json config (cfg 0-4), one extra JSON line each")
     ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")

@@ -29,11 +29,12 @@ extern "C" {
 #define NNP_OK 0
 #define NNP_ERR_INVALID_ARG (-1)     /* null/negative/unsorted/out-of-range argument, dims[0] != AEV length */
 #define NNP_ERR_UNKNOWN_SPECIES (-2) /* an ML atom's Z has no species slot or no network (MM atoms' Z unread) */
-#define NNP_ERR_BOX_UNSUPPORTED (-3) /* non-zero off-diagonal or non-positive length (orthorhombic only)      */
+#define NNP_ERR_BOX_UNSUPPORTED (-3) /* not orthorhombic / GROMACS-triclinic, or a triclinic box too small     */
 #define NNP_ERR_CAPACITY (-4)        /* a neighbour row overflowed the workspace's row capacity                */
 #define NNP_ERR_COINCIDENT (-5)      /* two ML atoms at distance exactly 0                                     */
 #define NNP_ERR_CUDA (-6)            /* CUDA runtime error or no device                                        */
 #define NNP_ERR_UNSUPPORTED (-7)     /* descriptor shape outside the kernels' range (see nnp_model_create)     */
+#define NNP_ERR_STALE (-8)           /* cell binning reused beyond its validity (nnp_workspace_set_bin_reuse)   */
 
 typedef struct nnp_model nnp_model;         /* opaque, immutable after create, shareable between workspaces */
 typedef struct nnp_workspace nnp_workspace; /* opaque scratch, one per stream, not thread-safe              */
@@ -115,6 +116,19 @@ int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
  * memory and the AEV as ONE kernel (no grid-wide barriers, no cell list); rows, E and F are those of the general path
  * up to fp32 summation order of the positions' frame.  0: always the general cell-list path. */
 int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
+
+/* Reuse of the cell binning over several MD steps ("Verlet-buffered list reuse"; the
+ * paper's runs update GROMACS' own lists every 10-100 steps).  every_n <= 1 (default): every nnp_eval bins and sorts the
+ * ML atoms.  every_n > 1: the cell grid is cut with edges >= Rcr + skin, and for the every_n - 1 evaluations that follow
+ * a full one -- same n_atoms, n_ml, box, pbc and the SAME atoms behind d_Z / d_ml_index (caller's responsibility) -- the
+ * binning, scan, scatter and ordering phases are replaced by one refresh pass that re-reads the positions into the
+ * stored order.  The neighbour ROWS are still built from the current positions with the pinned predicate every step, so
+ * rows, E and F are exactly those of a full evaluation as long as no atom has left its cell by more than skin / 2 in
+ * any direction; one that has raises NNP_ERR_STALE through nnp_status() (outputs of that step unspecified, the next
+ * evaluation rebuilds).  skin in Angstrom (before unit conversion: in the caller's length unit).  Orthorhombic periodic
+ * boxes on the cell-list path only: everything else keeps rebuilding every step.  The step counter lives on the host:
+ * a CUDA graph captures whichever kind of step it was recorded on. */
+int nnp_workspace_set_bin_reuse(nnp_workspace*, int32_t every_n, double skin);
 
 /* External pair list ("The 2026 version adds the internal pair-list built by GROMACS ... as
  * available inputs").  With d_pairs != NULL every later nnp_eval takes its neighbour

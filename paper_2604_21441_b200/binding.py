@@ -16,7 +16,7 @@ NNP_MLP_FP32_SIMT, NNP_MLP_F16X3, NNP_MLP_F16X1 = 0, 1, 2
 
 EXPORTS = [
     "nnp_model_create", "nnp_model_create_ensemble", "nnp_model_destroy", "nnp_model_aev_length", "nnp_workspace_create",
-    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_eval",
+    "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_workspace_set_bin_reuse", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
 ]
@@ -70,6 +70,7 @@ def lib():
         L.nnp_workspace_set_units.argtypes = [vp, C.c_double, C.c_double]
         L.nnp_workspace_set_pair_list.argtypes = [vp, vp, i64]
         L.nnp_workspace_set_small_path.argtypes = [vp, i32]
+        L.nnp_workspace_set_bin_reuse.argtypes = [vp, i32, C.c_double]
         L.nnp_eval.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_eval_host.argtypes = [vp, i64, vp, vp, vp, i32, vp, i64, vp, vp]
         L.nnp_status.argtypes = [vp]
@@ -134,6 +135,10 @@ def nnp_workspace_set_dense_k(ws, dense):
 
 def nnp_workspace_set_units(ws, angstrom_per_length_unit, energy_units_per_ev):
     return lib().nnp_workspace_set_units(ws, float(angstrom_per_length_unit), float(energy_units_per_ev))
+
+
+def nnp_workspace_set_bin_reuse(ws, every_n, skin):
+    return lib().nnp_workspace_set_bin_reuse(ws, int(every_n), float(skin))
 
 
 def nnp_workspace_set_small_path(ws, on):
@@ -286,6 +291,10 @@ class Workspace:
         self._virial = virial
         _check(nnp_workspace_set_virial_output(self.handle, None if virial is None else virial.data_ptr()),
                "nnp_workspace_set_virial_output")
+
+    def set_bin_reuse(self, every_n, skin=0.0):
+        """Reuse the cell binning for every_n - 1 evaluations after a full one (cells cut skin wider); 0 / 1 = off."""
+        _check(nnp_workspace_set_bin_reuse(self.handle, every_n, skin), "nnp_workspace_set_bin_reuse")
 
     def set_small_path(self, on):
         _check(nnp_workspace_set_small_path(self.handle, on), "nnp_workspace_set_small_path")

@@ -23,6 +23,7 @@ extern "C" const char* nnp_strerror(int code) {
     case NNP_ERR_COINCIDENT: return "two ML atoms coincide";
     case NNP_ERR_CUDA: return "CUDA error or no CUDA device";
     case NNP_ERR_UNSUPPORTED: return "descriptor or network shape outside the kernels' range";
+    case NNP_ERR_STALE: return "an atom left its cell by more than skin / 2 while the cell binning was being reused";
     default: return "unknown error";
   }
 }
@@ -269,6 +270,14 @@ extern "C" int nnp_workspace_set_pair_list(nnp_workspace* ws, const int32_t* d_p
   return NNP_OK;
 }
 
+extern "C" int nnp_workspace_set_bin_reuse(nnp_workspace* ws, int32_t every_n, double skin) {
+  if (!ws || (every_n > 1 && !(skin > 0.0))) return NNP_ERR_INVALID_ARG;
+  ws->reuse_every = every_n > 1 ? every_n : 0;
+  ws->reuse_skin = every_n > 1 ? skin : 0.0;
+  ws->reuse_left = 0;   // the next evaluation bins afresh (with the new cell width)
+  return NNP_OK;
+}
+
 extern "C" int nnp_workspace_set_small_path(nnp_workspace* ws, int32_t on) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   ws->small_path = on ? 1 : 0;
@@ -374,6 +383,7 @@ extern "C" int nnp_status(nnp_workspace* ws) {
   if (f & FLAG_SPECIES) return NNP_ERR_UNKNOWN_SPECIES;
   if (f & FLAG_CAP) return NNP_ERR_CAPACITY;
   if (f & FLAG_COINCIDENT) return NNP_ERR_COINCIDENT;
+  if (f & FLAG_STALE) { ws->reuse_left = 0; return NNP_ERR_STALE; }   // the next evaluation bins afresh
   return NNP_OK;
 }
 

@@ -646,6 +646,40 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
   }
 }
 
+// ---------------------------------------------------------------- binning reuse
+// The evaluations between two full binnings keep the stored order (spos.w, scell, bstart, groups, tiles) and only
+// re-read the positions: local coordinate = position relative to the atom's (old) cell, by the nearest image of the
+// cell centre in fp64.  An atom may have drifted out of its cell by up to skin / 2 (the grid was cut with edges
+// >= Rcr + skin, so neighbours within Rcr still sit in adjacent cells); beyond that the step is flagged stale.
+__global__ void __launch_bounds__(256)
+k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const int32_t* __restrict__ ml, int n_ml,
+          double half_skin, float4* __restrict__ spos, const int* __restrict__ scell, unsigned long long* __restrict__ facc,
+          int* __restrict__ flags) {
+  pdl_trigger();
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ip >= n_ml) return;
+  const float w = spos[ip].w;
+  const int a = __float_as_int(w) & 0x0fffffff;
+  const size_t i = ml ? (size_t)ml[a] : (size_t)a;
+  const int cell = scell[ip];
+  const int nc1 = g->nc[1], nc2 = g->nc[2];
+  const int cc[3] = {cell / (nc1 * nc2), (cell / nc2) % nc1, cell % nc2};
+  float loc[3];
+  bool stale = false;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    const double e = g->edge_d[d], L = g->L_d[d];
+    double t = (double)pos[3 * i + d] - ((double)cc[d] + 0.5) * e;   // relative to the cell centre
+    t -= L * rint(t / L);
+    t += 0.5 * e;
+    stale |= (t < -half_skin) || (t > e + half_skin);
+    loc[d] = (float)t;
+  }
+  if (stale) atomicOr(flags, FLAG_STALE);
+  spos[ip] = make_float4(loc[0], loc[1], loc[2], w);
+  facc[3 * (size_t)ip + 0] = 0ull; facc[3 * (size_t)ip + 1] = 0ull; facc[3 * (size_t)ip + 2] = 0ull;
+}
+
 // ---------------------------------------------------------------- host launcher
 // Largest cluster (16, else the portable 8) that can hold k_prep's 1024-thread CTAs on this device; 0 = none.
 int prep_cluster_size() {
@@ -679,15 +713,34 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.pbc = pbc; a.n_atoms = (int)n_atoms; a.n_ml = (int)n_ml; a.max_cells = ws->max_cells; a.max_tiles = ws->max_tiles;
   a.dense_k = ws->dense_k;
   a.host_grid = 0;
+  // binning reuse: orthorhombic periodic boxes; the grid is cut skin wider on every step while it is switched on
+  const bool reuse_ok = ws->reuse_every > 1 && pbc && !box_is_triclinic(box) && n_ml > 0;
+  const double skin = reuse_ok ? ws->reuse_skin * ws->len_scale : 0.0;
+  bool same = reuse_ok && ws->reuse_left > 0 && ws->reuse_n_atoms == n_atoms && ws->reuse_n_ml == n_ml &&
+              ws->reuse_ml == (const void*)d_ml && ws->reuse_Z == (const void*)d_Z;
+  for (int k = 0; k < 9 && same; ++k) same = ws->reuse_box[k] == box[k];
   if (pbc && box_is_triclinic(box)) {
     grid_triclinic(&a.hg, box, (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);   // nnp_eval checked neighbor_box_ok
     a.host_grid = 1;
   } else if (pbc) {   // the cell grid of a periodic box needs no device data
     const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]}, org[3] = {0.0, 0.0, 0.0};
-    grid_from_extent(&a.hg, 1, ext, org, box[0], box[4], box[8], (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);
+    grid_from_extent(&a.hg, 1, ext, org, box[0], box[4], box[8], (double)m->aev.Rcr * (1.0 + 1e-4) + skin, ws->max_cells);
     a.host_grid = 1;
   }
   void* args[] = {&a};
+  if (same) {
+    // refresh-only step: the stored order stays, positions are re-read (the grid on the device is the same one)
+    --ws->reuse_left;
+    k_refresh<<<(unsigned)((n_ml + 255) / 256), 256, 0, st>>>(ws->grid, d_pos, d_ml, (int)n_ml, 0.5 * skin, ws->spos, ws->scell,
+                                                             ws->facc, ws->flags);
+  } else {
+  if (reuse_ok) {
+    ws->reuse_left = ws->reuse_every - 1; ws->reuse_n_atoms = n_atoms; ws->reuse_n_ml = n_ml;
+    ws->reuse_ml = d_ml; ws->reuse_Z = d_Z;
+    for (int k = 0; k < 9; ++k) ws->reuse_box[k] = box[k];
+  } else {
+    ws->reuse_left = 0;
+  }
   if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ws->prep_cluster); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = 0; cfg.stream = st;
@@ -701,6 +754,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     const int64_t want = std::max<int64_t>((n_ml + 1023) / 1024, ((int64_t)m->aev.S * ws->max_cells * 32 + 1023) / 1024);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, ws->num_sms));
     cudaLaunchCooperativeKernel((const void*)k_prep<false>, dim3(grid), dim3(1024), args, 0, st);
+  }
   }
   int nl = 1;
   if (n_ml > 0 && ws->ext_pairs) {

@@ -23,7 +23,7 @@ constexpr uint32_t JMASK = (1u << JBITS) - 1u;
 constexpr int FIX_SHIFT = 40;     // fixed-point scale 2^40 for the int64 force accumulators (K8)
 
 // device-side sticky status bits
-enum : int { FLAG_ARG = 1, FLAG_SPECIES = 2, FLAG_CAP = 4, FLAG_COINCIDENT = 8 };
+enum : int { FLAG_ARG = 1, FLAG_SPECIES = 2, FLAG_CAP = 4, FLAG_COINCIDENT = 8, FLAG_STALE = 16 };
 
 // Descriptor constants, passed to kernels by value.
 struct AevConst {
@@ -169,6 +169,10 @@ struct nnp_workspace {
   double* d_virial;          // caller's DEVICE [9] output, or nullptr = virial off
   float* pos_scaled;         // [max_atoms][3] positions converted to Angstrom (unit conversion on)
   double len_scale, e_scale; // Angstrom per caller length unit; caller energy units per eV (1, 1 = off)
+  int reuse_every;           // > 1: the cell binning is reused for reuse_every - 1 evaluations after a full one
+  double reuse_skin;         // Angstrom per caller length unit applied at use; cells are cut >= Rcr + skin wide
+  int reuse_left;            // refresh-only evaluations left before the next full binning
+  int64_t reuse_n_atoms, reuse_n_ml; float reuse_box[9]; const void* reuse_ml; const void* reuse_Z;   // what the stored order belongs to
   const int32_t* ext_pairs;  // caller's DEVICE [n_ext_pairs][2] candidate pair list, or nullptr = own cell search
   int64_t n_ext_pairs;
   void* tc_ws;               // tensor-core path scratch

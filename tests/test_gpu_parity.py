@@ -770,3 +770,43 @@ def test_two_workspaces_on_two_streams():
     assert w1.status() == 0 and w2.status() == 0
     for t, E, F in outs:
         assert float(E.cpu()[0]) == alone[t][0] and np.array_equal(F.cpu().numpy(), alone[t][1])
+
+
+def test_bin_reuse_over_md_like_steps():
+    """SURVEY.md section 8.f item 4 (Verlet-buffered reuse): the cell binning is reused for 4 of every 5 evaluations while
+    the atoms jitter; rows stay bit-exact against the oracle and E, F inside the bars on every step; an atom that leaves
+    its cell by more than skin / 2 on a reuse step is reported (NNP_ERR_STALE) and the next evaluation recovers."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 7, sigma=0.05)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    m, ws = make(cfg)
+    ws.set_bin_reuse(5, 1.0)
+    dZ = torch.from_numpy(cfg["Z"]).cuda()     # the same device buffers on every step, as an MD engine would pass them
+    dpos = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    for t in range(7):
+        dpos.copy_(torch.from_numpy(P[t]))
+        E, F = ws.eval(dpos, dZ, cfg["box"], 1)
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        ref = oracle.evaluate(om, P[t], cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
+        check_lists(ws, cfg, P[t], n)
+        check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, n)
+    # step 7 is a reuse step (full binnings at steps 0 and 5): push one atom 1.5 A out of its cell
+    bad = P[0].copy(); bad[17] += np.array([1.5, 1.5, 1.5], dtype=np.float32) * 2
+    dpos.copy_(torch.from_numpy(bad))
+    ws.eval(dpos, dZ, cfg["box"], 1)
+    assert ws.status() == -8
+    E, F = ws.eval(dpos, dZ, cfg["box"], 1)    # rebuilds
+    torch.cuda.synchronize()
+    assert ws.status() == 0
+    ref = oracle.evaluate(om, bad, cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
+    check_lists(ws, cfg, bad, n)
+    check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, n)
+    # switched off: plain evaluations again, bitwise equal to a fresh workspace
+    ws.set_bin_reuse(0)
+    E1, F1 = run_gpu(ws, P[3], cfg["Z"], cfg["box"])
+    m2, ws2 = make(cfg)
+    E2, F2 = run_gpu(ws2, P[3], cfg["Z"], cfg["box"])
+    assert E1 == E2 and np.array_equal(F1, F2)
