@@ -810,3 +810,32 @@ def test_bin_reuse_over_md_like_steps():
     m2, ws2 = make(cfg)
     E2, F2 = run_gpu(ws2, P[3], cfg["Z"], cfg["box"])
     assert E1 == E2 and np.array_equal(F1, F2)
+
+
+def test_bin_reuse_with_ml_subset_and_pair_list():
+    """Binning reuse on the cell-list path with an index-listed ML subset (cfg 4, small-system front end off), with and
+    without the engine's pair list: every step against the oracle."""
+    torch = _torch()
+    cfg = gen.get_config(4)
+    ml = cfg["ml_index"]
+    n = cfg["pos"].shape[0]
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    rng = np.random.default_rng(12)
+    m, ws = make(cfg)
+    ws.set_small_path(0)
+    ws.set_bin_reuse(4, 0.8)
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    dml = torch.from_numpy(ml).cuda()
+    dpos = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    pairs = _buffered_pairs(cfg["pos"], cfg["box"], 1, np.sort(ml), cfg["aev"]["Rcr"] + 1.0, seed=3)
+    dpairs = torch.from_numpy(pairs).cuda()
+    for t in range(6):
+        pos = (cfg["pos"] + rng.normal(0, 0.03, size=cfg["pos"].shape)).astype(np.float32)
+        dpos.copy_(torch.from_numpy(pos))
+        ws.set_pair_list(dpairs if t >= 3 else None)
+        E, F = ws.eval(dpos, dZ, cfg["box"], 1, dml)
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        ref = oracle.evaluate(om, pos, cfg["Z"], cfg["box"], 1, ml)
+        check_lists(ws, cfg, pos, len(ml), ml)
+        check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, len(ml), rows=ml)
