@@ -125,8 +125,8 @@ int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
  * stored order.  The neighbour ROWS are still built from the current positions with the pinned predicate every step, so
  * rows, E and F are exactly those of a full evaluation as long as no atom has left its cell by more than skin / 2 in
  * any direction; one that has raises NNP_ERR_STALE through nnp_status() (outputs of that step unspecified, the next
- * evaluation rebuilds).  skin in Angstrom (before unit conversion: in the caller's length unit).  Orthorhombic periodic
- * boxes on the cell-list path only: everything else keeps rebuilding every step.  The step counter lives on the host:
+ * evaluation rebuilds).  skin in the caller's length unit.  Periodic boxes (orthorhombic or triclinic) on the cell-list
+ * path only: open boundaries and the small-system front end keep rebuilding every step.  The step counter lives on the host:
  * a CUDA graph captures whichever kind of step it was recorded on. */
 int nnp_workspace_set_bin_reuse(nnp_workspace*, int32_t every_n, double skin);
 

@@ -98,7 +98,8 @@ bool box_is_triclinic(const float* box) { return box[3] != 0.f || box[6] != 0.f 
 bool neighbor_box_ok(const nnp_workspace* ws, const float* box) {
   if (!box_is_triclinic(box)) return true;
   GridInfo g;
-  return grid_triclinic(&g, box, (double)ws->model->aev.Rcr * (1.0 + 1e-4), ws->max_cells);
+  const double skin = ws->reuse_every > 1 ? ws->reuse_skin * ws->len_scale : 0.0;
+  return grid_triclinic(&g, box, (double)ws->model->aev.Rcr * (1.0 + 1e-4) + skin, ws->max_cells);
 }
 
 // ---------------------------------------------------------------- grid setup (1 block)
@@ -666,6 +667,27 @@ k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const i
   const int cc[3] = {cell / (nc1 * nc2), (cell / nc2) % nc1, cell % nc2};
   float loc[3];
   bool stale = false;
+  if (g->tric) {
+    // fractional coordinates (as in the binning), offset from the cell centre in units of cells, nearest image
+    const double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
+    double sf[3], f[3];
+    sf[2] = z / g->H_d[2];
+    sf[1] = (y - sf[2] * g->H_d[5]) / g->H_d[1];
+    sf[0] = (x - sf[1] * g->H_d[3] - sf[2] * g->H_d[4]) / g->H_d[0];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double ncd = (double)g->nc[d];
+      double t = sf[d] * ncd - ((double)cc[d] + 0.5);
+      t -= ncd * rint(t / ncd);
+      t += 0.5;
+      // edge_d = distance between the cell's faces: the excursion beyond a face in Angstrom
+      stale |= (t * g->edge_d[d] < -half_skin) || ((t - 1.0) * g->edge_d[d] > half_skin);
+      f[d] = t;
+    }
+    loc[0] = (float)(f[0] * g->ev_d[0] + f[1] * g->ev_d[3] + f[2] * g->ev_d[6]);
+    loc[1] = (float)(f[1] * g->ev_d[4] + f[2] * g->ev_d[7]);
+    loc[2] = (float)(f[2] * g->ev_d[8]);
+  } else {
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     const double e = g->edge_d[d], L = g->L_d[d];
@@ -674,6 +696,7 @@ k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const i
     t += 0.5 * e;
     stale |= (t < -half_skin) || (t > e + half_skin);
     loc[d] = (float)t;
+  }
   }
   if (stale) atomicOr(flags, FLAG_STALE);
   spos[ip] = make_float4(loc[0], loc[1], loc[2], w);
@@ -714,13 +737,13 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   a.dense_k = ws->dense_k;
   a.host_grid = 0;
   // binning reuse: orthorhombic periodic boxes; the grid is cut skin wider on every step while it is switched on
-  const bool reuse_ok = ws->reuse_every > 1 && pbc && !box_is_triclinic(box) && n_ml > 0;
+  const bool reuse_ok = ws->reuse_every > 1 && pbc && n_ml > 0;
   const double skin = reuse_ok ? ws->reuse_skin * ws->len_scale : 0.0;
   bool same = reuse_ok && ws->reuse_left > 0 && ws->reuse_n_atoms == n_atoms && ws->reuse_n_ml == n_ml &&
               ws->reuse_ml == (const void*)d_ml && ws->reuse_Z == (const void*)d_Z;
   for (int k = 0; k < 9 && same; ++k) same = ws->reuse_box[k] == box[k];
   if (pbc && box_is_triclinic(box)) {
-    grid_triclinic(&a.hg, box, (double)m->aev.Rcr * (1.0 + 1e-4), ws->max_cells);   // nnp_eval checked neighbor_box_ok
+    grid_triclinic(&a.hg, box, (double)m->aev.Rcr * (1.0 + 1e-4) + skin, ws->max_cells);   // nnp_eval checked neighbor_box_ok
     a.host_grid = 1;
   } else if (pbc) {   // the cell grid of a periodic box needs no device data
     const double ext[3] = {(double)box[0], (double)box[4], (double)box[8]}, org[3] = {0.0, 0.0, 0.0};

@@ -794,7 +794,7 @@ def test_bin_reuse_over_md_like_steps():
         check_lists(ws, cfg, P[t], n)
         check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, n)
     # step 7 is a reuse step (full binnings at steps 0 and 5): push one atom 1.5 A out of its cell
-    bad = P[0].copy(); bad[17] += np.array([1.5, 1.5, 1.5], dtype=np.float32) * 2
+    bad = P[0].copy(); bad[17] += np.float32(8.0)      # farther than a cell edge + skin / 2
     dpos.copy_(torch.from_numpy(bad))
     ws.eval(dpos, dZ, cfg["box"], 1)
     assert ws.status() == -8
@@ -810,6 +810,35 @@ def test_bin_reuse_over_md_like_steps():
     m2, ws2 = make(cfg)
     E2, F2 = run_gpu(ws2, P[3], cfg["Z"], cfg["box"])
     assert E1 == E2 and np.array_equal(F1, F2)
+
+
+def test_bin_reuse_triclinic():
+    torch = _torch()
+    cfg = gen.get_config(1)
+    pos0, H = gen.sheared_water_box(cfg, 0.3, -0.2, 0.4)
+    n = pos0.shape[0]
+    tcfg = dict(cfg); tcfg["box"] = H
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    rng = np.random.default_rng(14)
+    m, ws = make(cfg)
+    ws.set_bin_reuse(4, 1.0)
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    dpos = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    for t in range(5):
+        pos = (pos0 + rng.normal(0, 0.05, size=pos0.shape)).astype(np.float32)
+        if t == 2:      # whole-box-vector shifts on a reuse step: the nearest image of the stored cell is taken
+            pos = (pos.astype(np.float64) + rng.integers(-1, 2, size=pos.shape) @ H.astype(np.float64).reshape(3, 3)).astype(np.float32)
+        dpos.copy_(torch.from_numpy(pos))
+        E, F = ws.eval(dpos, dZ, H, 1)
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        ref = oracle.evaluate(om, pos, cfg["Z"], H)
+        check_lists(ws, tcfg, pos, n)
+        check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, n)
+    bad = pos0.copy(); bad[40] += np.float32(9.0)      # farther than a cell edge + skin / 2 along z
+    dpos.copy_(torch.from_numpy(bad))
+    ws.eval(dpos, dZ, H, 1)       # step 5 is a reuse step (full binnings at 0 and 4)
+    assert ws.status() == -8
 
 
 def test_bin_reuse_with_ml_subset_and_pair_list():
