@@ -214,6 +214,12 @@ int nnp_debug_mlp_timeline(nnp_workspace*, int64_t* h_ticks);
  * energy reduction K8}. */
 int nnp_workspace_set_profiling(nnp_workspace*, int32_t on);
 int nnp_debug_stage_times(nnp_workspace*, float* ms);
+/* Measured FP32-pipe peak of the current device: the denominator of the AEV kernels' roofline fractions (BASELINE.md
+ * section 4 asks for "a register-resident FMA loop" measurement).  Runs a register-resident loop
+ * of independent FMA chains on every SM (8 blocks of 256 threads per SM), timed with CUDA events on cuda_stream, and
+ * writes HOST *h_tflops = best of 5 launches, counting 2 flop per FMA lane.  variant 0: scalar FFMA with three register
+ * operands; variant 1: packed FFMA2 (fma.rn.f32x2, two FMA lanes per instruction, sm_100).  Synchronises the stream. */
+int nnp_debug_fp32_peak(void* cuda_stream, int32_t variant, double* h_tflops);
 
 #ifdef __cplusplus
 }

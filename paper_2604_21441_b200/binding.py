@@ -19,6 +19,7 @@ EXPORTS = [
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_workspace_set_bin_reuse", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
+    "nnp_debug_fp32_peak",
 ]
 
 
@@ -86,6 +87,7 @@ def lib():
         L.nnp_link_spread.argtypes = [vp, i64, i64, vp, vp, C.c_double, vp, i32, vp, vp]
         L.nnp_workspace_set_profiling.argtypes = [vp, i32]
         L.nnp_debug_stage_times.argtypes = [vp, vp]
+        L.nnp_debug_fp32_peak.argtypes = [vp, i32, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -208,6 +210,12 @@ def nnp_workspace_set_profiling(ws, on):
 
 def nnp_debug_stage_times(ws, h_ms):
     return lib().nnp_debug_stage_times(ws, h_ms)
+
+
+def nnp_debug_fp32_peak(cuda_stream, variant):
+    t = C.c_double(0.0)
+    rc = lib().nnp_debug_fp32_peak(cuda_stream, int(variant), C.byref(t))
+    return rc, t.value
 
 
 # ---------------------------------------------------------------- convenience owners

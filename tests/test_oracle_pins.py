@@ -198,8 +198,10 @@ def test_neighbor_list_is_the_double_loop():
         assert set(ca[sa[i]:sa[i + 1]]) <= set(cr[sr[i]:sr[i + 1]])
 
 
-@pytest.mark.parametrize("k", [0, 1, 4])
+@pytest.mark.parametrize("k", [0, 1, 2, 4])
 def test_cell_list_equals_definition(k):
+    """The oracle's cell-list mode (mode=1, what the cfg-2 / cfg-3 GPU lists and the timed CPU baseline use) equals its
+    O(N^2) definition (mode=0) -- at headline size too (cfg 2: one 24 000-atom double loop per cut-off)."""
     cfg = get_config(k)
     for Rc in (5.2, 3.5):
         s0, c0 = oracle.neighbors(cfg["pos"], cfg["box"], Rc, ml_index=cfg["ml_index"], mode=0)
@@ -474,6 +476,73 @@ def test_link_atom_placement_eq4(pbc, d):
         assert np.dot(rl - ra, v) > 0                                             # on the MM side
         np.testing.assert_allclose(rl, ra + d * v / np.linalg.norm(v), atol=2e-6)
 
+
+
+def _sheared_link_case(seed):
+    """A sheared GROMACS box (lower-triangular rows inside the shape limits), bonds of KNOWN direction v placed through
+    a KNOWN integer combination k.H of box vectors: r_MM = r_ML + v + k.H.  Returns everything the known answer needs."""
+    rng = np.random.default_rng(seed)
+    H = np.array([[14.0, 0.0, 0.0], [rng.uniform(-6.5, 6.5), 13.0, 0.0],
+                  [rng.uniform(-6.5, 6.5), rng.uniform(-6.0, 6.0), 12.0]])
+    n, nl = 8, 3
+    pos = rng.uniform(0.0, 12.0, size=(n, 3))
+    lm, lb = np.array([0, 1, 2], np.int32), np.array([5, 6, 7], np.int32)
+    vs, ks = [], []
+    for q in range(nl):
+        v = rng.normal(size=3)
+        v *= rng.uniform(1.0, 1.6) / np.linalg.norm(v)          # a covalent bond length, far below half a box width
+        k = rng.integers(-2, 3, size=3)
+        pos[lb[q]] = pos[lm[q]] + v + k @ H
+        vs.append(v); ks.append(k)
+    ext = np.zeros((n + nl, 3), np.float32)
+    ext[:n] = pos
+    return n, ext, lm, lb, H, np.array(vs), np.array(ks)
+
+
+@pytest.mark.parametrize("seed", [5, 6, 7])
+@pytest.mark.parametrize("d", [1.0, 0.73])
+def test_link_atom_placement_triclinic_known_answer(seed, d):
+    """PAPER.md lines 79-82, eq. 4 in a SHEARED box (oracle link_bond(), the box[3] / box[6] / box[7] terms): the bonded MM
+    partner sits in another periodic image, r_MM = r_ML + v + k.H with known v and integer k, so the known answer is
+    r_L = r_ML + d v/|v| -- any other image choice moves r_L by whole box vectors.  Cross-check: the bond image the
+    oracle took is the brute-force minimum over the 27 surrounding images of the row-reduced vector."""
+    n, ext, lm, lb, H, vs, ks = _sheared_link_case(seed)
+    box = H.astype(np.float32).reshape(9)
+    assert np.any(ks != 0)
+    oracle.link_place(ext, n, lm, lb, box, d, 1)
+    Hf = box.reshape(3, 3).astype(np.float64)
+    for q in range(len(lm)):
+        ra, rb = ext[lm[q]].astype(np.float64), ext[lb[q]].astype(np.float64)
+        rl = ext[n + q].astype(np.float64)
+        want = ra + d * vs[q] / np.linalg.norm(vs[q])
+        np.testing.assert_allclose(rl, want, atol=3e-6)          # fp32 storage of r_MM and r_L
+        # brute force: the shortest of all images rb - ra + m.H, m in {-3..3}^3, is the bond the oracle used
+        best = min((np.linalg.norm(rb - ra + np.array(m) @ Hf), m)
+                   for m in [(a, b, c) for a in range(-3, 4) for b in range(-3, 4) for c in range(-3, 4)])
+        np.testing.assert_allclose((rl - ra) / d, (rb - ra + np.array(best[1]) @ Hf) / best[0], atol=3e-6)
+
+
+def test_link_force_spread_triclinic_conserves_force_and_is_chain_rule():
+    """Force redistribution with the sheared-box bond: total force conserved and the shares are the chain rule of eq. 4
+    written out with the KNOWN bond vector v (not the oracle's image search)."""
+    d = 1.0
+    n, ext, lm, lb, H, vs, ks = _sheared_link_case(9)
+    box = H.astype(np.float32).reshape(9)
+    oracle.link_place(ext, n, lm, lb, box, d, 1)
+    rng = np.random.default_rng(2)
+    F = rng.normal(size=(n + len(lm), 3))
+    F0 = F.copy()
+    oracle.link_spread(F, ext, n, lm, lb, box, d, 1)
+    np.testing.assert_allclose(F.sum(axis=0), F0.sum(axis=0), atol=1e-12)
+    assert np.all(F[n:] == 0.0)
+    want = F0.copy()
+    for q in range(len(lm)):
+        l = np.linalg.norm(vs[q]); u = vs[q] / l
+        perp = (d / l) * (F0[n + q] - u * np.dot(u, F0[n + q]))
+        want[lm[q]] += F0[n + q] - perp
+        want[lb[q]] += perp
+        want[n + q] = 0.0
+    np.testing.assert_allclose(F, want, atol=2e-6)               # v is known to fp32 rounding of the stored positions
 
 @pytest.mark.parametrize("pbc", [0, 1])
 def test_link_force_spread_conserves_force_and_torque(pbc):
