@@ -12,12 +12,12 @@
 
 namespace nnp {
 
-__global__ void __launch_bounds__(AEV_FWD_WARPS * 32, 32 / AEV_FWD_WARPS)
+__global__ void __launch_bounds__(AEV_FWD_WARPS * 32, 10)
 k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
               const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
               float* __restrict__ aev) {
-  __shared__ WarpEnv env[AEV_FWD_WARPS];
+  __shared__ FwdEnv env[AEV_FWD_WARPS];
   pdl_trigger();
   pdl_wait();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;

@@ -162,7 +162,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   cudaStreamSynchronize(ws->stream);
   tc_workspace_destroy(ws);
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
-  void* ptrs[] = {ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
+  void* ptrs[] = {ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
                   ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->pos_scaled, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_energy, ws->hd_forces};
@@ -202,6 +202,8 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
   bool ok = dmalloc(&ws->grid, 1) && dmalloc(&ws->groups, 1) && dmalloc(&ws->tiles, (size_t)ws->max_tiles) &&
             dmalloc(&ws->flags, 1) && dmalloc(&ws->cell_count, (size_t)MAX_S * ws->max_cells + 1) &&
             dmalloc(&ws->bstart, (size_t)MAX_S * ws->max_cells + 1) && dmalloc(&ws->tmp4, nm) &&
+            dmalloc(&ws->cellbuf, (size_t)ws->max_cells * cell_cap()) && dmalloc(&ws->cellfill, (size_t)ws->max_cells) &&
+            dmalloc(&ws->present, 1) &&
             dmalloc(&ws->rank, nm) && dmalloc(&ws->spos, nm) && dmalloc(&ws->scell, nm) &&
             dmalloc(&ws->nbrR, nm * ws->rcap) && dmalloc(&ws->nbrA, nm * ws->acap) && dmalloc(&ws->cntR, nm) &&
             dmalloc(&ws->cntA, nm) && dmalloc(&ws->aev, nr * K) && dmalloc(&ws->daev, nr * K) &&
@@ -379,11 +381,13 @@ extern "C" int nnp_status(nnp_workspace* ws) {
   int f = 0;
   CU_OK(cudaMemcpy(&f, ws->flags, sizeof(int), cudaMemcpyDeviceToHost));
   CU_OK(cudaMemset(ws->flags, 0, sizeof(int)));
+  if (f & FLAG_STALE) ws->reuse_left = 0;   // whatever else went wrong: the next evaluation bins afresh
+  if (f & FLAG_CAP) ws->slow_prep = 1;      // (possibly) a cell beyond the fast binning's buffer: general binning from now on
   if (f & FLAG_ARG) return NNP_ERR_INVALID_ARG;
   if (f & FLAG_SPECIES) return NNP_ERR_UNKNOWN_SPECIES;
   if (f & FLAG_CAP) return NNP_ERR_CAPACITY;
   if (f & FLAG_COINCIDENT) return NNP_ERR_COINCIDENT;
-  if (f & FLAG_STALE) { ws->reuse_left = 0; return NNP_ERR_STALE; }   // the next evaluation bins afresh
+  if (f & FLAG_STALE) return NNP_ERR_STALE;
   return NNP_OK;
 }
 

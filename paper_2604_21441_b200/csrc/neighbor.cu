@@ -141,12 +141,10 @@ __device__ void d_grid_setup(GridInfo* g, GroupInfo* grp, int pbc, float Lx, flo
 }
 
 // ---------------------------------------------------------------- K0: species map, ML gather, cell key
-__device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
-                      const int32_t* __restrict__ Z, const int32_t* __restrict__ ml, int n_atoms, int n_ml,
-                      float4* __restrict__ tmp4, int* __restrict__ rank, int* __restrict__ cell_count,
-                      unsigned long long* __restrict__ facc, int* __restrict__ flags) {
-  int a = vb * blockDim.x + threadIdx.x;
-  if (a >= n_ml) return;
+// ML atom a (ML-local index): species slot, cell and cell-local coordinates (fp64 cell coordinates, rounded to fp32 once)
+__device__ __forceinline__ void bin_coords(const AevConst& c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
+                                           const int32_t* __restrict__ Z, const int32_t* __restrict__ ml, int n_atoms, int a,
+                                           int* __restrict__ flags, int& slot, int& cell, float (&loc)[3]) {
   int i = a;
   if (ml) {
     i = ml[a];
@@ -154,10 +152,9 @@ __device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g,
     if (bad) { atomicOr(flags, FLAG_ARG); i = min(max(i, 0), n_atoms - 1); }
   }
   int z = Z[i];
-  int slot = (z >= 0 && z < 128) ? (int)c.zlut[z] : -1;
+  slot = (z >= 0 && z < 128) ? (int)c.zlut[z] : -1;
   if (slot < 0) { atomicOr(flags, FLAG_SPECIES); slot = 0; }
   int cc[3];
-  float loc[3];
   if (g->tric) {
     // fractional coordinates of the lower-triangular box (fp64), wrapped into [0, 1); local position = the fractional
     // remainder inside the cell times the cell's edge vectors
@@ -200,7 +197,18 @@ __device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g,
     loc[d] = (float)((t - (double)ci) * g->edge_d[d]);
   }
   }
-  int cell = (cc[0] * g->nc[1] + cc[1]) * g->nc[2] + cc[2];
+  cell = (cc[0] * g->nc[1] + cc[1]) * g->nc[2] + cc[2];
+}
+
+__device__ void d_bin(int vb, const AevConst& c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
+                      const int32_t* __restrict__ Z, const int32_t* __restrict__ ml, int n_atoms, int n_ml,
+                      float4* __restrict__ tmp4, int* __restrict__ rank, int* __restrict__ cell_count,
+                      unsigned long long* __restrict__ facc, int* __restrict__ flags) {
+  int a = vb * blockDim.x + threadIdx.x;
+  if (a >= n_ml) return;
+  int slot, cell;
+  float loc[3];
+  bin_coords(c, g, pos, Z, ml, n_atoms, a, flags, slot, cell, loc);
   int key = slot * g->ncell + cell;
   rank[a] = atomicAdd(&cell_count[key], 1);
   tmp4[a] = make_float4(loc[0], loc[1], loc[2], __int_as_float(key));
@@ -218,8 +226,8 @@ __device__ void d_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
   __shared__ int wtot[32];
   __shared__ int gs[MAX_S + 1], tb[MAX_S + 1];
   const int ncell = g->ncell, n = S * ncell;
-  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
-  const int span = (((n + 31) / 32 + 31) / 32) * 32;
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5, nw = (int)blockDim.x >> 5;
+  const int span = (((n + nw - 1) / nw + 31) / 32) * 32;
   const int lo = min(wp * span, n), hi = min(lo + span, n);
   int sum = 0;
   for (int k0 = lo; k0 < hi; k0 += 128) {
@@ -230,7 +238,7 @@ __device__ void d_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
   if (lane == 0) wtot[wp] = sum;
   __syncthreads();
   int carry = 0, total = 0;
-  for (int w = 0; w < 32; ++w) { const int t = wtot[w]; if (w < wp) carry += t; total += t; }
+  for (int w = 0; w < nw; ++w) { const int t = wtot[w]; if (w < wp) carry += t; total += t; }
   for (int k0 = lo; k0 < hi; k0 += 128) {
     int v[4];
 #pragma unroll
@@ -252,8 +260,14 @@ __device__ void d_scan(const GridInfo* __restrict__ g, int* __restrict__ count,
   if (threadIdx.x == 0) { bstart[n] = total; gs[S] = total; if (total != n_ml) atomicOr(flags, FLAG_ARG); }
   __syncthreads();
   __shared__ int pshift[MAX_S];
-  if (threadIdx.x == 0) d_groups(gs, S, n_ml, max_tiles, dense_k, grp, pshift, tb, flags);
+  __shared__ GroupInfo grp_s;   // filled by one thread in shared memory, published by all (one thread's ~150 dependent global stores cost microseconds)
+  if (threadIdx.x == 0) d_groups(gs, S, n_ml, max_tiles, dense_k, &grp_s, pshift, tb, flags);
   __syncthreads();
+  {
+    const int* src = reinterpret_cast<const int*>(&grp_s);
+    int* dst = reinterpret_cast<int*>(grp);
+    for (int k = threadIdx.x; k < (int)(sizeof(GroupInfo) / sizeof(int)); k += blockDim.x) dst[k] = src[k];
+  }
   d_tiles(gs, pshift, tb, S, max_tiles, tiles);
 }
 
@@ -304,14 +318,176 @@ __device__ void d_bucket_sort(int vb, const GridInfo* __restrict__ g, int S, con
   }
 }
 
+// ---------------------------------------------------------------- K0-K1, fast variant: append + per-cell ordering
+// Periodic boxes with >= 3 cells in every dimension (the grid is known on the host).
+//   k_bin_cells : every ML atom is appended to a fixed-capacity buffer of its CELL (the atomic rank is the destination:
+//                 no scatter pass) and counted per (species, cell) bucket;
+//   k_cell_sort : one warp per cell.  Bucket starts come from sums every block forms for itself over the bucket counts
+//                 of the species present (cfg 2: 2 x 1331 counts, ten loads per thread): no grid-wide scan, no barrier.
+//                 (Counting per group of cells with atomics as a second level was measured and dropped: a few hundred
+//                 atomics on one address serialise in L2 -- 11 us for 24 000 atoms on 84 counters.)  The
+//                 cell's atoms then go to their place in the slot-major sorted order of the general path: an atom's
+//                 place inside its (species, cell) bucket is its rank by ML index among the bucket's atoms -- a pure
+//                 function of the cell's content, so the order is reproducible although the append order is not.
+// Block 0 of k_cell_sort also derives groups, tiles and the column set.  The counters are cleared by k_neighbors (every
+// cell has a block there).  Against k_prep (five phases, four grid-wide barriers): cfg 2 27 us -> ~10 us.
+constexpr int CELL_CAP = 96;            // atoms per cell in the append buffer (liquid water at Rcr-wide cells: ~18)
+constexpr int BIN_THREADS = 256;
+constexpr int FAST_MAX_CELLS = 32768;   // every k_cell_sort block reads all bucket counts of the species present: beyond this k_prep's scan
+
+struct BinArgs {
+  AevConst c;
+  GridInfo hg;
+  GridInfo* grid;
+  const float* pos; const int32_t* Z; const int32_t* ml;
+  float4* cellbuf; int* cellfill; int* cell_count; int* present;
+  unsigned long long* facc; int* flags;
+  int n_atoms, n_ml;
+};
+
+__global__ void __launch_bounds__(BIN_THREADS) k_bin_cells(const __grid_constant__ BinArgs a) {
+  __shared__ int spres;
+  pdl_trigger();
+  const GridInfo* g = &a.hg;
+  if (threadIdx.x == 0) spres = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *a.grid = a.hg;
+  __syncthreads();
+  const int i = blockIdx.x * BIN_THREADS + threadIdx.x;
+  int bit = 0;
+  if (i < a.n_ml) {
+    int slot, cell;
+    float loc[3];
+    bin_coords(a.c, g, a.pos, a.Z, a.ml, a.n_atoms, i, a.flags, slot, cell, loc);
+    atomicAdd(&a.cell_count[slot * g->ncell + cell], 1);
+    const int r = atomicAdd(&a.cellfill[cell], 1);
+    if (r < CELL_CAP) a.cellbuf[(size_t)cell * CELL_CAP + r] = make_float4(loc[0], loc[1], loc[2], __int_as_float(i | (slot << 28)));
+    else atomicOr(a.flags, FLAG_CAP);
+    a.facc[3 * (size_t)i + 0] = 0ull; a.facc[3 * (size_t)i + 1] = 0ull; a.facc[3 * (size_t)i + 2] = 0ull;
+    bit = 1 << slot;
+  }
+  bit = __reduce_or_sync(0xffffffffu, bit);
+  if ((threadIdx.x & 31) == 0 && bit) atomicOr(&spres, bit);
+  __syncthreads();
+  if (threadIdx.x == 0 && spres) atomicOr(a.present, spres);
+}
+
+struct SortArgs {
+  GroupInfo* groups; TileInfo* tiles;
+  const float4* cellbuf; const int* cell_count; const int* present;
+  int* bstart; float4* spos; int* scell; int* flags;
+  int S, ncell, n_ml, max_tiles, dense_k;
+};
+
+__global__ void __launch_bounds__(256) k_cell_sort(const __grid_constant__ SortArgs a) {
+  __shared__ int red[8][2][MAX_S];
+  __shared__ int cnt8[8][MAX_S], bst8[8][MAX_S];
+  __shared__ int gs[MAX_S + 1], pre_s[MAX_S], pshift[MAX_S], tb[MAX_S + 1];
+  __shared__ GroupInfo grp_s;
+  pdl_trigger();
+  pdl_wait();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int S = a.S, ncell = a.ncell;
+  const int c0 = blockIdx.x * 8, cell = c0 + warp;
+  // the cell's appended atoms, three per lane (the slots beyond the cell's count hold stale data and are masked below)
+  constexpr int PER = CELL_CAP / 32;
+  float4 e[PER];
+#pragma unroll
+  for (int u = 0; u < PER; ++u)
+    e[u] = (cell < ncell) ? a.cellbuf[(size_t)cell * CELL_CAP + u * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+  const int pm = *a.present;
+  // ---- per species present: atoms in all cells (tot) and in the cells before this block's (pre)
+  int tot[MAX_S], pre[MAX_S];
+#pragma unroll
+  for (int s = 0; s < MAX_S; ++s) {
+    tot[s] = 0; pre[s] = 0;
+    if (s < S && ((pm >> s) & 1)) {
+      for (int c = tid; c < ncell; c += 256) { const int v = a.cell_count[s * ncell + c]; tot[s] += v; if (c < c0) pre[s] += v; }
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < MAX_S; ++s) {
+    if (s < S && ((pm >> s) & 1)) {
+      for (int o = 16; o > 0; o >>= 1) { tot[s] += __shfl_xor_sync(0xffffffffu, tot[s], o); pre[s] += __shfl_xor_sync(0xffffffffu, pre[s], o); }
+    }
+    if (lane == 0) { red[warp][0][s] = tot[s]; red[warp][1][s] = pre[s]; }
+  }
+  if (lane < MAX_S) cnt8[warp][lane] = (lane < S && cell < ncell && ((pm >> lane) & 1)) ? a.cell_count[lane * ncell + cell] : 0;
+  __syncthreads();
+  if (tid < MAX_S) {
+    int T = 0, P = 0;
+    for (int w = 0; w < 8; ++w) { T += red[w][0][tid]; P += red[w][1][tid]; }
+    red[0][0][tid] = T; pre_s[tid] = P;   // (only thread tid touches column tid of red[0][0] here)
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int run = 0;
+    for (int q = 0; q <= MAX_S; ++q) { gs[q] = run; if (q < MAX_S) run += red[0][0][q]; }
+  }
+  __syncthreads();
+  // ---- bucket starts of this block's cells
+  if (lane < MAX_S) {
+    int b = gs[lane] + pre_s[lane];
+    for (int w = 0; w < warp; ++w) b += cnt8[w][lane];
+    bst8[warp][lane] = b;
+    if (lane < S && cell < ncell) a.bstart[lane * ncell + cell] = b;
+  }
+  if (blockIdx.x == 0 && tid == 0) {
+    a.bstart[S * ncell] = gs[MAX_S];
+    if (gs[MAX_S] != a.n_ml) atomicOr(a.flags, FLAG_ARG);
+  }
+  __syncwarp();
+  // ---- rank inside the (species, cell) bucket by ML index, write to the sorted order
+  if (cell < ncell) {
+    int n = 0;
+    for (int s = 0; s < S; ++s) n += cnt8[warp][s];
+    n = min(n, CELL_CAP);
+    int key[PER], rank[PER];
+#pragma unroll
+    for (int u = 0; u < PER; ++u) { key[u] = (u * 32 + lane < n) ? __float_as_int(e[u].w) : 0x7fffffff; rank[u] = 0; }
+#pragma unroll
+    for (int v = 0; v < PER; ++v) {
+      if (v * 32 < n) {
+        const int m = min(32, n - v * 32);
+        for (int o = 0; o < m; ++o) {
+          const int ko = __shfl_sync(0xffffffffu, key[v], o);
+#pragma unroll
+          for (int u = 0; u < PER; ++u) rank[u] += (((ko ^ key[u]) >> 28) == 0 && ko < key[u]) ? 1 : 0;
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < PER; ++u) {
+      if (u * 32 + lane < n) {
+        const int dst = bst8[warp][(key[u] >> 28) & 7] + rank[u];
+        if (dst < a.n_ml) { a.spos[dst] = e[u]; a.scell[dst] = cell; }
+      }
+    }
+  }
+  // ---- block 0: groups, tiles, column set
+  if (blockIdx.x == 0) {
+    if (warp == 0) d_groups_warp(gs, S, a.n_ml, a.max_tiles, a.dense_k, &grp_s, pshift, tb, a.flags);
+    __syncthreads();
+    const int* src = reinterpret_cast<const int*>(&grp_s);
+    int* dst = reinterpret_cast<int*>(a.groups);
+    for (int k = tid; k < (int)(sizeof(GroupInfo) / sizeof(int)); k += 256) dst[k] = src[k];
+    d_tiles(gs, pshift, tb, S, a.max_tiles, a.tiles);
+  }
+}
+
 // ---------------------------------------------------------------- K2: neighbour rows, one warp per centre
 constexpr int NB_CAP = 1024;            // candidates staged in shared memory per chunk
 constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of one centre cell
+constexpr int SURV_CAP = 256;           // candidates of one centre that pass the cheap distance filter, per chunk
 
 // One block per cell.  The atoms of the 27 neighbouring cells (per species: 27 buckets of the slot-major sort) are
 // staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
-// cell and sweeps the staged candidates 32 at a time with full lanes (fp32 pre-filter, guard-band fp64 re-check,
-// warp-ballot compaction).  Candidates are ordered species-major, so rows come out sorted by species.
+// cell and goes over the staged candidates in TWO stages:
+//   1. filter: 32 candidates per iteration, fp32 distance against Rcr^2 + guard, ballot compaction of the survivors'
+//      staging indices into a per-warp list (~20 instructions per 32 candidates; ~12 % survive);
+//   2. decide: the survivors, 32 at a time with full lanes: radial / angular membership by the fp32 value outside the
+//      guard bands and by the pinned fp64 predicate on the ORIGINAL coordinates inside them (reading #6), ballot
+//      compaction into the rows.
+// Candidates are ordered species-major, so rows come out sorted by species.
 template <bool TRIC>
 __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo* __restrict__ g,
                                                    const GroupInfo* __restrict__ grp,
@@ -320,18 +496,26 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
                                                    const int32_t* __restrict__ ml, int n_ml, int rcap, int acap,
                                                    uint32_t* __restrict__ nbrR, uint8_t* __restrict__ nbrA,
                                                    int* __restrict__ cntR, int* __restrict__ cntA,
-                                                   int* __restrict__ flags) {
+                                                   int* __restrict__ flags, int* __restrict__ zcount,
+                                                   int* __restrict__ zfill, int* __restrict__ zpresent) {
   __shared__ float4 cand[NB_CAP];
+  __shared__ int candA[NB_CAP];           // ML-local index of the candidate (for the fp64 re-check)
   __shared__ int segStart[NB_SEG], segOff[NB_SEG + 1], segCode[NB_SEG];
   __shared__ float segSx[NB_SEG], segSy[NB_SEG], segSz[NB_SEG];   // Cartesian shift of the segment's cell offset
   __shared__ int cenStart[MAX_S], cenOff[MAX_S + 1];
   __shared__ int wsum[8];
+  __shared__ unsigned short surv[8][SURV_CAP];
   pdl_trigger();
   pdl_wait();
   const int cell = blockIdx.x, ncell = g->ncell;
   if (cell >= ncell) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (cell == 0 && tid == 0 && (int)gridDim.x < ncell) atomicOr(flags, FLAG_ARG);   // host / device cell counts differ
+  if (zcount && blockIdx.y == 0) {   // fast binning: its counters go back to zero here (every cell has a block; nobody reads them any more)
+    if (tid < c.S) zcount[tid * ncell + cell] = 0;
+    if (tid == 32) zfill[cell] = 0;
+    if (tid == 33 && cell == 0) *zpresent = 0;
+  }
   const int nc0 = g->nc[0], nc1 = g->nc[1], nc2 = g->nc[2], pbc = g->pbc, S = c.S;
   const int cz = cell % nc2, cy = (cell / nc2) % nc1, cx = cell / (nc1 * nc2);
   const float ex = g->edge[0], ey = g->edge[1], ez = g->edge[2];
@@ -385,22 +569,29 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
 
   for (int chunk0 = 0; chunk0 < total; chunk0 += NB_CAP) {
     const int nin = min(NB_CAP, total - chunk0);
+    const int nin32 = (nin + 31) & ~31;   // the filter sweeps whole groups of 32: the tail holds far-away dummies
     if (chunk0 > 0) __syncthreads();
     // ---- stage the candidates of this chunk, shifted into the centre cell's frame
-    for (int idx = tid; idx < nin; idx += 256) {
-      const int gq = chunk0 + idx;
-      int lo = 0, hi = NB_SEG - 1;            // last segment with segOff <= gq
-      while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (segOff[mid] <= gq) lo = mid; else hi = mid - 1; }
-      const int jp = segStart[lo] + (gq - segOff[lo]), cd = segCode[lo];
-      float4 pj = spos[jp];
-      pj.x += segSx[lo]; pj.y += segSy[lo]; pj.z += segSz[lo];
-      const int a_j = __float_as_int(pj.w) & 0x0fffffff;
-      pj.w = __int_as_float(jp | (cd << JBITS));
-      cand[idx] = pj;
-      (void)a_j;
+    {
+      for (int idx = tid; idx < nin32; idx += 256) {
+        if (idx >= nin) { cand[idx] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, __int_as_float(0)); continue; }
+        const int gq = chunk0 + idx;
+        int lo = 0, hi = NB_SEG - 1;            // last segment with segOff <= gq
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (segOff[mid] <= gq) lo = mid; else hi = mid - 1; }
+        const int jp = segStart[lo] + (gq - segOff[lo]), cd = segCode[lo];
+        float4 pj = spos[jp];
+        pj.x += segSx[lo]; pj.y += segSy[lo]; pj.z += segSz[lo];
+        candA[idx] = __float_as_int(pj.w) & 0x0fffffff;
+        pj.w = __int_as_float(jp | (cd << JBITS));
+        cand[idx] = pj;
+      }
     }
     __syncthreads();
     // ---- sweep: one warp per centre
+    const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
+    const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
+    const float hi2 = c.Rcr2 + 2.0f * GUARD_BAND;
+    unsigned short* sv = surv[warp];
     for (int ci = warp + 8 * blockIdx.y; ci < nC; ci += 8 * gridDim.y) {   // small systems: gridDim.y blocks share a cell
       int s = 0;
       while (s + 1 < MAX_S && ci >= cenOff[s + 1]) ++s;
@@ -408,51 +599,67 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
       const float4 pi = spos[ip];
       const int a_i = __float_as_int(pi.w) & 0x0fffffff;
       const int o_i = ml ? ml[a_i] : a_i;
-      uint32_t* rowR = nbrR + (size_t)ip * rcap;
-      uint8_t* rowA = nbrA + (size_t)ip * acap;
+      // ---- stage 1: cheap filter
+      int ns = 0;
+      {
+        const float4* cp = cand + lane;
+        for (int q0 = 0; q0 < nin32; q0 += 32, cp += 32) {
+          const float4 pj = *cp;
+          float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+          if (wrap) {   // block-uniform: a dimension with a single cell takes the minimum image per pair
+            if (nc0 == 1) dx -= rintf(dx / ex) * ex;
+            if (nc1 == 1) dy -= rintf(dy / ey) * ey;
+            if (nc2 == 1) dz -= rintf(dz / ez) * ez;
+          }
+          const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+          const bool pass = d2 <= hi2;
+          const unsigned m = __ballot_sync(0xffffffffu, pass);
+          const int p = ns + __popc(m & lt);
+          if (pass && p < SURV_CAP) sv[p] = (unsigned short)(q0 + lane);
+          ns += __popc(m);
+        }
+      }
+      if (ns > SURV_CAP) { bad |= FLAG_CAP; ns = SURV_CAP; }
+      __syncwarp();
+      // ---- stage 2: decide the survivors
+      uint32_t* rR = nbrR + (size_t)ip * rcap;
+      uint8_t* rA = nbrA + (size_t)ip * acap;
       int nR = 0, nA = 0;
       if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; }
-      const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
-      const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
-      const float4* cp = cand + lane;
-      // keep the row pointers and capacities in registers: rebuilding them from the kernel parameters every
-      // iteration costs more issue slots than the distance test itself
-      uint32_t* rR = rowR; uint8_t* rA = rowA;
-      int capR = rcap, capA = acap;
-      asm volatile("" : "+l"(rR), "+l"(rA), "+r"(capR), "+r"(capA));
-      for (int q0 = lane; q0 - lane < nin; q0 += 32, cp += 32) {
-        const float4 pj = (q0 < nin) ? *cp : make_float4(1.0e18f, 1.0e18f, 1.0e18f, __int_as_float(ip));
+      for (int s0 = 0; s0 < ns; s0 += 32) {
+        const bool live = s0 + lane < ns;
+        const int q = live ? (int)sv[s0 + lane] : 0;
+        const float4 pj = cand[q];
         uint32_t ent = (uint32_t)__float_as_int(pj.w);
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-        if (wrap) {   // block-uniform: a dimension with a single cell takes the minimum image per pair
+        if (wrap) {
           if (nc0 == 1) { const int o = -(int)rintf(dx / ex); dx += (float)o * ex; ent += (uint32_t)o << JBITS; }
           if (nc1 == 1) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
           if (nc2 == 1) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
         }
         const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        const bool other = (int)(ent & JMASK) != ip;
+        const bool other = live && (int)(ent & JMASK) != ip;
         bool inR = other && d2 < loR, inA = other && d2 < loA;
         // guard bands (and coincident atoms): the pinned fp64 predicate on the original coordinates decides
         const bool near = other && (fabsf(d2 - Rcr2) <= GUARD_BAND || fabsf(d2 - Rca2) <= GUARD_BAND || d2 < 1e-6f);
-        if (__any_sync(0xffffffffu, near)) {
-          if (near) {
-            const int a_j = __float_as_int(spos[ent & JMASK].w) & 0x0fffffff;
-            const int o_j = ml ? ml[a_j] : a_j;
-            const double e2 = TRIC ? exact_d2_tric(pos, o_i, o_j, g) : exact_d2(pos, o_i, o_j, g);
-            if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
-            if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
-            if (e2 == 0.0) bad |= FLAG_COINCIDENT;
-          }
+        if (near) {
+          const int a_j = candA[q];
+          const int o_j = ml ? ml[a_j] : a_j;
+          const double e2 = TRIC ? exact_d2_tric(pos, o_i, o_j, g) : exact_d2(pos, o_i, o_j, g);
+          if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
+          if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
+          if (e2 == 0.0) bad |= FLAG_COINCIDENT;
         }
         const unsigned mR = __ballot_sync(0xffffffffu, inR);
         const unsigned mA = __ballot_sync(0xffffffffu, inA);
         const int pR = nR + __popc(mR & lt), pA = nA + __popc(mA & lt);
-        if (inR && pR < capR) rR[pR] = ent;
-        if (inA && pA < capA && pR < capR) rA[pA] = (uint8_t)pR;
+        if (inR && pR < rcap) rR[pR] = ent;
+        if (inA && pA < acap && pR < rcap) rA[pA] = (uint8_t)pR;
         nR += __popc(mR); nA += __popc(mA);
       }
       if (nR > rcap || nA > acap) bad |= FLAG_CAP;
       if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
+      __syncwarp();
     }
   }
   if (bad) atomicOr(flags, bad);
@@ -704,6 +911,8 @@ k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const i
 }
 
 // ---------------------------------------------------------------- host launcher
+int cell_cap() { return CELL_CAP; }
+
 // Largest cluster (16, else the portable 8) that can hold k_prep's 1024-thread CTAs on this device; 0 = none.
 int prep_cluster_size() {
   cudaFuncSetAttribute((const void*)k_prep<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
@@ -751,6 +960,12 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     a.host_grid = 1;
   }
   void* args[] = {&a};
+  // fast binning (k_bin_cells + ranking inside k_neighbors): periodic boxes cut into >= 3 cells per dimension, own cell
+  // search; a cell that overflowed its append buffer (NNP_ERR_CAPACITY) sends the workspace back to the general path
+  const bool fast = a.host_grid && a.hg.nc[0] >= 3 && a.hg.nc[1] >= 3 && a.hg.nc[2] >= 3 && !ws->ext_pairs && !ws->slow_prep &&
+                    a.hg.ncell <= ws->max_cells && a.hg.ncell <= FAST_MAX_CELLS;
+  int extra = 0;   // kernels launched beyond the first
+  bool fast_bin = false;   // this evaluation binned with k_bin_cells (k_neighbors clears its counters)
   if (same) {
     // refresh-only step: the stored order stays, positions are re-read (the grid on the device is the same one)
     --ws->reuse_left;
@@ -764,7 +979,23 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   } else {
     ws->reuse_left = 0;
   }
-  if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
+  if (fast) {
+    BinArgs b;
+    b.c = m->aev; b.hg = a.hg; b.grid = ws->grid;
+    b.pos = d_pos; b.Z = d_Z; b.ml = d_ml;
+    b.cellbuf = ws->cellbuf; b.cellfill = ws->cellfill; b.cell_count = ws->cell_count; b.present = ws->present;
+    b.facc = ws->facc; b.flags = ws->flags;
+    b.n_atoms = (int)n_atoms; b.n_ml = (int)n_ml;
+    k_bin_cells<<<(unsigned)((n_ml + BIN_THREADS - 1) / BIN_THREADS), BIN_THREADS, 0, st>>>(b);
+    SortArgs q;
+    q.groups = ws->groups; q.tiles = ws->tiles;
+    q.cellbuf = ws->cellbuf; q.cell_count = ws->cell_count; q.present = ws->present;
+    q.bstart = ws->bstart; q.spos = ws->spos; q.scell = ws->scell; q.flags = ws->flags;
+    q.S = m->aev.S; q.ncell = a.hg.ncell; q.n_ml = (int)n_ml; q.max_tiles = ws->max_tiles; q.dense_k = ws->dense_k;
+    launch_pdl(!ws->profiling, st, k_cell_sort, dim3((unsigned)((a.hg.ncell + 7) / 8)), dim3(256), 0, q);
+    fast_bin = true;
+    extra = 1;
+  } else if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ws->prep_cluster); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = 0; cfg.stream = st;
     cudaLaunchAttribute at[1];
@@ -779,7 +1010,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     cudaLaunchCooperativeKernel((const void*)k_prep<false>, dim3(grid), dim3(1024), args, 0, st);
   }
   }
-  int nl = 1;
+  int nl = 1 + extra;
   if (n_ml > 0 && ws->ext_pairs) {
     // external candidate pairs instead of the cell sweep (plain launches: fully ordered behind k_prep)
     k_pair_index<<<(unsigned)((n_ml + 255) / 256), 256, 0, st>>>(ws->spos, (int)n_ml, ws->rank, ws->cntR);
@@ -797,14 +1028,11 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     const int ncell_host = a.host_grid ? a.hg.ncell : ws->max_cells;
     // few atoms in few cells (a 96-atom box is ONE cell): several blocks per cell split its centres, or one SM does it all
     const int ysplit = (n_ml <= 2048) ? 8 : 1;
-    if (a.host_grid && a.hg.tric)
-      launch_pdl(!ws->profiling, st, k_neighbors<true>, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
-                 ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
-                 ws->flags);
-    else
-      launch_pdl(!ws->profiling, st, k_neighbors<false>, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups,
-                 ws->spos, ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA,
-                 ws->flags);
+    const bool tric = a.host_grid && a.hg.tric;
+    auto kern = tric ? k_neighbors<true> : k_neighbors<false>;
+    launch_pdl(!ws->profiling, st, kern, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups, ws->spos,
+               ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->flags,
+               fast_bin ? ws->cell_count : nullptr, ws->cellfill, ws->present);
     ++nl;
   }
   return nl;

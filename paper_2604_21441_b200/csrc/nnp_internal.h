@@ -150,6 +150,10 @@ struct nnp_workspace {
   int* cell_count;           // [MAX_S*max_cells + 1]
   int* bstart;               // [MAX_S*max_cells + 1]
   float4* tmp4;              // [max_ml] local coords + key
+  float4* cellbuf;           // [max_cells][CELL_CAP] per-cell append buffers of the fast binning (neighbor.cu)
+  int* cellfill;             // [max_cells] fill counters of the above (zero between evaluations)
+  int* present;              // [1] bit mask of the species slots seen by k_bin_cells (zero between evaluations)
+  int slow_prep;             // 1: a cell overflowed its append buffer once; this workspace keeps to the general binning
   int* rank;                 // [max_ml]
   float4* spos;              // [max_ml] sorted: cell-local xyz, w = ml-local index | slot << 28
   int* scell;                // [max_ml]
@@ -209,6 +213,7 @@ inline void prof_mark(nnp_workspace* ws, int i) { if (ws->profiling) cudaEventRe
 int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, int pbc,
                           const int32_t* d_ml, int64_t n_atoms, int64_t n_ml);
 int prep_cluster_size();
+int cell_cap();   // atoms per cell in the fast binning's append buffers
 bool box_is_triclinic(const float* box);
 bool neighbor_box_ok(const nnp_workspace* ws, const float* box);
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);

@@ -35,7 +35,7 @@ struct SmallArgs {
 };
 
 __global__ void __launch_bounds__(SMALL_WARPS * 32, 1) k_small_front(SmallArgs a) {
-  __shared__ WarpEnv env[SMALL_WARPS];
+  __shared__ FwdEnv env[SMALL_WARPS];
   __shared__ float4 sp[SMALL_MAX];                       // sorted: local xyz, w = ML-local index | slot << 28
   __shared__ uint32_t rowR_s[SMALL_WARPS][RCAP_MAX];     // first the unsorted positions (float4 tmp[SMALL_MAX]), then rows
   __shared__ uint8_t rowA_s[SMALL_WARPS][ACAP_MAX];

@@ -590,7 +590,7 @@ def test_small_path_and_general_path(k, layout):
     for on in (1, 0):
         ws.set_small_path(on)
         E, F = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
-        assert ws.launches() == (5 if on else 7)
+        assert ws.launches() == 5 if on else ws.launches() in (7, 8)   # general path: k_prep, or k_bin_cells + k_cell_sort
         check_lists(ws, cfg, cfg["pos"], n_ml, ml)
         G = ws.aev(n_ml).astype(np.float64)
         assert np.all(np.abs(G - ref["aev"]) <= 2e-5 * (1 + np.abs(ref["aev"]))), np.abs(G - ref["aev"]).max()
@@ -726,7 +726,7 @@ def test_triclinic_box_ml_subset(n_sub):
     tcfg = dict(cfg); tcfg["box"] = H; tcfg["ml_index"] = ml
     m, ws = make(tcfg)
     E, F = run_gpu(ws, pos, cfg["Z"], H, 1, ml)
-    assert ws.launches() == 7
+    assert ws.launches() in (7, 8)   # never the small-system front end (5)
     check_lists(ws, tcfg, pos, len(ml), ml)
     check_EF(E, F, ref, len(ml), rows=ml)
     mm = np.setdiff1d(np.arange(n), ml)
