@@ -73,19 +73,26 @@ typedef struct {
 #define NNP_MLP_F16X1 2
 
 /* Creates the immutable model: copies parameters, uploads weights (and the derived fp16 hi/lo tile
- * images) to the current CUDA device.  Limits: n_species <= 8, nShfR <= 16, nShfA*nShfZ == 32,
- * hidden widths multiples of 16 and <= 256, n_layers <= 4  -> otherwise NNP_ERR_UNSUPPORTED.
+ * images) to the current CUDA device.  Limits: n_species <= 8, nShfR == 16, nShfA == 4, nShfZ == 8 (the kernels' lane
+ * mappings), hidden widths multiples of 16 and <= 256, n_layers <= 4  -> otherwise NNP_ERR_UNSUPPORTED.
  * The tensor-core modes additionally need n_layers == 4, hidden widths multiples of 32 and |w| < 6e4
- * (fp16 range); a model outside that runs in NNP_MLP_FP32_SIMT and set_mlp_mode(F16*) returns UNSUPPORTED. */
+ * (fp16 range); a model outside that runs in NNP_MLP_FP32_SIMT (about 8x slower MLP stage) and set_mlp_mode(F16*)
+ * returns UNSUPPORTED -- nnp_model_default_mlp_mode() tells which arithmetic a new workspace of the model starts in. */
 int nnp_model_create(const nnp_aev_params* aev, const nnp_mlp_desc* nets /* HOST [n_species] */, nnp_model** out);
 /* Ensemble of n_members (1..8) networks per element, E = mean of the members' energies -- ANI-2x "is an ensemble of 8
  * networks".  nets: HOST [n_members][n_species], member-major; every member must have the same
  * layer widths per species.  nnp_model_create is the n_members = 1 case.  All members share one AEV.
- * The members of a tile hand over in order between the co-resident CTAs of ONE persistent kernel: an ensemble evaluation
- * needs the device to itself while its MLP kernel runs (do not run ensemble workspaces concurrently on several streams). */
+ * The members of a tile hand over in order between the co-resident CTAs of ONE persistent kernel, so two ensemble MLP
+ * kernels must not share the device.  The library enforces that: ensemble evaluations of ALL workspaces of the process
+ * are ordered across streams with an event (each waits for the previous ensemble MLP launch), so workspaces on several
+ * streams are safe to use concurrently -- their MLP stages simply do not overlap.  Not enforced while a stream is being
+ * captured into a CUDA graph: do not replay ensemble graphs concurrently on several streams. */
 int nnp_model_create_ensemble(const nnp_aev_params* aev, const nnp_mlp_desc* nets, int32_t n_members, nnp_model** out);
 int nnp_model_destroy(nnp_model*);
 int nnp_model_aev_length(const nnp_model*);
+/* NNP_MLP_F16X3 if the model has tensor-core weight images, NNP_MLP_FP32_SIMT if its networks fall outside the tensor-core
+ * shape limits above (the fall-back is not silent: ask here); NNP_ERR_INVALID_ARG for a NULL model. */
+int nnp_model_default_mlp_mode(const nnp_model*);
 
 /* Allocates all device scratch for up to max_ml_atoms ML atoms out of up to max_atoms atoms.
  * cuda_stream: a cudaStream_t (0 = legacy default stream).  Neighbour-row capacities default to
@@ -162,7 +169,10 @@ int nnp_eval(nnp_workspace*, int64_t n_atoms, const float* d_pos, const int32_t*
 
 /* Same evaluation with HOST buffers: copies inputs to workspace-owned device buffers, runs nnp_eval,
  * copies energy and forces back and synchronises the stream.  h_ml_index may be NULL.  This is the
- * end-to-end entry point a host MD engine (GROMACS nnpot) would call. */
+ * end-to-end entry point a host MD engine (GROMACS nnpot) would call.  Per call: ONE host-to-device
+ * copy (positions) and ONE device-to-host copy (forces); the energy arrives through a mapped pinned word the output
+ * kernel writes; atomic numbers and the ML index are compared with the copy of the previous call and uploaded only when
+ * they changed (a change also ends any binning reuse: the next evaluation bins afresh). */
 int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int32_t* h_Z, const float box[9],
                   int32_t pbc, const int32_t* h_ml_index, int64_t n_ml, double* h_energy, float* h_forces);
 
@@ -173,7 +183,9 @@ int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int
  *   nnp_link_place : writes r_L = r_ML + d (r_MM - r_ML)/|r_MM - r_ML| into rows n_atoms.. of d_pos (call before nnp_eval)
  *   nnp_link_spread: adds the chain-rule shares of the link rows of d_forces onto the bonded atoms and zeroes the
  *                    link rows (call after nnp_eval): F_ML += F_L - (d/l)(F_L - u(u.F_L)), F_MM += (d/l)(F_L - u(u.F_L))
- * d = link distance in Angstrom (PAPER.md default 1.0); bond vectors take the minimum image when pbc != 0 (box as in
+ * d = link distance in the SAME length unit as d_pos and box (PAPER.md default: 1.0 Angstrom; the link kernels take no
+ * workspace and do no unit conversion -- a caller working in nm with nnp_workspace_set_units(10, ...) passes d = 0.1);
+ * bond vectors take the minimum image when pbc != 0 (box as in
  * nnp_eval, HOST: orthorhombic or GROMACS-style triclinic).  d_link_ml / d_link_mm: DEVICE [n_links] int32 atom indices < n_atoms.  Asynchronous on the given
  * cudaStream_t; out-of-range indices and zero-length bonds are skipped.  Returns NNP_ERR_INVALID_ARG / _BOX_UNSUPPORTED
  * for bad arguments. */
@@ -205,7 +217,9 @@ int nnp_debug_atomic_energies(nnp_workspace*, float* h_e);
 int nnp_debug_counters(nnp_workspace*, int64_t* launches);
 /* SM-clock ticks of the tensor-core MLP kernel's CTA 0 over its first 32 GEMM rounds (HOST h_ticks[64]): even
  * entries = operand handed to the MMA warp, odd entries = accumulator complete.  Differences give the time spent
- * in epilogues (odd -> next even) and in MMA rounds (even -> odd); used by the profiling notes. */
+ * in epilogues (odd -> next even) and in MMA rounds (even -> odd); used by the profiling notes.  Profiling scaffolding:
+ * only a library built with -DNNP_TC_TIMELINE (NNP_EXTRA_NVCC_FLAGS of build.py) records it; the default build carries no
+ * instrumentation in the kernel and returns NNP_ERR_UNSUPPORTED here. */
 int nnp_debug_mlp_timeline(nnp_workspace*, int64_t* h_ticks);
 /* Stage timing of nnp_eval with CUDA events on the workspace stream.  set_profiling(1) makes every later
  * nnp_eval record an event at each stage boundary (not capturable into a CUDA graph while on);

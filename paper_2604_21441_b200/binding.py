@@ -19,7 +19,7 @@ EXPORTS = [
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_workspace_set_bin_reuse", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
-    "nnp_debug_fp32_peak",
+    "nnp_debug_fp32_peak", "nnp_model_default_mlp_mode",
 ]
 
 
@@ -63,6 +63,7 @@ def lib():
         L.nnp_model_create_ensemble.argtypes = [vp, vp, i32, C.POINTER(vp)]
         L.nnp_model_destroy.argtypes = [vp]
         L.nnp_model_aev_length.argtypes = [vp]
+        L.nnp_model_default_mlp_mode.argtypes = [vp]
         L.nnp_workspace_create.argtypes = [vp, i64, i64, vp, C.POINTER(vp)]
         L.nnp_workspace_destroy.argtypes = [vp]
         L.nnp_workspace_set_mlp_mode.argtypes = [vp, i32]
@@ -115,6 +116,10 @@ def nnp_model_destroy(model):
 
 def nnp_model_aev_length(model):
     return lib().nnp_model_aev_length(model)
+
+
+def nnp_model_default_mlp_mode(model):
+    return lib().nnp_model_default_mlp_mode(model)
 
 
 def nnp_workspace_create(model, max_atoms, max_ml_atoms, cuda_stream):
@@ -267,6 +272,7 @@ class Model:
         self.n_members = M
         self.handle = h
         self.aev_length = nnp_model_aev_length(h)
+        self.default_mlp_mode = nnp_model_default_mlp_mode(h)   # NNP_MLP_FP32_SIMT: networks outside the tensor-core limits
 
     def close(self):
         if getattr(self, "handle", None):

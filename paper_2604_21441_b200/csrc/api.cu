@@ -18,8 +18,8 @@ extern "C" const char* nnp_strerror(int code) {
     case NNP_OK: return "ok";
     case NNP_ERR_INVALID_ARG: return "invalid argument";
     case NNP_ERR_UNKNOWN_SPECIES: return "ML atom with an atomic number that has no species slot or no network";
-    case NNP_ERR_BOX_UNSUPPORTED: return "box must be orthorhombic with positive lengths";
-    case NNP_ERR_CAPACITY: return "neighbour row or tile capacity exceeded";
+    case NNP_ERR_BOX_UNSUPPORTED: return "box must be orthorhombic or GROMACS-style triclinic (lower triangular, within the shape limits, >= 3 cut-off wide cells per dimension when skewed) with positive lengths";
+    case NNP_ERR_CAPACITY: return "neighbour row, cell buffer or tile capacity exceeded";
     case NNP_ERR_COINCIDENT: return "two ML atoms coincide";
     case NNP_ERR_CUDA: return "CUDA error or no CUDA device";
     case NNP_ERR_UNSUPPORTED: return "descriptor or network shape outside the kernels' range";
@@ -149,6 +149,11 @@ extern "C" int nnp_model_destroy(nnp_model* m) {
 
 extern "C" int nnp_model_aev_length(const nnp_model* m) { return m ? m->aev.L : NNP_ERR_INVALID_ARG; }
 
+extern "C" int nnp_model_default_mlp_mode(const nnp_model* m) {
+  if (!m) return NNP_ERR_INVALID_ARG;
+  return m->tc ? NNP_MLP_F16X3 : NNP_MLP_FP32_SIMT;
+}
+
 // ------------------------------------------------------------------------------------------------ workspace
 template <class T>
 static bool dmalloc(T** p, size_t n) {
@@ -165,8 +170,11 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   void* ptrs[] = {ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
                   ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->pos_scaled, ws->hd_pos, ws->hd_Z, ws->hd_ml,
-                  ws->hd_energy, ws->hd_forces};
+                  ws->hd_forces};
   for (void* p : ptrs) if (p) cudaFree(p);
+  if (ws->hd_energy) cudaFreeHost(ws->hd_energy);
+  if (ws->hz_copy) cudaFreeHost(ws->hz_copy);
+  if (ws->hml_copy) cudaFreeHost(ws->hml_copy);
   cudaGetLastError();
   delete ws;
   return NNP_OK;
@@ -211,8 +219,15 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
             dmalloc(&ws->dbuf[0], nr * HP) && dmalloc(&ws->dbuf[1], nr * HP) && dmalloc(&ws->e_atom, nr) &&
             dmalloc(&ws->facc, 3 * nm) && dmalloc(&ws->epart, nm / 256 + 2) && dmalloc(&ws->ticket, 1) && dmalloc(&ws->wcentre, 9 * nm) &&
             dmalloc(&ws->wblk, 9 * (nm / 256 + 2)) && dmalloc(&ws->pos_scaled, 3 * (size_t)max_atoms) && dmalloc(&ws->hd_pos, 3 * (size_t)max_atoms) &&
-            dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) && dmalloc(&ws->hd_energy, 1) &&
+            dmalloc(&ws->hd_Z, (size_t)max_atoms) && dmalloc(&ws->hd_ml, nm) &&
             dmalloc(&ws->hd_forces, 3 * (size_t)max_atoms);
+  if (ok) {   // host side of nnp_eval_host: the mapped energy word and the pinned copies of Z / ml_index of the last call
+    ok = cudaHostAlloc((void**)&ws->hd_energy, sizeof(double), cudaHostAllocMapped) == cudaSuccess &&
+         cudaHostGetDevicePointer((void**)&ws->hd_energy_dev, ws->hd_energy, 0) == cudaSuccess &&
+         cudaHostAlloc((void**)&ws->hz_copy, sizeof(int32_t) * std::max<size_t>((size_t)max_atoms, 1), cudaHostAllocDefault) == cudaSuccess &&
+         cudaHostAlloc((void**)&ws->hml_copy, sizeof(int32_t) * std::max<size_t>(nm, 1), cudaHostAllocDefault) == cudaSuccess;
+    if (ok) *ws->hd_energy = 0.0;
+  }
   if (ok) ok = (tc_workspace_create(ws) == NNP_OK);
   if (!ok || cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); nnp_workspace_destroy(ws); return NNP_ERR_CUDA; }
   *out = ws;
@@ -364,14 +379,27 @@ extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_
   if (h_ml && (n_ml < 0 || n_ml > ws->max_ml)) return NNP_ERR_INVALID_ARG;
   cudaStream_t st = ws->stream;
   CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
-  CU_OK(cudaMemcpyAsync(ws->hd_Z, h_Z, sizeof(int32_t) * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
-  if (h_ml) CU_OK(cudaMemcpyAsync(ws->hd_ml, h_ml, sizeof(int32_t) * (size_t)n_ml, cudaMemcpyHostToDevice, st));
-  int rc = nnp_eval(ws, n_atoms, ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml, ws->hd_energy,
+  // atomic numbers and the ML index rarely change between MD steps: they are compared with the host copy of the last
+  // call and uploaded only when different (the comparison also makes binning reuse safe for this entry point: the
+  // device buffers are always the same, so pointer identity alone would say "same atoms" -- a change bins afresh)
+  const size_t zb = sizeof(int32_t) * (size_t)n_atoms, mb = h_ml ? sizeof(int32_t) * (size_t)n_ml : 0;
+  const bool z_same = ws->hz_valid && ws->hz_n == n_atoms && (zb == 0 || memcmp(ws->hz_copy, h_Z, zb) == 0);
+  const bool ml_same = ws->hml_valid && ws->hml_n == (h_ml ? n_ml : -1) && (mb == 0 || memcmp(ws->hml_copy, h_ml, mb) == 0);
+  if (!z_same) {
+    if (zb) { memcpy(ws->hz_copy, h_Z, zb); CU_OK(cudaMemcpyAsync(ws->hd_Z, ws->hz_copy, zb, cudaMemcpyHostToDevice, st)); }
+    ws->hz_n = n_atoms; ws->hz_valid = 1;
+  }
+  if (!ml_same) {
+    if (mb) { memcpy(ws->hml_copy, h_ml, mb); CU_OK(cudaMemcpyAsync(ws->hd_ml, ws->hml_copy, mb, cudaMemcpyHostToDevice, st)); }
+    ws->hml_n = h_ml ? n_ml : -1; ws->hml_valid = 1;
+  }
+  if (!z_same || !ml_same) ws->reuse_left = 0;
+  int rc = nnp_eval(ws, n_atoms, ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml, ws->hd_energy_dev,
                     ws->hd_forces);
   if (rc) return rc;
-  CU_OK(cudaMemcpyAsync(h_energy, ws->hd_energy, sizeof(double), cudaMemcpyDeviceToHost, st));
   CU_OK(cudaMemcpyAsync(h_forces, ws->hd_forces, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyDeviceToHost, st));
   CU_OK(cudaStreamSynchronize(st));
+  *h_energy = *ws->hd_energy;   // mapped pinned word, written by the output kernel (or the memset of an empty subset)
   return NNP_OK;
 }
 
@@ -383,6 +411,7 @@ extern "C" int nnp_status(nnp_workspace* ws) {
   CU_OK(cudaMemset(ws->flags, 0, sizeof(int)));
   if (f & FLAG_STALE) ws->reuse_left = 0;   // whatever else went wrong: the next evaluation bins afresh
   if (f & FLAG_CAP) ws->slow_prep = 1;      // (possibly) a cell beyond the fast binning's buffer: general binning from now on
+  if (f & FLAG_TIMEOUT) return NNP_ERR_CUDA;   // a kernel gave up waiting for its producer (force.cu): outputs invalid
   if (f & FLAG_ARG) return NNP_ERR_INVALID_ARG;
   if (f & FLAG_SPECIES) return NNP_ERR_UNKNOWN_SPECIES;
   if (f & FLAG_CAP) return NNP_ERR_CAPACITY;

@@ -2,11 +2,12 @@
 // deterministic force assembly F_a = sum_j (p_aj - p_ja)  (eq. 2 F = -grad E;
 // BASELINE.json north_star stage (4); formulas SURVEY.md Appendix A "Forces").
 //
-// K7: one warp per centre.  Radial: lane <-> neighbour.  Angular: lane <-> neighbour j (P = 1, 2 or 4 lanes
-// per j share the partner loop), each lane accumulating ONLY its own p_ij over all partners k, so no
-// cross-lane scatter is needed; every unordered triplet is therefore visited from both ends.
-// K8: p_ij is converted to 2^-40 fixed point and accumulated with 64-bit integer atomics (integer addition
-// is associative, so the result does not depend on the arrival order): forces are bitwise reproducible.
+// K7: one warp per centre.  Radial: lane <-> neighbour.  Angular: lanes hold the angular neighbours; every unordered
+// triplet {j,k} is evaluated ONCE (round-robin pairing: in round m lane j pairs with k = (j + m) mod n), lane j keeps
+// its own share p_ij and hands p_ik to lane k by shuffle; more than 32 angular neighbours fall back to a loop that
+// visits every pair from both ends.
+// K8: p_ij is converted to 2^-40 fixed point and accumulated with 64-bit INTEGER atomics (integer addition is
+// associative, so the result does not depend on the arrival order): forces are bitwise reproducible.
 #include "aev_common.cuh"
 
 namespace nnp {
@@ -74,12 +75,15 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
                const float* daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre,
-               const int* tile_done, int done_target) {
+               const int* tile_done, int done_target, int* __restrict__ flags) {
   __shared__ WarpEnv env[AEV_WARPS];
+  __shared__ int timed_out;
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
   __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block, times TILE_M
   pdl_trigger();
   if (!tile_done) pdl_wait();   // with per-tile flags the MLP kernel is NOT awaited as a whole (see below)
+  if (threadIdx.x == 0) timed_out = 0;
+  __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   if (threadIdx.x < MAX_S * MAX_S) {
     const int sa = threadIdx.x / MAX_S, sb = threadIdx.x % MAX_S;
@@ -106,10 +110,14 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
           asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(tile_done + tw) : "memory");
           if (seen < done_target) __nanosleep(500);
         } while (seen < done_target && ++spins < (1 << 22));   // ~2 s: a flag that never comes must not hang the GPU
+        // ... and must not pass silently either: the evaluation is flagged (nnp_status -> NNP_ERR_CUDA) and the block's
+        // centres are skipped -- their dE/dAEV rows are not there
+        if (seen < done_target) { atomicOr(flags, FLAG_TIMEOUT); atomicExch(&timed_out, 1); }
       }
     }
   }
   __syncthreads();
+  if (timed_out) return;
   const int ip = blockIdx.x * AEV_WARPS + w;
   if (ip >= n_ml) return;
   WarpEnv& e = env[w];
@@ -421,11 +429,11 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
     if (ws->d_virial)
       launch_pdl(done != nullptr, ws->stream, k_aev_backward<true>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
                  ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
-                 ws->facc, ws->wcentre, done, ws->tile_done_target);
+                 ws->facc, ws->wcentre, done, ws->tile_done_target, ws->flags);
     else
       launch_pdl(done != nullptr, ws->stream, k_aev_backward<false>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
                  ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
-                 ws->facc, nullptr, done, ws->tile_done_target);
+                 ws->facc, nullptr, done, ws->tile_done_target, ws->flags);
     prof_mark(ws, 4);
     launch_pdl(!ws->profiling, ws->stream, k_force_out, dim3((unsigned)((n_ml + 255) / 256)), dim3(256), 0, ws->spos, ws->facc,
                d_ml, (int)n_ml, d_forces, ws->groups, ws->e_atom, ws->epart, ws->ticket, d_energy, ws->wcentre, ws->wblk,

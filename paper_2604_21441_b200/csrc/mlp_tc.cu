@@ -18,6 +18,7 @@
 // (measured against the fp64 oracle in DESIGN.md).  NNP_MLP_F16X1 keeps only hi*hi.
 #include <cuda_fp16.h>
 #include <string.h>
+#include <mutex>
 #include <vector>
 #include "nnp_internal.h"
 
@@ -296,8 +297,14 @@ __device__ __forceinline__ void tc_store_act(uint32_t abuf, int row, int j, cons
   }
 }
 
-// SM-clock timeline of CTA 0's first rounds (debug export nnp_debug_mlp_timeline): where a tile's time goes.
+// SM-clock timeline of CTA 0's first rounds (debug export nnp_debug_mlp_timeline): where a tile's time goes.  Profiling
+// scaffolding: compiled in only with -DNNP_TC_TIMELINE (the product kernel carries no instrumentation).
+#ifdef NNP_TC_TIMELINE
 __device__ long long g_tc_timeline[64];
+#define TC_STAMP() do { if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64(); } while (0)
+#else
+#define TC_STAMP() do { } while (0)
+#endif
 
 template <int NPASS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
@@ -451,7 +458,9 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
     const int q = warp & 3, part = warp >> 2, row = q * 32 + lane;
     const uint32_t tlane = tmem + ((uint32_t)(q * 32) << 16);
     uint32_t fph = 0, buf = 1;
+#ifdef NNP_TC_TIMELINE
     int tl = 0;   // timeline slot (block 0, thread 0 only): even = operand handed to the MMA warp, odd = accumulator back
+#endif
     // Hand-over protocol.  The A operand goes to the MMA warp PANEL BY PANEL (64 columns): every thread arrives once a
     // round on each of the four panel barriers, as soon as its share of the panel is in shared memory, so the MMAs of
     // the next GEMM start on panel 0 while this epilogue is still producing panels 1-3.  That GEMM accumulates into the
@@ -460,13 +469,13 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
     auto arrive_panel = [&](int i) {
       tc_fence_before();
       fence_proxy_async();
-      if (i == 3 && blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
+      if (i == 3) TC_STAMP();
       mbar_arrive(bar_panel + 8 * i);
     };
     auto arrive_all = [&]() {
       tc_fence_before();
       fence_proxy_async();
-      if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
+      TC_STAMP();
 #pragma unroll
       for (int i = 0; i < 4; ++i) mbar_arrive(bar_panel + 8 * i);
     };
@@ -477,7 +486,7 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       fph ^= 1;
       asm volatile("bar.sync 2, %0;" ::"n"(TC_EPI_WARPS * 32) : "memory");
       tc_fence_after();
-      if (blockIdx.x == 0 && threadIdx.x == 0 && tl < 64) g_tc_timeline[tl++] = clock64();
+      TC_STAMP();
     };
     uint32_t* const cs1 = cscr + (size_t)blockIdx.x * TC_CSCR_WORDS;   // CELU' of layer 1: [chunk j][2][128 rows][4 words]
     uint32_t* const cs2 = cs1 + TC_CW1 * 128;
@@ -847,7 +856,39 @@ void tc_workspace_destroy(nnp_workspace* ws) {
 }
 
 int tc_read_timeline(long long* h64) {
+#ifdef NNP_TC_TIMELINE
   return cudaMemcpyFromSymbol(h64, g_tc_timeline, sizeof(long long) * 64) == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
+#else
+  (void)h64;
+  return NNP_ERR_UNSUPPORTED;   // built without -DNNP_TC_TIMELINE
+#endif
+}
+
+// Ensemble hand-over guard.  The members of a tile hand over between the CO-RESIDENT CTAs of one persistent launch: a
+// CTA spins on done[tile] until the CTA holding the previous member releases it.  Two such launches running at the same
+// time on different streams could each hold SMs the other's awaited CTA needs -- a deadlock.  The library therefore
+// orders ensemble MLP launches across ALL workspaces of the process: every launch waits (cudaStreamWaitEvent) for the
+// previous ensemble launch, whatever stream that was on, and records the event the next one waits for.  (Skipped while
+// the stream is being captured into a CUDA graph: an event recorded outside the capture cannot be waited on inside it --
+// replaying ensemble graphs concurrently on several streams stays the caller's responsibility.)
+namespace {
+std::mutex g_ens_mutex;
+cudaEvent_t g_ens_event = nullptr;
+bool g_ens_recorded = false;
+}  // namespace
+
+static void ensemble_guard_before(cudaStream_t st) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return; }
+  std::lock_guard<std::mutex> lk(g_ens_mutex);
+  if (g_ens_recorded) cudaStreamWaitEvent(st, g_ens_event, 0);
+}
+static void ensemble_guard_after(cudaStream_t st) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); return; }
+  std::lock_guard<std::mutex> lk(g_ens_mutex);
+  if (!g_ens_event && cudaEventCreateWithFlags(&g_ens_event, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); g_ens_event = nullptr; return; }
+  if (cudaEventRecord(g_ens_event, st) == cudaSuccess) g_ens_recorded = true; else cudaGetLastError();
 }
 
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
@@ -860,6 +901,9 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   TcPackAll pall;
   for (int mem = 0; mem < MAX_MEMBERS; ++mem)
     for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
+  const bool ens = m->n_members > 1;
+  if (ens) ensemble_guard_before(ws->stream);
+  // (a wait on another stream's event in front of the launch: no programmatic overlap with the predecessor then)
   const bool pdl = !ws->profiling;
   launch_pdl(pdl, ws->stream, k_tc_pack_w1, dim3(32, m->aev.S, m->n_members), dim3(256), 0, tm->d_nets, ws->groups, pall,
              tw->key, tw->done, ws->max_tiles);
@@ -872,6 +916,7 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
   else
     launch_pdl(pdl, ws->stream, k_mlp_tc<3>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[0], tm->d_nets, tm->d_tabs,
                tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale, tw->cscr);
+  if (ens) ensemble_guard_after(ws->stream);
   return 2;
 }
 

@@ -23,7 +23,7 @@ constexpr uint32_t JMASK = (1u << JBITS) - 1u;
 constexpr int FIX_SHIFT = 40;     // fixed-point scale 2^40 for the int64 force accumulators (K8)
 
 // device-side sticky status bits
-enum : int { FLAG_ARG = 1, FLAG_SPECIES = 2, FLAG_CAP = 4, FLAG_COINCIDENT = 8, FLAG_STALE = 16 };
+enum : int { FLAG_ARG = 1, FLAG_SPECIES = 2, FLAG_CAP = 4, FLAG_COINCIDENT = 8, FLAG_STALE = 16, FLAG_TIMEOUT = 32 };
 
 // Descriptor constants, passed to kernels by value.
 struct AevConst {
@@ -185,7 +185,11 @@ struct nnp_workspace {
   int profiling;             // 1: record a CUDA event at every stage boundary of nnp_eval
   cudaEvent_t ev[8];         // 0 start, 1 after neighbour, 2 after AEV fwd, 3 after MLP, 4 after AEV bwd, 5 end
   // host-buffer entry point
-  float* hd_pos; int32_t* hd_Z; int32_t* hd_ml; double* hd_energy; float* hd_forces;
+  float* hd_pos; int32_t* hd_Z; int32_t* hd_ml; float* hd_forces;
+  double* hd_energy;         // mapped pinned HOST word the output kernel writes the energy to (hd_energy_dev = its device alias)
+  double* hd_energy_dev;
+  int32_t* hz_copy; int32_t* hml_copy;   // pinned host copies of Z / ml_index as last uploaded
+  int64_t hz_n, hml_n; int hz_valid, hml_valid;
 };
 
 namespace nnp {
