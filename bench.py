@@ -26,16 +26,35 @@ METRIC = "nnp_energy_force_atom_steps_per_s"
 UNIT = "atom-steps/s"
 WORKLOAD = "cfg2_water_8000 (24000 atoms, AEV 1008, H 1008-256-192-160-1 / O 1008-224-192-160-1)"
 N_POS_SETS = 16
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x FMA x max SM clock
+FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # unit counts x max SM clock: context only, the run MEASURES its peak
 # algorithmic FP32 work of the AEV kernels: per directed radial pair / per unordered triplet
 FLOP_FWD_PAIR, FLOP_FWD_TRIPLET = 16 * 6, 170
 FLOP_BWD_PAIR, FLOP_BWD_TRIPLET = 16 * 10, 350
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's main kernel, from the committed ncu full-set
-# capture profiles/r01h_launches.md (cfg-2 workload, F16X3, compact K); None where no capture exists for the mode.
-NCU_TRAFFIC_BYTES = {"neighbour": 0.502e6 + 0.491e6, "aev_forward": 8.08e6, "mlp": 18.33e6 + 0.413e6, "aev_backward": 20.98e6,
-                     "output": 1.07e6}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of each stage's kernels, from the committed summary of the
+    round's `ncu --set full` capture (profiles/r02_traffic.json names the command that made it).  No file -> no claim."""
+    if not os.path.exists(TRAFFIC_FILE):
+        return None, None
+    d = json.load(open(TRAFFIC_FILE))
+    return d.get("stage_bytes_per_launch"), "profiles/r02_traffic.json (" + d.get("how", "ncu --set full, per launch") + ")"
+
+
+def measured_fp32_peak(nnp, stream):
+    """Register-resident FMA loops of the library: scalar FFMA and packed FFMA2; the larger is the peak."""
+    out = {}
+    for name, v in (("ffma", 0), ("ffma2", 1)):
+        rc, t = nnp.nnp_debug_fp32_peak(stream, v)
+        if rc != 0:
+            raise RuntimeError(f"nnp_debug_fp32_peak failed: {rc}")
+        out[name] = t
+    out["used"] = max(out["ffma"], out["ffma2"])
+    out["nominal"] = FP32_PEAK_NOMINAL_TFLOPS
+    return out
 
 
 def peaks():
@@ -191,6 +210,7 @@ def run_ours(args, rank, world, local_rank):
     F = torch.zeros((n, 3), dtype=torch.float32, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     box = cfg["box"]
+    fp32 = measured_fp32_peak(nnp, torch.cuda.current_stream().cuda_stream)   # before the timed region
 
     def barrier():
         if dist is not None:
@@ -238,6 +258,40 @@ def run_ours(args, rank, world, local_rank):
         stage += ws.stage_times()     # waits for this step's last event
     ws.set_profiling(0)
 
+    # ---- the MLP stage in the other arithmetic / column modes (SURVEY.md section 8.d "report both": compact K and the
+    # dense K = 1008 -> 1024 shape "as ANI would run it"; F16X1 beside the default F16X3), stage-event timing as above
+    nH, nO = int((cfg["Z"] == 1).sum()), int((cfg["Z"] == 8).sum())
+    mlp_variants = None
+    plain_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1 and args.bin_reuse <= 1
+    if world == 1 and not args.no_extras and plain_build:
+        mlp_variants = {}
+        vsteps = min(args.steps, 20)
+        for label, mode, dense in (("f16x3_compact_k", nnp.NNP_MLP_F16X3, 0), ("f16x1_compact_k", nnp.NNP_MLP_F16X1, 0),
+                                   ("f16x3_dense_k", nnp.NNP_MLP_F16X3, 1), ("f16x1_dense_k", nnp.NNP_MLP_F16X1, 1)):
+            ws.set_mlp_mode(mode)
+            ws.set_dense_k(dense)
+            for t in range(3):
+                ws.eval(dpos[t], dZ, box, 1, None, E, F)
+            ws.set_profiling(1)
+            acc = np.zeros(5)
+            for k in range(vsteps):
+                flush.zero_()
+                ws.eval(dpos[k % N_POS_SETS], dZ, box, 1, None, E, F)
+                acc += ws.stage_times()
+            ws.set_profiling(0)
+            K1 = 1024 if dense else 160
+            fl = nH * mlp_flops_per_atom(cfg["nets"][1][0], K1) + nO * mlp_flops_per_atom(cfg["nets"][8][0], K1)
+            ms_mlp = float(acc[2] / vsteps)
+            mlp_variants[label] = {"mlp_ms": ms_mlp, "step_ms_stage_sum": float(acc.sum() / vsteps), "first_layer_k": K1,
+                                   "achieved_tflops": fl / (ms_mlp * 1e-3) / 1e12, "frac_of_tensor_peak": fl / (ms_mlp * 1e-3) / 1e12 / peaks()["bf16"],
+                                   "mma_per_counted_product": 3 if mode == nnp.NNP_MLP_F16X3 else 1}
+        ws.set_mlp_mode(nnp.NNP_MLP_F16X3)
+        ws.set_dense_k(0)
+        for t in range(2):
+            ws.eval(dpos[t], dZ, box, 1, None, E, F)
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+
     # ---- end to end: nnp_eval_host with pinned host buffers (H2D of pos/Z, D2H of E/F, sync inside the call)
     hpos = [torch.from_numpy(P[t]).pin_memory() for t in range(N_POS_SETS)]
     hZ = torch.from_numpy(cfg["Z"]).pin_memory()
@@ -265,15 +319,14 @@ def run_ours(args, rank, world, local_rank):
     e2e = world * n * args.steps / e2e_s
     stage_ms = stage / args.steps
     names = ["neighbour", "aev_forward", "mlp", "aev_backward", "output"]
-    nH, nO = int((cfg["Z"] == 1).sum()), int((cfg["Z"] == 8).sum())
     # compacted AEV width for an H/O-only system: 2 radial + 3 angular 32-column blocks (dense-K: all 32 blocks)
     Kc = 1024 if args.dense_k else 160
     mlp_flops = args.ensemble * (nH * mlp_flops_per_atom(cfg["nets"][1][0], Kc) + nO * mlp_flops_per_atom(cfg["nets"][8][0], Kc))
     work = {
         "neighbour": ("hbm", n * (16 + 32 + 8) + 4 * pairs_R + pairs_R // 4, pk["hbm"], "GB/s", 1e9),
-        "aev_forward": ("alu", pairs_R * FLOP_FWD_PAIR + triplets * FLOP_FWD_TRIPLET, FP32_PEAK_TFLOPS, "TFLOP/s", 1e12),
+        "aev_forward": ("alu", pairs_R * FLOP_FWD_PAIR + triplets * FLOP_FWD_TRIPLET, fp32["used"], "TFLOP/s", 1e12),
         "mlp": ("tensor", mlp_flops, pk["bf16"], "TFLOP/s", 1e12),
-        "aev_backward": ("alu", pairs_R * FLOP_BWD_PAIR + triplets * FLOP_BWD_TRIPLET, FP32_PEAK_TFLOPS, "TFLOP/s", 1e12),
+        "aev_backward": ("alu", pairs_R * FLOP_BWD_PAIR + triplets * FLOP_BWD_TRIPLET, fp32["used"], "TFLOP/s", 1e12),
         "output": ("hbm", n * (24 + 16 + 12), pk["hbm"], "GB/s", 1e9),
     }
     stages = {}
@@ -285,11 +338,20 @@ def run_ours(args, rank, world, local_rank):
     dom = names[int(np.argmax(stage_ms))]
     roof = dict(stages[dom])
     roof.pop("ms")
-    default_build = args.mlp_mode in ("default", "f16x3") and not args.dense_k and args.ensemble == 1 and args.bin_reuse <= 1
-    roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else "derived (DESIGN.md section 6)",
-                traffic=NCU_TRAFFIC_BYTES.get(dom) if default_build else None,
-                traffic_source="profiles/r01h_launches.md (ncu --set full, per launch)")
+    default_build = plain_build
+    traffic, traffic_src = ncu_traffic()
+    roof.update(kernel=dom, peak_source=pk["src"] if roof["bound"] != "alu" else
+                "measured in this run (nnp_debug_fp32_peak: register-resident FFMA / FFMA2 loops, best of 5)",
+                traffic=(traffic or {}).get(dom) if default_build else None, traffic_source=traffic_src)
+    if dom == "mlp":
+        roof["note"] = "F16X3 executes three MMAs per counted product: the creditable ceiling of this fraction is 1/3"
 
+    sweep = cpu_cfgs = None
+    if world == 1 and not args.no_extras and plain_build:
+        del ws
+        sweep = [{k: v for k, v in r.items() if k not in ("sweep", "metric", "unit")} for r in sweep_records(40, flush)]
+        if not args.no_cpu_baseline:
+            cpu_cfgs = cpu_oracle_records()
     cpu = None
     if world == 1 and not args.no_cpu_baseline and args.ensemble == 1:
         import oracle
@@ -313,22 +375,26 @@ def run_ours(args, rank, world, local_rank):
                    "bin_reuse": args.bin_reuse,
                    "radial_pairs": pairs_R, "triplets": triplets, "parallelism": f"replicas x{world}"},
         "ns_per_day_2fs": 0.1728 * args.steps / total_s,
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 12 * n + 8,
-                "ms_per_step": 1e3 * e2e_s / args.steps},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 12 * n, "d2h_bytes_per_step": 12 * n + 8,
+                "ms_per_step": 1e3 * e2e_s / args.steps,
+                "note": "nnp_eval_host: positions H2D, forces D2H, energy through a mapped pinned word; Z is uploaded only when it changed"},
         "gpu_launches": int(launches_per_step * args.steps),
         "clocks": clk, "roofline": roof, "stages": stages, "cpu_baseline": cpu,
+        "vs_cpu_baseline": (value / cpu["value"]) if cpu else None, "fp32_peak_tflops": fp32,
+        "mlp_variants": mlp_variants, "sweep": sweep, "cpu_oracle_configs": cpu_cfgs,
         "ms_per_step_min": float(ms.min()), "ms_per_step_median": float(np.median(ms)), "wall_s": wall}))
     if dist is not None:
         dist.destroy_process_group()
 
 
-def run_sweep(args):
-    """BASELINE.json's metric is quoted "vs water-box size": device-resident timing of every config (cfg 0-4), one JSON
-    line each (not the contract line; run explicitly with --sweep).  Positions cycle over 4 perturbed sets, L2 flushed."""
+def sweep_records(base_steps, flush=None):
+    """BASELINE.json's metric is quoted "vs water-box size": device-resident timing of every config (cfg 0-4), one record
+    each.  Positions cycle over 4 perturbed sets, L2 flushed between timed steps; plus the back-to-back (no flush)
+    latency per evaluation, the number that matters for the small ML regions of PAPER.md lines 108 / 140."""
     import torch
     import paper_2604_21441_b200 as nnp
-    torch.cuda.set_device(0)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    if flush is None:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     for k in range(5):
         cfg = gen.get_config(k)
         n = cfg["pos"].shape[0]
@@ -346,7 +412,7 @@ def run_sweep(args):
             ws.eval(dpos[t % 4], dZ, cfg["box"], 1, dml, E, F)
         torch.cuda.synchronize()
         assert ws.status() == 0
-        steps = args.steps if k < 3 else max(10, args.steps // 4)
+        steps = base_steps if k < 3 else max(10, base_steps // 4)
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         for i in range(steps):      # timed pass: no stage events (they would serialise the PDL-overlapped kernels)
             flush.zero_()
@@ -363,12 +429,59 @@ def run_sweep(args):
         ws.set_profiling(0)
         torch.cuda.synchronize()
         ms = np.array([a.elapsed_time(b) for a, b in ev])
-        print(json.dumps({"sweep": True, "metric": METRIC, "unit": UNIT, "config": {"workload": cfg["name"], "n_atoms": n, "n_ml": n_ml},
-                          "value": n_ml / (ms.mean() * 1e-3), "ms_per_step": float(ms.mean()), "ms_per_step_min": float(ms.min()),
-                          "ns_per_day_2fs": 0.1728 / (ms.mean() * 1e-3), "steps": steps,
-                          "stage_ms": dict(zip(["neighbour", "aev_forward", "mlp", "aev_backward", "output"],
-                                               [float(x) for x in stage / steps]))}), flush=True)
+        # back-to-back evaluations, no flush, one event pair around the lot: the per-evaluation latency of an MD loop
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nb = 4 * steps
+        e0.record()
+        for i in range(nb):
+            ws.eval(dpos[i % 4], dZ, cfg["box"], 1, dml, E, F)
+        e1.record()
+        torch.cuda.synchronize()
+        assert ws.status() == 0
+        yield {"sweep": True, "metric": METRIC, "unit": UNIT, "config": {"workload": cfg["name"], "n_atoms": n, "n_ml": n_ml},
+               "value": n_ml / (ms.mean() * 1e-3), "ms_per_step": float(ms.mean()), "ms_per_step_min": float(ms.min()),
+               "ns_per_day_2fs": 0.1728 / (ms.mean() * 1e-3), "steps": steps, "launches_per_step": int(ws.launches()),
+               "us_per_eval_back_to_back": 1e3 * e0.elapsed_time(e1) / nb,
+               "stage_ms": dict(zip(["neighbour", "aev_forward", "mlp", "aev_backward", "output"],
+                                    [float(x) for x in stage / steps]))}
         del ws, model
+
+
+def run_sweep(args):
+    import torch
+    torch.cuda.set_device(0)
+    for rec in sweep_records(args.steps):
+        print(json.dumps(rec), flush=True)
+
+
+def cpu_oracle_records(budget_1thread_s=25.0):
+    """the oracle as it stands (gcc -O2 -fopenmp, fp64, cell-list mode) on the box's host cores,
+    every config, all cores and one thread.  Evaluations per record are bounded so the whole leg stays under a minute;
+    cfg 3 on one thread (~4x cfg 2) is extrapolated from its all-core run and marked so."""
+    import oracle
+    all_cores = oracle.num_threads()
+    out = []
+    plan = {0: (20, 5), 4: (20, 5), 1: (3, 1), 2: (2, 1), 3: (1, 0)}      # cfg -> evaluations (all cores, one thread)
+    for k in (0, 1, 2, 3, 4):
+        cfg = gen.get_config(k)
+        ml = cfg["ml_index"]
+        n_ml = cfg["pos"].shape[0] if ml is None else len(ml)
+        om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+        rec = {"workload": cfg["name"], "n_ml": n_ml}
+        for label, threads, reps in (("all_cores", all_cores, plan[k][0]), ("one_thread", 1, plan[k][1])):
+            if reps == 0:
+                rec[label] = None
+                continue
+            oracle.set_num_threads(threads)
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nbr_mode=1)
+            dt = (time.perf_counter() - t0) / reps
+            rec[label] = {"threads": threads, "evaluations": reps, "ms_per_eval": 1e3 * dt, "atom_steps_per_s": n_ml / dt,
+                          "ns_per_day_2fs": 0.1728 / dt}
+        oracle.set_num_threads(all_cores)
+        out.append(rec)
+    return out
 
 
 def main():
@@ -383,6 +496,7 @@ def main():
     ap.add_argument("--bin-reuse", type=int, default=0, help="reuse the cell binning for N-1 of every N steps (0 = rebuild every step)")
     ap.add_argument("--skin", type=float, default=0.5, help="cell-width buffer in Angstrom for --bin-reuse")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extra records of the contract line (MLP variants, cfg 0-4 sweep, per-config oracle timings)")
     ap.add_argument("--sweep", action="store_true", help="time every BASELINE.json config (cfg 0-4), one extra JSON line each")
     ap.add_argument("--ref-budget-s", type=float, default=150.0, help="CPU seconds the reference arm may spend in total")
     args = ap.parse_args()

@@ -10,6 +10,8 @@ LIB = os.path.join(HERE, "libnnp_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-Xptxas", "-v"]
+# extra compile flags for profiling builds, e.g. NNP_EXTRA_NVCC_FLAGS=-DNNP_TC_TIMELINE (records the MLP kernel's timeline)
+FLAGS += os.environ.get("NNP_EXTRA_NVCC_FLAGS", "").split()
 
 
 def sources():
