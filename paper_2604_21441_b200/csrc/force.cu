@@ -21,36 +21,88 @@ __device__ __forceinline__ long long shfl_xor_ll(long long v, int o) {
 
 // Both shares of one unordered angular pair {j,k} of centre i: oj = dE_i/dr_j and ok = dE_i/dr_k contributions of the
 // 32 sub-features of the pair's species block (SURVEY.md Appendix A "Forces"; gb = this centre's dE/dAEV pieces).
+// Per-warp staging of one centre's environment for the backward pass.
+struct BwdEnv {
+  float4 u[RCAP_MAX];      // radial neighbours: unit vector (x,y,z) and R
+  float4 ua[ACAP_MAX];     // angular neighbours (subset, same order): unit vector and R
+  float fA[ACAP_MAX];      // f_C(R; Rca)
+  float dfA[ACAP_MAX];     // f_C'(R; Rca)
+  uint8_t slotR[RCAP_MAX];
+  uint8_t slotA[ACAP_MAX];
+  uint8_t ainv[RCAP_MAX];  // position in the radial row -> index among the angular neighbours, 255 = not one
+};
+
+__device__ __forceinline__ void bwd_load_env(const AevConst& c, const GridInfo* __restrict__ g,
+                                             const float4* __restrict__ spos, const uint32_t* __restrict__ rowR,
+                                             const uint8_t* __restrict__ rowA, int nR, int nA, float4 ci, int lane,
+                                             BwdEnv& e) {
+  float ev[9];   // cell edge vectors (orthorhombic: diagonal)
+#pragma unroll
+  for (int k = 0; k < 9; ++k) ev[k] = g->ev[k];
+  for (int q0 = 0; q0 < nR; q0 += 32) {
+    const int q = q0 + lane;
+    if (q < nR) {
+      const uint32_t ent = rowR[q];
+      const int jp = (int)(ent & JMASK);
+      const int oc = (int)(ent >> JBITS);
+      const float4 pj = spos[jp];
+      float sx, sy, sz;
+      cell_shift(ev, (oc & 3) - 1, ((oc >> 2) & 3) - 1, ((oc >> 4) & 3) - 1, sx, sy, sz);
+      const float dx = (pj.x - ci.x) + sx, dy = (pj.y - ci.y) + sy, dz = (pj.z - ci.z) + sz;
+      const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+      const float rinv = rsqrtf(d2);
+      e.u[q] = make_float4(dx * rinv, dy * rinv, dz * rinv, d2 * rinv);
+      e.slotR[q] = (uint8_t)((__float_as_int(pj.w) >> 28) & 7);
+      e.ainv[q] = 255;
+    }
+  }
+  __syncwarp();
+  for (int a0 = 0; a0 < nA; a0 += 32) {
+    const int a = a0 + lane;
+    if (a < nA) {
+      const int p = rowA[a];
+      const float4 v = e.u[p];
+      float f, df;
+      cutoff(fminf(v.w, c.Rca), c.inv_Rca, f, df);
+      e.ua[a] = v; e.fA[a] = f; e.dfA[a] = df; e.slotA[a] = e.slotR[p]; e.ainv[p] = (uint8_t)a;
+    }
+  }
+  __syncwarp();
+}
+
 struct PairShares { float jx, jy, jz, kx, ky, kz; };
-__device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, const float4* gb, float4 uj,
+// Packed fp32 arithmetic (fma.rn.f32x2, sm_100): the theta shifts are handled two per instruction, and the dot products
+// over z of the 4 x 8 dE/dAEV block accumulate two partial sums per instruction -- the kernel is bound by issue slots.
+__device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, const float4* gb, int gs, float4 uj,
                                                   float fj, float dfj, float4 uk, float fk, float dfk) {
   const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
   const float cc = c.cTheta * u;
   const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
   const float kd = 0.5f * c.zeta * c.cTheta / ss;            // -0.5 zeta dtheta/du
-  float F1[NSHFZ], dF1[NSHFZ];
+  const float2 cc2 = make_float2(cc, cc), ss2 = make_float2(ss, ss), ncc2 = make_float2(-cc, -cc);
+  const float2 h2 = make_float2(0.5f, 0.5f), kd2 = make_float2(kd, kd);
+  float2 F1[NSHFZ / 2], dF1[NSHFZ / 2];                       // pairs over z: (z, z + 1)
 #pragma unroll
-  for (int z = 0; z < NSHFZ; ++z) {
-    const float cosd = fmaf(cc, c.cosZ[z], ss * c.sinZ[z]);
-    const float sind = fmaf(ss, c.cosZ[z], -cc * c.sinZ[z]);
-    const float B = fmaxf(fmaf(0.5f, cosd, 0.5f), 1e-30f);    // floor keeps lg2 finite (B^(zeta-1) -> 0 or 1)
-    const float Bm = ex2f(zm1 * lg2f(B));                     // B^(zeta-1): two MUFU ops
-    F1[z] = Bm * B;
-    dF1[z] = kd * Bm * sind;                                  // dF1/du
+  for (int zp = 0; zp < NSHFZ / 2; ++zp) {
+    const float2 cz = make_float2(c.cosZ[2 * zp], c.cosZ[2 * zp + 1]), sz = make_float2(c.sinZ[2 * zp], c.sinZ[2 * zp + 1]);
+    const float2 cosd = __ffma2_rn(cc2, cz, __fmul2_rn(ss2, sz));
+    const float2 sind = __ffma2_rn(ss2, cz, __fmul2_rn(ncc2, sz));
+    float2 B = __ffma2_rn(h2, cosd, h2);
+    B.x = fmaxf(B.x, 1e-30f); B.y = fmaxf(B.y, 1e-30f);       // floor keeps lg2 finite (B^(zeta-1) -> 0 or 1)
+    const float2 Bm = make_float2(ex2f(zm1 * lg2f(B.x)), ex2f(zm1 * lg2f(B.y)));   // B^(zeta-1): two MUFU ops each
+    F1[zp] = __fmul2_rn(Bm, B);
+    dF1[zp] = __fmul2_rn(__fmul2_rn(kd2, Bm), sind);          // dF1/du
   }
   const float Rbar = 0.5f * (uj.w + uk.w);
   float S0 = 0.f, S1 = 0.f, sV = 0.f;
 #pragma unroll
   for (int a = 0; a < NSHFA; ++a) {
-    const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
-    float Wv = g0.x * F1[0], V = g0.x * dF1[0];
-    Wv = fmaf(g0.y, F1[1], Wv); V = fmaf(g0.y, dF1[1], V);
-    Wv = fmaf(g0.z, F1[2], Wv); V = fmaf(g0.z, dF1[2], V);
-    Wv = fmaf(g0.w, F1[3], Wv); V = fmaf(g0.w, dF1[3], V);
-    Wv = fmaf(g1.x, F1[4], Wv); V = fmaf(g1.x, dF1[4], V);
-    Wv = fmaf(g1.y, F1[5], Wv); V = fmaf(g1.y, dF1[5], V);
-    Wv = fmaf(g1.z, F1[6], Wv); V = fmaf(g1.z, dF1[6], V);
-    Wv = fmaf(g1.w, F1[7], Wv); V = fmaf(g1.w, dF1[7], V);
+    const float4 g0 = gb[(2 * a) * gs], g1 = gb[(2 * a + 1) * gs];
+    float2 W2 = __fmul2_rn(make_float2(g0.x, g0.y), F1[0]), V2 = __fmul2_rn(make_float2(g0.x, g0.y), dF1[0]);
+    W2 = __ffma2_rn(make_float2(g0.z, g0.w), F1[1], W2); V2 = __ffma2_rn(make_float2(g0.z, g0.w), dF1[1], V2);
+    W2 = __ffma2_rn(make_float2(g1.x, g1.y), F1[2], W2); V2 = __ffma2_rn(make_float2(g1.x, g1.y), dF1[2], V2);
+    W2 = __ffma2_rn(make_float2(g1.z, g1.w), F1[3], W2); V2 = __ffma2_rn(make_float2(g1.z, g1.w), dF1[3], V2);
+    const float Wv = W2.x + W2.y, V = V2.x + V2.y;
     const float x = Rbar - c.ShfA[a];
     const float F2 = ex2f(-c.etaA_l2e * x * x);
     const float WF = Wv * F2;
@@ -70,16 +122,18 @@ __device__ __forceinline__ PairShares pair_shares(const AevConst& c, float zm1, 
 }
 
 template <bool VIRIAL>
-__global__ void __launch_bounds__(AEV_WARPS * 32, 32 / AEV_WARPS)
+// 3 blocks per SM: 80 registers.  (At 4 blocks / 64 registers the packed-arithmetic version spills ~250 bytes per thread
+// inside the triplet loop -- local-memory loads are long-scoreboard stalls: 95 us against 86 us.)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 3)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
                const float* daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre,
                const int* tile_done, int done_target, int* __restrict__ flags) {
-  __shared__ WarpEnv env[AEV_WARPS];
+  __shared__ BwdEnv env[AEV_WARPS];
   __shared__ int timed_out;
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
-  __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block, times TILE_M
+  __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block
   pdl_trigger();
   if (!tile_done) pdl_wait();   // with per-tile flags the MLP kernel is NOT awaited as a whole (see below)
   if (threadIdx.x == 0) timed_out = 0;
@@ -89,7 +143,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     const int sa = threadIdx.x / MAX_S, sb = threadIdx.x % MAX_S;
     const int s1 = min(sa, sb), s2 = max(sa, sb);
     int off = 0;
-    if (s2 < c.S) { const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)]; off = max(cp, 0) * (BLK / 4) * TILE_M; }
+    if (s2 < c.S) { const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)]; off = max(cp, 0) * (BLK / 4); }
     pairoff[threadIdx.x] = off;
   }
   // Overlap with the MLP kernel (programmatic dependent launch): this grid may start while the persistent MLP CTAs
@@ -120,16 +174,20 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   if (timed_out) return;
   const int ip = blockIdx.x * AEV_WARPS + w;
   if (ip >= n_ml) return;
-  WarpEnv& e = env[w];
+  BwdEnv& e = env[w];
   const float4 ci = spos[ip];
   const int si = (__float_as_int(ci.w) >> 28) & 7;
   const int nR = cntR[ip], nA = cntA[ip];
   const uint32_t* __restrict__ rowR = nbrR + (size_t)ip * rcap;
-  load_env(c, g, spos, rowR, nbrA + (size_t)ip * acap, nR, nA, ci, lane, e);
   const int Kc = grp->Kc;
-  // row of dE/dAEV in the piece-major tile layout: float4 piece q of this row = gi4[q * TILE_M]
+  // row of dE/dAEV in the piece-major tile layout: float4 piece q of this row = gb[q * gs].  (Read through L1 where it
+  // is needed: staging the row in shared memory first was measured twice -- round 1 and again with the packed
+  // arithmetic, 86 -> 92 us -- and lost both times: extra registers across the gather and bank conflicts between the
+  // lanes' different species-pair blocks.)
   const size_t grow = (size_t)(ip + grp->pad_shift[si]);
-  const float4* gi4 = reinterpret_cast<const float4*>(daev + daev_off(grow, 0, Kc));
+  const float4* gb = reinterpret_cast<const float4*>(daev + daev_off(grow, 0, Kc));
+  constexpr int gs = TILE_M;
+  bwd_load_env(c, g, spos, rowR, nbrA + (size_t)ip * acap, nR, nA, ci, lane, e);
 
   // ---- angular: p_ij for the angular neighbours, staged in Pacc
   if (nA <= 32) {
@@ -163,7 +221,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
           int k = jl + m;
           if (k >= ns) k -= ns;
           k += base;
-          const PairShares o = pair_shares(c, zm1, gi4 + pairoff[sj * MAX_S + e.slotA[k]], uj, fj, dfj, e.ua[k], e.fA[k],
+          const PairShares o = pair_shares(c, zm1, gb + pairoff[sj * MAX_S + e.slotA[k]] * gs, gs, uj, fj, dfj, e.ua[k], e.fA[k],
                                            e.dfA[k]);
           px += o.jx; py += o.jy; pz += o.jz;
           qx = o.kx; qy = o.ky; qz = o.kz;
@@ -199,7 +257,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const int r = r0 + g2, k = 16 + r;
         float qx = 0.f, qy = 0.f, qz = 0.f;
         if (r < nb) {
-          const PairShares o = pair_shares(c, zm1, gi4 + pairoff[sj * MAX_S + e.slotA[k]], uj, fj, dfj, e.ua[k], e.fA[k],
+          const PairShares o = pair_shares(c, zm1, gb + pairoff[sj * MAX_S + e.slotA[k]] * gs, gs, uj, fj, dfj, e.ua[k], e.fA[k],
                                            e.dfA[k]);
           px += o.jx; py += o.jy; pz += o.jz;
           qx = o.kx; qy = o.ky; qz = o.kz;
@@ -237,7 +295,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         const int sk = e.slotA[k];
         const int s1 = min(sj, sk), s2 = max(sj, sk);
         const int pidx = s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1);
-        const float4* gb = gi4 + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * TILE_M;
+        const float4* gbp = gb + (size_t)grp->cpos[c.nRB + pidx] * (BLK / 4) * gs;
         const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
         const float cc = c.cTheta * u;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 1e-12f));
@@ -257,7 +315,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
         float sW = 0.f, sV = 0.f;
 #pragma unroll
         for (int a = 0; a < NSHFA; ++a) {
-          const float4 g0 = gb[(2 * a) * TILE_M], g1 = gb[(2 * a + 1) * TILE_M];
+          const float4 g0 = gbp[(2 * a) * gs], g1 = gbp[(2 * a + 1) * gs];
           float W = g0.x * F1[0], V = g0.x * dF1[0];
           W = fmaf(g0.y, F1[1], W); V = fmaf(g0.y, dF1[1], V);
           W = fmaf(g0.z, F1[2], W); V = fmaf(g0.z, dF1[2], V);
@@ -300,28 +358,30 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     if (q < nR) {
       const float4 uq = e.u[q];
       const int s = e.slotR[q];
-      const float4* gr = gi4 + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * TILE_M;
-      const float f = e.wR[q];   // c_R f_C
+      const float4* gr = gb + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * gs;
       float fc, dfc;
       cutoff(fminf(uq.w, c.Rcr), c.inv_Rcr, fc, dfc);
-      const float df = c.cR * dfc;
-      float coef = 0.f;
+      const float f = c.cR * fc, df = c.cR * dfc;
+      // sum over the 16 shifts of g_m d/dR [c_R exp(-eta (R - Shf_m)^2) f_C(R)], two shifts per packed instruction
+      const float2 R2 = make_float2(uq.w, uq.w), hf2 = make_float2(-2.0f * c.etaR * f, -2.0f * c.etaR * f), df2 = make_float2(df, df);
+      float2 coef2 = make_float2(0.f, 0.f);
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
-        const float4 gv = gr[v * TILE_M];
-        const float gg[4] = {gv.x, gv.y, gv.z, gv.w};
+        const float4 gv = gr[v * gs];
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const float x = uq.w - c.ShfR[4 * v + t];
-          const float ex = ex2f(-c.etaR_l2e * x * x);
-          coef = fmaf(gg[t] * ex, fmaf(-2.0f * c.etaR * x, f, df), coef);
+        for (int t = 0; t < 4; t += 2) {
+          const float2 x = __fadd2_rn(R2, make_float2(-c.ShfR[4 * v + t], -c.ShfR[4 * v + t + 1]));
+          const float2 y = __fmul2_rn(x, x);
+          const float2 ex = make_float2(ex2f(-c.etaR_l2e * y.x), ex2f(-c.etaR_l2e * y.y));
+          const float2 gg = (t == 0) ? make_float2(gv.x, gv.y) : make_float2(gv.z, gv.w);
+          coef2 = __ffma2_rn(__fmul2_rn(gg, ex), __ffma2_rn(x, hf2, df2), coef2);
         }
       }
+      const float coef = coef2.x + coef2.y;
       float px = coef * uq.x, py = coef * uq.y, pz = coef * uq.z;
-      // angular share of this neighbour, if it is one: binary search of q in posA
-      int lo = 0, hi = nA;
-      while (lo < hi) { int mid = (lo + hi) >> 1; if (e.posA[mid] < q) lo = mid + 1; else hi = mid; }
-      if (lo < nA && e.posA[lo] == q) { px += Pacc[w][lo][0]; py += Pacc[w][lo][1]; pz += Pacc[w][lo][2]; }
+      // angular share of this neighbour, if it is one
+      const int ia = e.ainv[q];
+      if (ia != 255) { px += Pacc[w][ia][0]; py += Pacc[w][ia][1]; pz += Pacc[w][ia][2]; }
       const long long fx = to_fix(px), fy = to_fix(py), fz = to_fix(pz);
       ox += fx; oy += fy; oz += fz;
       if (VIRIAL) {   // strain derivative dE/d eps_ab = sum p_ij[a] d_ij[b], d_ij = R u
