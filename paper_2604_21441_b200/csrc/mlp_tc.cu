@@ -166,21 +166,9 @@ __device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_
   const __half2 h = __floats2half2_rn(x0, x1);
   const float2 hf = __half22float2(h);
   hi = h2_bits(h);
-  lo = h2_bits(__floats2half2_rn(x0 - hf.x, x1 - hf.y));
+  const float2 d = __ffma2_rn(hf, make_float2(-1.0f, -1.0f), make_float2(x0, x1));   // x - hi, exact, one packed instruction
+  lo = h2_bits(__floats2half2_rn(d.x, d.y));
 }
-// CELU' in [0, 1] as unorm16 pairs (1.0 exact; absolute error 2^-17).  Conversions go through the 2^23 trick
-// (x + 2^23 holds round-to-nearest(x) in its low mantissa bits) so that they stay on the FMA/ALU pipes.
-__device__ __forceinline__ uint32_t pack_c(float c0, float c1) {
-  const uint32_t q0 = __float_as_uint(fmaf(c0, 65535.f, 8388608.f)), q1 = __float_as_uint(fmaf(c1, 65535.f, 8388608.f));
-  return __byte_perm(q0, q1, 0x5410);
-}
-__device__ __forceinline__ float unpack_c_lo(uint32_t q) {
-  return (__uint_as_float(__byte_perm(q, 0x4B000000u, 0x7610)) - 8388608.f) * (1.0f / 65535.f);
-}
-__device__ __forceinline__ float unpack_c_hi(uint32_t q) {
-  return (__uint_as_float(__byte_perm(q, 0x4B000000u, 0x7632)) - 8388608.f) * (1.0f / 65535.f);
-}
-
 // ------------------------------------------------------------------------------------------------ layer-1 images
 // The AEV columns that are materialised depend on the species present in the evaluation (GroupInfo::blkmap), so the
 // layer-1 operand images are (re)packed on the device, only when that column set changed since the last call.
@@ -241,8 +229,9 @@ constexpr int TC_THREADS = (TC_EPI_WARPS + 2) * 32;   // + weight producer warp 
 constexpr uint32_t TC_PANEL = 16384;                  // 128 rows x 128 B
 constexpr uint32_t TC_LO = 4 * TC_PANEL;              // lo half of the A buffer
 constexpr uint32_t TC_ACCW = 256;                     // TMEM: two 256-column accumulators (columns 0 and 256), used alternately
-constexpr int TC_CW1 = 128, TC_CW2 = 128;             // words per row of the packed CELU' of layers 1 and 2 (global scratch)
-constexpr int TC_CSCR_WORDS = (TC_CW1 + TC_CW2) * 128;  // per CTA
+constexpr int TC_CW1 = 256, TC_CW2 = 256;             // words per row of CELU' (fp32) of layers 1 and 2 (global scratch)
+constexpr int TC_CSCR_WORDS = (TC_CW1 + TC_CW2) * 128;  // per CTA: 256 KB, written in the forward and read back in the backward
+                                                      // epilogues by the same thread; 38 MB for 148 CTAs, L2-resident
 
 template <int NPASS> struct TcCfg {
   static constexpr int NH = (NPASS == 3) ? 2 : 1;
@@ -488,13 +477,14 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       tc_fence_after();
       TC_STAMP();
     };
-    uint32_t* const cs1 = cscr + (size_t)blockIdx.x * TC_CSCR_WORDS;   // CELU' of layer 1: [chunk j][2][128 rows][4 words]
-    uint32_t* const cs2 = cs1 + TC_CW1 * 128;
+    float* const cs1 = reinterpret_cast<float*>(cscr) + (size_t)blockIdx.x * TC_CSCR_WORDS;   // CELU' of layer 1: [piece = column / 4][128 rows][4 floats]
+    float* const cs2 = cs1 + TC_CW1 * 128;
     for (int w = blockIdx.x; w < n_items; w += gridDim.x) {
       int t, mem; TileInfo ti; TileNet tn; tile_net(w, t, mem, ti, tn);
       const Net& net = all_nets[mem].net[ti.slot];
       const bool accumulate = mem > 0;
       const float alpha = net.alpha, kexp = 1.4426950408889634f / alpha;
+      const float2 alpha2 = make_float2(alpha, alpha), nalpha2 = make_float2(-alpha, -alpha), kexp2 = make_float2(kexp, kexp);
       const bool valid = row < ti.nvalid;
       // ---- F1 rounds: AEV columns [64 p0, 64 p1) -> fp16 hi/lo panels
       const int np = tc_npanels(Kc);
@@ -538,13 +528,14 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
       for (int l = 1; l <= 2; ++l) {
         const int N = (l == 1) ? tn.N1 : tn.N2;
         const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[l - 1]);
-        uint32_t* const cs = (l == 1) ? cs1 : cs2;
+        float* const cs = (l == 1) ? cs1 : cs2;
         const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
         for (int pi4 = 0; pi4 < 4; ++pi4) {
           const int j = part + TC_NPART * pi4;
           if (j * 16 < N) {
-          uint32_t v[16], hi[8], lo[8], cp[8];
+          uint32_t v[16], hi[8], lo[8];
+          float ce[16];
           tmem_ld16(tacc + j * 16, v);
           float4 bv[4];
 #pragma unroll
@@ -552,16 +543,20 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
           tmem_wait_ld();
 #pragma unroll
           for (int i = 0; i < 16; i += 2) {
+            // CELU and CELU' of two columns in packed fp32: e = exp(min(z, 0) / alpha) = CELU'(z) (ex2(0) = 1 exactly, no
+            // select), CELU(z) = max(z, 0) + alpha (e - 1) = fma(alpha, e, max(z, 0) - alpha)
             const float4 b4 = bv[i >> 2];
-            const float z0 = __uint_as_float(v[i]) + ((i & 2) ? b4.z : b4.x);
-            const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
-            const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
-            const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
-            cp[i >> 1] = pack_c(e0, e1);   // CELU'(z) = exp(min(z, 0) / alpha): ex2(0) = 1 exactly, no select needed
-            split2(h0, h1, hi[i >> 1], lo[i >> 1]);
+            const float2 z = __fadd2_rn(make_float2(__uint_as_float(v[i]), __uint_as_float(v[i + 1])),
+                                        (i & 2) ? make_float2(b4.z, b4.w) : make_float2(b4.x, b4.y));
+            const float2 t = __fmul2_rn(make_float2(fminf(z.x, 0.f), fminf(z.y, 0.f)), kexp2);
+            const float2 e = make_float2(exp2f(t.x), exp2f(t.y));
+            const float2 h = __ffma2_rn(alpha2, e, __fadd2_rn(make_float2(fmaxf(z.x, 0.f), fmaxf(z.y, 0.f)), nalpha2));
+            ce[i] = e.x; ce[i + 1] = e.y;
+            split2(h.x, h.y, hi[i >> 1], lo[i >> 1]);
           }
-          __stcg(reinterpret_cast<uint4*>(cs + ((size_t)(2 * j) * 128 + row) * 4), make_uint4(cp[0], cp[1], cp[2], cp[3]));
-          __stcg(reinterpret_cast<uint4*>(cs + ((size_t)(2 * j + 1) * 128 + row) * 4), make_uint4(cp[4], cp[5], cp[6], cp[7]));
+#pragma unroll
+          for (int i = 0; i < 4; ++i)   // CELU' in fp32, piece-major like dE/dAEV: 512 contiguous bytes per warp store
+            __stcg(reinterpret_cast<float4*>(cs + ((size_t)(4 * j + i) * 128 + row) * 4), make_float4(ce[4 * i], ce[4 * i + 1], ce[4 * i + 2], ce[4 * i + 3]));
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
           }
           arrive_panel(pi4);
@@ -574,7 +569,8 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
         const int nl = net.n_layers;
         const float4* __restrict__ bias4 = reinterpret_cast<const float4*>(net.b[2]);
         const float4* __restrict__ w44 = reinterpret_cast<const float4*>(net.W[nl - 1]);
-        float e = 0.f;
+        float2 e2 = make_float2(0.f, 0.f);
+        const float2 esc2 = make_float2(escale, escale);
         const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
         for (int pi4 = 0; pi4 < 4; ++pi4) {
@@ -589,18 +585,21 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
 #pragma unroll
           for (int i = 0; i < 16; i += 2) {
             const float4 b4 = bv[i >> 2], w4 = wv[i >> 2];
-            const float z0 = __uint_as_float(v[i]) + ((i & 2) ? b4.z : b4.x);
-            const float z1 = __uint_as_float(v[i + 1]) + ((i & 2) ? b4.w : b4.y);
-            const float wa = (i & 2) ? w4.z : w4.x, wb = (i & 2) ? w4.w : w4.y;   // escale = 1/members rides on dl3
-            const float e0 = exp2f(fminf(z0, 0.f) * kexp), e1 = exp2f(fminf(z1, 0.f) * kexp);
-            const float h0 = z0 > 0.f ? z0 : fmaf(alpha, e0, -alpha), h1 = z1 > 0.f ? z1 : fmaf(alpha, e1, -alpha);
-            e = fmaf(h0, wa, e); e = fmaf(h1, wb, e);
-            split2(escale * wa * e0, escale * wb * e1, hi[i >> 1], lo[i >> 1]);   // e = CELU'(z) (1 for z > 0)
+            const float2 z = __fadd2_rn(make_float2(__uint_as_float(v[i]), __uint_as_float(v[i + 1])),
+                                        (i & 2) ? make_float2(b4.z, b4.w) : make_float2(b4.x, b4.y));
+            const float2 w2 = (i & 2) ? make_float2(w4.z, w4.w) : make_float2(w4.x, w4.y);   // escale = 1/members rides on dl3
+            const float2 t = __fmul2_rn(make_float2(fminf(z.x, 0.f), fminf(z.y, 0.f)), kexp2);
+            const float2 ce = make_float2(exp2f(t.x), exp2f(t.y));                            // CELU'(z) (1 for z > 0)
+            const float2 h = __ffma2_rn(alpha2, ce, __fadd2_rn(make_float2(fmaxf(z.x, 0.f), fmaxf(z.y, 0.f)), nalpha2));
+            e2 = __ffma2_rn(h, w2, e2);
+            const float2 d = __fmul2_rn(__fmul2_rn(esc2, w2), ce);
+            split2(d.x, d.y, hi[i >> 1], lo[i >> 1]);
           }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
           }
           arrive_panel(pi4);
         }
+        float e = e2.x + e2.y;
         if (part > 0) e_part[(part - 1) * 128 + row] = e;
         if (accumulate && threadIdx.x == 0) {   // the previous member of this tile must have finished its updates
           int seen;
@@ -623,12 +622,11 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
 #pragma unroll 1
       for (int l = 2; l >= 1; --l) {
         const int N = (l == 1) ? tn.N1 : tn.N2;
-        const uint32_t* const cs = (l == 1) ? cs1 : cs2;
-        uint4 cn0 = make_uint4(0u, 0u, 0u, 0u), cn1 = cn0;   // this thread wrote these words itself in the forward pass
-        if (part * 16 < N) {
-          cn0 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * part) * 128 + row) * 4));
-          cn1 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * part + 1) * 128 + row) * 4));
-        }
+        const float* const cs = (l == 1) ? cs1 : cs2;
+        float4 cn[4];   // this thread wrote these words itself in the forward pass
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          cn[i] = (part * 16 < N) ? __ldcg(reinterpret_cast<const float4*>(cs + ((size_t)(4 * part + i) * 128 + row) * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
         wait_acc();   // B3 (l = 2) / B2 (l = 1) complete
         const uint32_t tacc = tlane + buf * TC_ACCW;
 #pragma unroll 1
@@ -637,16 +635,20 @@ k_mlp_tc(const NetTable* __restrict__ all_nets, const TcTable* __restrict__ all_
           if (j * 16 < N) {
           uint32_t v[16], hi[8], lo[8];
           tmem_ld16(tacc + j * 16, v);
-          const uint32_t cp[8] = {cn0.x, cn0.y, cn0.z, cn0.w, cn1.x, cn1.y, cn1.z, cn1.w};
+          const float4 cc[4] = {cn[0], cn[1], cn[2], cn[3]};
           if ((j + TC_NPART) * 16 < N) {
-            cn0 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * (j + TC_NPART)) * 128 + row) * 4));
-            cn1 = __ldcg(reinterpret_cast<const uint4*>(cs + ((size_t)(2 * (j + TC_NPART) + 1) * 128 + row) * 4));
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+              cn[i] = __ldcg(reinterpret_cast<const float4*>(cs + ((size_t)(4 * (j + TC_NPART) + i) * 128 + row) * 4));
           }
           tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 16; i += 2)
-            split2(__uint_as_float(v[i]) * unpack_c_lo(cp[i >> 1]), __uint_as_float(v[i + 1]) * unpack_c_hi(cp[i >> 1]),
-                   hi[i >> 1], lo[i >> 1]);
+          for (int i = 0; i < 16; i += 2) {
+            const float4 c4 = cc[i >> 2];
+            const float2 d = __fmul2_rn(make_float2(__uint_as_float(v[i]), __uint_as_float(v[i + 1])),
+                                        (i & 2) ? make_float2(c4.z, c4.w) : make_float2(c4.x, c4.y));
+            split2(d.x, d.y, hi[i >> 1], lo[i >> 1]);
+          }
           tc_store_act<NPASS>(abuf, row, j, hi, lo);
           }
           arrive_panel(pi4);
