@@ -493,7 +493,8 @@ def main():
     ap.add_argument("--mlp-mode", default="default", choices=["default", "simt", "f16x3", "f16x1"])
     ap.add_argument("--ensemble", type=int, default=1, help="networks per element (ANI-2x: 8); E = mean over members")
     ap.add_argument("--dense-k", action="store_true", help="materialise all 1008 AEV columns (K = 1024 first layer)")
-    ap.add_argument("--bin-reuse", type=int, default=0, help="reuse the cell binning for N-1 of every N steps (0 = rebuild every step)")
+    ap.add_argument("--bin-reuse", "--list-reuse", dest="bin_reuse", type=int, default=0,
+                    help="reuse cell binning and neighbour rows for N-1 of every N steps (0 = rebuild every step, the contract workload)")
     ap.add_argument("--skin", type=float, default=0.5, help="cell-width buffer in Angstrom for --bin-reuse")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra records of the contract line (MLP variants, cfg 0-4 sweep, per-config oracle timings)")

@@ -124,17 +124,21 @@ int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
  * up to fp32 summation order of the positions' frame.  0: always the general cell-list path. */
 int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
 
-/* Reuse of the cell binning over several MD steps ("Verlet-buffered list reuse"; the
- * paper's runs update GROMACS' own lists every 10-100 steps).  every_n <= 1 (default): every nnp_eval bins and sorts the
- * ML atoms.  every_n > 1: the cell grid is cut with edges >= Rcr + skin, and for the every_n - 1 evaluations that follow
- * a full one -- same n_atoms, n_ml, box, pbc and the SAME atoms behind d_Z / d_ml_index (caller's responsibility) -- the
- * binning, scan, scatter and ordering phases are replaced by one refresh pass that re-reads the positions into the
- * stored order.  The neighbour ROWS are still built from the current positions with the pinned predicate every step, so
- * rows, E and F are exactly those of a full evaluation as long as no atom has left its cell by more than skin / 2 in
- * any direction; one that has raises NNP_ERR_STALE through nnp_status() (outputs of that step unspecified, the next
- * evaluation rebuilds).  skin in the caller's length unit.  Periodic boxes (orthorhombic or triclinic) on the cell-list
- * path only: open boundaries and the small-system front end keep rebuilding every step.  The step counter lives on the host:
- * a CUDA graph captures whichever kind of step it was recorded on. */
+/* Verlet-buffered reuse of the cell binning AND the neighbour rows over several MD steps (
+ * the engine's own pair list lives for many steps -- the paper's runs update GROMACS' lists every 10-100
+ * steps).  every_n <= 1 (default): every nnp_eval bins, sorts and searches from scratch.  every_n > 1: the cell grid is cut
+ * with edges >= Rcr + skin and a full evaluation additionally keeps, per centre, its WIDE row: every neighbour within
+ * Rcr + skin.  For the every_n - 1 evaluations that follow -- same n_atoms, n_ml, box, pbc and the SAME atoms behind d_Z /
+ * d_ml_index (caller's responsibility; nnp_eval_host compares the contents) -- binning, scan, ordering and the 27-cell
+ * candidate sweep are replaced by a refresh pass (positions re-read into the stored order) and a pass over the wide rows
+ * that decides every stored pair from the CURRENT positions with the pinned predicate (fp32 outside the guard band, fp64
+ * inside).  The effective rows, E and F are therefore exactly those of a full evaluation on the same order of atoms, as
+ * long as no atom has moved by more than skin / 2 since the last full evaluation; one that has raises NNP_ERR_STALE through
+ * nnp_status() (outputs of that step unspecified, the next evaluation rebuilds).  skin in the caller's length unit.
+ * Periodic boxes (orthorhombic or triclinic) on the cell-list path; with an external pair list set only the binning is
+ * reused (the list is the engine's own buffered list); open boundaries and the small-system front end keep rebuilding every
+ * step.  The first call with every_n > 1 allocates the wide rows (768 bytes per ML atom).  The step counter lives on the
+ * host: a CUDA graph captures whichever kind of step it was recorded on. */
 int nnp_workspace_set_bin_reuse(nnp_workspace*, int32_t every_n, double skin);
 
 /* External pair list ("The 2026 version adds the internal pair-list built by GROMACS ... as

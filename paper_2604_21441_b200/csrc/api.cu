@@ -167,7 +167,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   cudaStreamSynchronize(ws->stream);
   tc_workspace_destroy(ws);
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
-  void* ptrs[] = {ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
+  void* ptrs[] = {ws->wideR, ws->cntW, ws->spos_ref, ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
                   ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->pos_scaled, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_forces};
@@ -289,6 +289,19 @@ extern "C" int nnp_workspace_set_pair_list(nnp_workspace* ws, const int32_t* d_p
 
 extern "C" int nnp_workspace_set_bin_reuse(nnp_workspace* ws, int32_t every_n, double skin) {
   if (!ws || (every_n > 1 && !(skin > 0.0))) return NNP_ERR_INVALID_ARG;
+  if (every_n > 1 && !ws->wideR) {   // first use: the wide rows of the row reuse (allocated here, never inside nnp_eval)
+    ws->wcap = 192;
+    const size_t nm = (size_t)std::max<int64_t>(ws->max_ml, 1);
+    if (cudaMalloc((void**)&ws->wideR, nm * ws->wcap * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc((void**)&ws->cntW, nm * sizeof(int)) != cudaSuccess ||
+        cudaMalloc((void**)&ws->spos_ref, nm * sizeof(float4)) != cudaSuccess) {
+      cudaGetLastError();
+      if (ws->wideR) cudaFree(ws->wideR);
+      if (ws->cntW) cudaFree(ws->cntW);
+      ws->wideR = nullptr; ws->cntW = nullptr; ws->spos_ref = nullptr;
+      return NNP_ERR_CUDA;
+    }
+  }
   ws->reuse_every = every_n > 1 ? every_n : 0;
   ws->reuse_skin = every_n > 1 ? skin : 0.0;
   ws->reuse_left = 0;   // the next evaluation bins afresh (with the new cell width)

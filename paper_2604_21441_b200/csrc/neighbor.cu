@@ -479,6 +479,36 @@ constexpr int NB_CAP = 1024;            // candidates staged in shared memory pe
 constexpr int NB_SEG = MAX_S * 27;      // (species, neighbour cell) segments of one centre cell
 constexpr int SURV_CAP = 256;           // candidates of one centre that pass the cheap distance filter, per chunk
 
+// The decision on 32 candidates of centre ip (one per lane; d = displacement from the centre, ent = row entry, a_j = the
+// candidate's ML-local index): radial / angular membership by the fp32 value outside the guard bands, by the pinned
+// fp64 predicate on the ORIGINAL coordinates inside them (reading #6); ballot compaction into the rows.  Shared by the
+// cell sweep and the row refresh from stored wide rows, so both give the same rows.
+template <bool TRIC>
+__device__ __forceinline__ void decide32(const AevConst& c, const GridInfo* __restrict__ g, const float* __restrict__ pos,
+                                         const int32_t* __restrict__ ml, bool live, float dx, float dy, float dz, uint32_t ent,
+                                         int a_j, int ip, int o_i, unsigned lt, uint32_t* rR, uint8_t* rA, int rcap, int acap,
+                                         int& nR, int& nA, int& bad) {
+  const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
+  const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+  const bool other = live && (int)(ent & JMASK) != ip;
+  bool inR = other && d2 < loR, inA = other && d2 < loA;
+  // guard bands (and coincident atoms): the pinned fp64 predicate on the original coordinates decides
+  const bool near = other && (fabsf(d2 - Rcr2) <= GUARD_BAND || fabsf(d2 - Rca2) <= GUARD_BAND || d2 < 1e-6f);
+  if (near) {
+    const int o_j = ml ? ml[a_j] : a_j;
+    const double e2 = TRIC ? exact_d2_tric(pos, o_i, o_j, g) : exact_d2(pos, o_i, o_j, g);
+    if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
+    if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
+    if (e2 == 0.0) bad |= FLAG_COINCIDENT;
+  }
+  const unsigned mR = __ballot_sync(0xffffffffu, inR);
+  const unsigned mA = __ballot_sync(0xffffffffu, inA);
+  const int pR = nR + __popc(mR & lt), pA = nA + __popc(mA & lt);
+  if (inR && pR < rcap) rR[pR] = ent;
+  if (inA && pA < acap && pR < rcap) rA[pA] = (uint8_t)pR;
+  nR += __popc(mR); nA += __popc(mA);
+}
+
 // One block per cell.  The atoms of the 27 neighbouring cells (per species: 27 buckets of the slot-major sort) are
 // staged once in shared memory, already shifted into the centre cell's frame; then each warp takes a centre of the
 // cell and goes over the staged candidates in TWO stages:
@@ -497,7 +527,8 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
                                                    uint32_t* __restrict__ nbrR, uint8_t* __restrict__ nbrA,
                                                    int* __restrict__ cntR, int* __restrict__ cntA,
                                                    int* __restrict__ flags, int* __restrict__ zcount,
-                                                   int* __restrict__ zfill, int* __restrict__ zpresent) {
+                                                   int* __restrict__ zfill, int* __restrict__ zpresent,
+                                                   uint32_t* __restrict__ wide, int* __restrict__ cntW, int wcap, float wide_r2) {
   __shared__ float4 cand[NB_CAP];
   __shared__ int candA[NB_CAP];           // ML-local index of the candidate (for the fp64 re-check)
   __shared__ int segStart[NB_SEG], segOff[NB_SEG + 1], segCode[NB_SEG];
@@ -589,8 +620,7 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
     __syncthreads();
     // ---- sweep: one warp per centre
     const bool wrap = pbc && (nc0 == 1 || nc1 == 1 || nc2 == 1);
-    const float Rcr2 = c.Rcr2, Rca2 = c.Rca2, loR = c.Rcr2 - GUARD_BAND, loA = c.Rca2 - GUARD_BAND;
-    const float hi2 = c.Rcr2 + 2.0f * GUARD_BAND;
+    const float hi2 = (wide ? wide_r2 : c.Rcr2) + 2.0f * GUARD_BAND;
     unsigned short* sv = surv[warp];
     for (int ci = warp + 8 * blockIdx.y; ci < nC; ci += 8 * gridDim.y) {   // small systems: gridDim.y blocks share a cell
       int s = 0;
@@ -624,8 +654,8 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
       // ---- stage 2: decide the survivors
       uint32_t* rR = nbrR + (size_t)ip * rcap;
       uint8_t* rA = nbrA + (size_t)ip * acap;
-      int nR = 0, nA = 0;
-      if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; }
+      int nR = 0, nA = 0, nW = 0;
+      if (chunk0 > 0) { nR = cntR[ip]; nA = cntA[ip]; if (wide) nW = cntW[ip]; }
       for (int s0 = 0; s0 < ns; s0 += 32) {
         const bool live = s0 + lane < ns;
         const int q = live ? (int)sv[s0 + lane] : 0;
@@ -637,27 +667,16 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
           if (nc1 == 1) { const int o = -(int)rintf(dy / ey); dy += (float)o * ey; ent += (uint32_t)(o * 4) << JBITS; }
           if (nc2 == 1) { const int o = -(int)rintf(dz / ez); dz += (float)o * ez; ent += (uint32_t)(o * 16) << JBITS; }
         }
-        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        const bool other = live && (int)(ent & JMASK) != ip;
-        bool inR = other && d2 < loR, inA = other && d2 < loA;
-        // guard bands (and coincident atoms): the pinned fp64 predicate on the original coordinates decides
-        const bool near = other && (fabsf(d2 - Rcr2) <= GUARD_BAND || fabsf(d2 - Rca2) <= GUARD_BAND || d2 < 1e-6f);
-        if (near) {
-          const int a_j = candA[q];
-          const int o_j = ml ? ml[a_j] : a_j;
-          const double e2 = TRIC ? exact_d2_tric(pos, o_i, o_j, g) : exact_d2(pos, o_i, o_j, g);
-          if (fabsf(d2 - Rcr2) <= GUARD_BAND) inR = e2 <= c.Rcr2_d;
-          if (fabsf(d2 - Rca2) <= GUARD_BAND) inA = e2 <= c.Rca2_d;
-          if (e2 == 0.0) bad |= FLAG_COINCIDENT;
-        }
-        const unsigned mR = __ballot_sync(0xffffffffu, inR);
-        const unsigned mA = __ballot_sync(0xffffffffu, inA);
-        const int pR = nR + __popc(mR & lt), pA = nA + __popc(mA & lt);
-        if (inR && pR < rcap) rR[pR] = ent;
-        if (inA && pA < acap && pR < rcap) rA[pA] = (uint8_t)pR;
-        nR += __popc(mR); nA += __popc(mA);
+        // row reuse (nnp_workspace_set_bin_reuse): the filter ran with the cut-off widened by the skin, and everything it
+        // let through is kept as the centre's WIDE row, from which the rows of the following steps are decided
+        if (wide && live && nW + s0 + lane < wcap) wide[(size_t)ip * wcap + nW + s0 + lane] = ent;
+        decide32<TRIC>(c, g, pos, ml, live, dx, dy, dz, ent, candA[q], ip, o_i, lt, rR, rA, rcap, acap, nR, nA, bad);
       }
       if (nR > rcap || nA > acap) bad |= FLAG_CAP;
+      if (wide) {
+        if (nW + ns > wcap) bad |= FLAG_CAP;
+        if (lane == 0) cntW[ip] = min(nW + ns, wcap);
+      }
       if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
       __syncwarp();
     }
@@ -862,7 +881,7 @@ k_pair_rows(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict
 __global__ void __launch_bounds__(256)
 k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const int32_t* __restrict__ ml, int n_ml,
           double half_skin, float4* __restrict__ spos, const int* __restrict__ scell, unsigned long long* __restrict__ facc,
-          int* __restrict__ flags) {
+          int* __restrict__ flags, const float4* __restrict__ spos_ref) {
   pdl_trigger();
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   if (ip >= n_ml) return;
@@ -905,9 +924,68 @@ k_refresh(const GridInfo* __restrict__ g, const float* __restrict__ pos, const i
     loc[d] = (float)t;
   }
   }
+  if (spos_ref) {   // the ROWS are reused too: every pair within Rcr now must have been within Rcr + skin when the wide rows
+                    // were built, i.e. no atom may have moved by more than skin / 2 since (same cell frame: plain difference)
+    const float4 r = spos_ref[ip];
+    const float ux = loc[0] - r.x, uy = loc[1] - r.y, uz = loc[2] - r.z;
+    stale |= (double)(ux * ux + uy * uy + uz * uz) > half_skin * half_skin;
+  }
   if (stale) atomicOr(flags, FLAG_STALE);
   spos[ip] = make_float4(loc[0], loc[1], loc[2], w);
   facc[3 * (size_t)ip + 0] = 0ull; facc[3 * (size_t)ip + 1] = 0ull; facc[3 * (size_t)ip + 2] = 0ull;
+}
+
+// Row reuse ("Verlet-buffered list reuse"; the engine's pair list lives
+// for many steps): on the steps between two full builds the rows are decided from the stored WIDE rows (everything within
+// Rcr + skin at build time) instead of the 27-cell sweep: one warp per centre, 32 wide entries at a time, the refreshed
+// cell-local coordinates, and the same decision (decide32: fp32 outside the guard bands, pinned fp64 predicate inside) --
+// so the rows are exactly those of a full build on the same order of atoms, at a fraction of the candidates (~80 / centre
+// against 486).
+template <bool TRIC>
+__global__ void __launch_bounds__(256, 4)   // latency-bound (two dependent gathers per group): 64 registers, no spills
+k_rows_from_wide(AevConst c, const GridInfo* __restrict__ g, const float4* __restrict__ spos, const float* __restrict__ pos,
+                 const int32_t* __restrict__ ml, int n_ml, int rcap, int acap, const uint32_t* __restrict__ wide,
+                 const int* __restrict__ cntW, int wcap, uint32_t* __restrict__ nbrR, uint8_t* __restrict__ nbrA,
+                 int* __restrict__ cntR, int* __restrict__ cntA, int* __restrict__ flags) {
+  pdl_trigger();
+  pdl_wait();
+  const int lane = threadIdx.x & 31, ip = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (ip >= n_ml) return;
+  float ev[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) ev[k] = g->ev[k];
+  const float4 pi = spos[ip];
+  const int a_i = __float_as_int(pi.w) & 0x0fffffff;
+  const int o_i = ml ? ml[a_i] : a_i;
+  const unsigned lt = lanemask_lt();
+  const int nW = cntW[ip];
+  const uint32_t* wr = wide + (size_t)ip * wcap;
+  uint32_t* rR = nbrR + (size_t)ip * rcap;
+  uint8_t* rA = nbrA + (size_t)ip * acap;
+  int nR = 0, nA = 0, bad = 0;
+  // three groups of 32 entries per pass: all entry loads, then all position gathers in flight before the first decision
+  // (the pass is a chain of two dependent global loads per group; a wide row of liquid water holds ~85 entries)
+  for (int s0 = 0; s0 < nW; s0 += 96) {
+    uint32_t ent[3];
+    float4 pj[3];
+#pragma unroll
+    for (int u = 0; u < 3; ++u) ent[u] = (s0 + 32 * u + lane < nW) ? wr[s0 + 32 * u + lane] : (uint32_t)ip;
+#pragma unroll
+    for (int u = 0; u < 3; ++u) pj[u] = spos[ent[u] & JMASK];
+#pragma unroll
+    for (int u = 0; u < 3; ++u) {
+      if (s0 + 32 * u < nW) {   // warp-uniform
+        const int oc = (int)(ent[u] >> JBITS);
+        float sx, sy, sz;
+        cell_shift(ev, (oc & 3) - 1, ((oc >> 2) & 3) - 1, ((oc >> 4) & 3) - 1, sx, sy, sz);
+        decide32<TRIC>(c, g, pos, ml, s0 + 32 * u + lane < nW, (pj[u].x - pi.x) + sx, (pj[u].y - pi.y) + sy, (pj[u].z - pi.z) + sz,
+                       ent[u], __float_as_int(pj[u].w) & 0x0fffffff, ip, o_i, lt, rR, rA, rcap, acap, nR, nA, bad);
+      }
+    }
+  }
+  if (nR > rcap || nA > acap) bad |= FLAG_CAP;
+  if (lane == 0) { cntR[ip] = min(nR, rcap); cntA[ip] = min(nA, acap); }
+  if (bad) atomicOr(flags, bad);
 }
 
 // ---------------------------------------------------------------- host launcher
@@ -962,6 +1040,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   void* args[] = {&a};
   // fast binning (k_bin_cells + ranking inside k_neighbors): periodic boxes cut into >= 3 cells per dimension, own cell
   // search; a cell that overflowed its append buffer (NNP_ERR_CAPACITY) sends the workspace back to the general path
+  // row reuse: own cell search only (an external pair list is itself the engine's buffered list)
+  const bool rows_reuse = reuse_ok && !ws->ext_pairs && ws->wideR != nullptr;
+  const bool tric_box = pbc && box_is_triclinic(box);
   const bool fast = a.host_grid && a.hg.nc[0] >= 3 && a.hg.nc[1] >= 3 && a.hg.nc[2] >= 3 && !ws->ext_pairs && !ws->slow_prep &&
                     a.hg.ncell <= ws->max_cells && a.hg.ncell <= FAST_MAX_CELLS;
   int extra = 0;   // kernels launched beyond the first
@@ -970,7 +1051,16 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     // refresh-only step: the stored order stays, positions are re-read (the grid on the device is the same one)
     --ws->reuse_left;
     k_refresh<<<(unsigned)((n_ml + 255) / 256), 256, 0, st>>>(ws->grid, d_pos, d_ml, (int)n_ml, 0.5 * skin, ws->spos, ws->scell,
-                                                             ws->facc, ws->flags);
+                                                             ws->facc, ws->flags, rows_reuse ? ws->spos_ref : nullptr);
+    if (rows_reuse) {   // the rows from the stored wide rows: no cell sweep on this step
+      if (tric_box)
+        launch_pdl(!ws->profiling, st, k_rows_from_wide<true>, dim3((unsigned)((n_ml + 7) / 8)), dim3(256), 0, m->aev, ws->grid, ws->spos,
+                   d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->wideR, ws->cntW, ws->wcap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->flags);
+      else
+        launch_pdl(!ws->profiling, st, k_rows_from_wide<false>, dim3((unsigned)((n_ml + 7) / 8)), dim3(256), 0, m->aev, ws->grid, ws->spos,
+                   d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->wideR, ws->cntW, ws->wcap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->flags);
+      return 2;
+    }
   } else {
   if (reuse_ok) {
     ws->reuse_left = ws->reuse_every - 1; ws->reuse_n_atoms = n_atoms; ws->reuse_n_ml = n_ml;
@@ -1032,7 +1122,10 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     auto kern = tric ? k_neighbors<true> : k_neighbors<false>;
     launch_pdl(!ws->profiling, st, kern, dim3(ncell_host, ysplit), dim3(256), 0, m->aev, ws->grid, ws->groups, ws->spos,
                ws->bstart, d_pos, d_ml, (int)n_ml, ws->rcap, ws->acap, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->flags,
-               fast_bin ? ws->cell_count : nullptr, ws->cellfill, ws->present);
+               fast_bin ? ws->cell_count : nullptr, ws->cellfill, ws->present, rows_reuse ? ws->wideR : nullptr, ws->cntW, ws->wcap,
+               (float)((m->aev.Rcr + skin) * (m->aev.Rcr + skin)));
+    if (rows_reuse)   // reference positions of the displacement check on the reuse steps (a full step: 1 in every_n)
+      cudaMemcpyAsync(ws->spos_ref, ws->spos, sizeof(float4) * (size_t)n_ml, cudaMemcpyDeviceToDevice, st);
     ++nl;
   }
   return nl;

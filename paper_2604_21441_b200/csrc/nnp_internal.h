@@ -153,6 +153,10 @@ struct nnp_workspace {
   float4* cellbuf;           // [max_cells][CELL_CAP] per-cell append buffers of the fast binning (neighbor.cu)
   int* cellfill;             // [max_cells] fill counters of the above (zero between evaluations)
   int* present;              // [1] bit mask of the species slots seen by k_bin_cells (zero between evaluations)
+  uint32_t* wideR;           // [max_ml][wcap] wide rows (everything within Rcr + skin at the last full build), row reuse only
+  int* cntW;                 // [max_ml]
+  float4* spos_ref;          // [max_ml] cell-local coordinates at the last full build
+  int wcap;
   int slow_prep;             // 1: a cell overflowed its append buffer once; this workspace keeps to the general binning
   int* rank;                 // [max_ml]
   float4* spos;              // [max_ml] sorted: cell-local xyz, w = ml-local index | slot << 28

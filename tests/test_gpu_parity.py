@@ -785,21 +785,23 @@ def test_bin_reuse_over_md_like_steps():
     torch = _torch()
     cfg = gen.get_config(1)
     n = cfg["pos"].shape[0]
-    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 7, sigma=0.05)
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 12, sigma=0.05)
     om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
     m, ws = make(cfg)
     ws.set_bin_reuse(5, 1.0)
     dZ = torch.from_numpy(cfg["Z"]).cuda()     # the same device buffers on every step, as an MD engine would pass them
     dpos = torch.empty((n, 3), dtype=torch.float32, device="cuda")
-    for t in range(7):
+    for t in range(12):                        # full builds at steps 0, 5, 10; the other nine reuse binning AND rows
         dpos.copy_(torch.from_numpy(P[t]))
         E, F = ws.eval(dpos, dZ, cfg["box"], 1)
         torch.cuda.synchronize()
         assert ws.status() == 0
+        # a reuse step runs no cell sweep: k_refresh + k_rows_from_wide in place of k_bin_cells + k_cell_sort + k_neighbors
+        assert ws.launches() == (8 if t % 5 == 0 else 7), (t, ws.launches())
         ref = oracle.evaluate(om, P[t], cfg["Z"], cfg["box"], 1, None, nbr_mode=1)
         check_lists(ws, cfg, P[t], n)
         check_EF(float(E.cpu()[0]), F.cpu().numpy().astype(np.float64), ref, n)
-    # step 7 is a reuse step (full binnings at steps 0 and 5): push one atom 1.5 A out of its cell
+    # step 12 is a reuse step (full builds at steps 0, 5, 10): push one atom far out of its cell
     bad = P[0].copy(); bad[17] += np.float32(8.0)      # farther than a cell edge + skin / 2
     dpos.copy_(torch.from_numpy(bad))
     ws.eval(dpos, dZ, cfg["box"], 1)
