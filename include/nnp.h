@@ -117,11 +117,19 @@ int nnp_workspace_set_units(nnp_workspace*, double angstrom_per_length_unit, dou
  * in 2^-32 fixed point (reproducible).  NULL (default) switches it off; the pointer must stay valid while set. */
 int nnp_workspace_set_virial_output(nnp_workspace*, double* d_virial9);
 
-/* Small-system front end (the ML/MM regime of PAPER.md lines 108, 140, 154, 164: 14-107
- * ML atoms, where per-step latency is what counts).  on != 0 (default): a periodic evaluation with at most 256 ML atoms,
- * box lengths <= 64 Angstrom and no external pair list runs species map, ordering, all-pairs neighbour search in shared
- * memory and the AEV as ONE kernel (no grid-wide barriers, no cell list); rows, E and F are those of the general path
- * up to fp32 summation order of the positions' frame.  0: always the general cell-list path. */
+/* Small-system path (the ML/MM regime of PAPER.md lines 108, 140, 154, 164: 14-107 ML
+ * atoms, where per-step latency -- kernel launches -- is what counts).  A periodic orthorhombic evaluation with at most
+ * 256 ML atoms, box lengths <= 64 Angstrom and no external pair list is taken off the general cell-list path:
+ *   on = 2 (default): the WHOLE evaluation is ONE kernel launch with no grid-wide barrier (k_small_all): per-CTA redundant
+ *          ordering, all-pairs neighbour search in shared memory, AEV, the per-element networks forward + backward in
+ *          plain fp32 on CUDA cores (whatever nnp_workspace_set_mlp_mode says: 2 x 10^5 MACs per atom do not fill a
+ *          tensor-core tile), AEV backward, fixed-point force assembly, output by the last CTA to finish.  Needs the
+ *          tensor-core-shaped networks (four layers, widths multiples of 32), no virial output, no unit conversion and
+ *          no stage profiling; otherwise it falls back to on = 1;
+ *   on = 1: only the front end (species map ... AEV) is one kernel; MLP (tensor cores), AEV backward and output follow as
+ *          separate launches (five in all);
+ *   on = 0: always the general cell-list path.
+ * Rows, E and F are those of the general path up to fp32 summation order (and the MLP arithmetic mode). */
 int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
 
 /* Verlet-buffered reuse of the cell binning AND the neighbour rows over several MD steps (

@@ -82,8 +82,8 @@ extern "C" int nnp_model_create_ensemble(const nnp_aev_params* p, const nnp_mlp_
     c.zlut[z] = (int8_t)s;
     for (int l = 0; l < d.n_layers; ++l) {
       const size_t in = (l == 0) ? (size_t)m->Kfull : (size_t)d.dims[l];
-      total += in * d.dims[l + 1] + (size_t)d.dims[l + 1];
-      total = (total + 3) & ~(size_t)3;
+      total += 2 * in * d.dims[l + 1] + (size_t)d.dims[l + 1];   // W [out][in], its transpose [in][out], b
+      total = (total + 7) & ~(size_t)7;
     }
   }
   if (nl_common == 0) { delete m; return NNP_ERR_INVALID_ARG; }
@@ -125,7 +125,17 @@ extern "C" int nnp_model_create_ensemble(const nnp_aev_params* p, const nnp_mlp_
       for (int o = 0; o < outw; ++o) blob[off + o] = d.b[l][o];
       off += outw;
       off = (off + 3) & ~(size_t)3;
-      n.WT[l] = nullptr;
+      // transposed copy [in][out] (layer 0: [Kfull][out]): the single-kernel small-system path reads forward weights with
+      // the output neuron on the thread index (coalesced), backward weights from W
+      n.WT[l] = dbase + off;
+      for (int o = 0; o < outw; ++o)
+        for (int i = 0; i < in; ++i) {
+          size_t col = (size_t)i;
+          if (l == 0 && i >= S * NSHFR) col = (size_t)c.nRB * BLK + (size_t)(i - S * NSHFR);
+          blob[off + col * outw + o] = d.W[l][(size_t)o * in + i];
+        }
+      off += ldw * outw;
+      off = (off + 3) & ~(size_t)3;
     }
   }
   if (cudaMemcpy(dbase, blob.data(), total * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -133,8 +143,12 @@ extern "C" int nnp_model_create_ensemble(const nnp_aev_params* p, const nnp_mlp_
   }
   m->dev_blob = dbase; m->blob_bytes = total * sizeof(float);
   m->tc = nullptr;
+  if (cudaMalloc((void**)&m->d_nets, sizeof(NetTable) * MAX_MEMBERS) != cudaSuccess ||
+      cudaMemcpy(m->d_nets, m->nets, sizeof(NetTable) * MAX_MEMBERS, cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaGetLastError(); if (m->d_nets) cudaFree(m->d_nets); cudaFree(dbase); delete m; return NNP_ERR_CUDA;
+  }
   int rc = tc_model_create(m, nets_all);
-  if (rc != NNP_OK) { cudaFree(dbase); delete m; return rc; }
+  if (rc != NNP_OK) { cudaFree(m->d_nets); cudaFree(dbase); delete m; return rc; }
   *out = m;
   return NNP_OK;
 }
@@ -142,6 +156,7 @@ extern "C" int nnp_model_create_ensemble(const nnp_aev_params* p, const nnp_mlp_
 extern "C" int nnp_model_destroy(nnp_model* m) {
   if (!m) return NNP_OK;
   tc_model_destroy(m);
+  if (m->d_nets) cudaFree(m->d_nets);
   if (m->dev_blob) cudaFree(m->dev_blob);
   delete m;
   return NNP_OK;
@@ -167,7 +182,7 @@ extern "C" int nnp_workspace_destroy(nnp_workspace* ws) {
   cudaStreamSynchronize(ws->stream);
   tc_workspace_destroy(ws);
   for (int i = 0; i < 6; ++i) if (ws->ev[i]) cudaEventDestroy(ws->ev[i]);
-  void* ptrs[] = {ws->wideR, ws->cntW, ws->spos_ref, ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
+  void* ptrs[] = {ws->small_acc, ws->small_ticket, ws->wideR, ws->cntW, ws->spos_ref, ws->cellbuf, ws->cellfill, ws->present, ws->grid, ws->groups, ws->tiles, ws->flags, ws->cell_count, ws->bstart, ws->tmp4, ws->rank, ws->spos,
                   ws->scell, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, ws->aev, ws->daev, ws->hbuf[0], ws->hbuf[1],
                   ws->hbuf[2], ws->dbuf[0], ws->dbuf[1], ws->e_atom, ws->facc, ws->epart, ws->ticket, ws->wcentre, ws->wblk, ws->pos_scaled, ws->hd_pos, ws->hd_Z, ws->hd_ml,
                   ws->hd_forces};
@@ -202,6 +217,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
     ws->num_sms = sms;
     ws->prep_cluster = prep_cluster_size();
     ws->small_path = 1;
+    ws->small_all = 1;
     ws->prep_cluster_max = 8192;   // measured: 24 000 atoms run 4 us slower in one cluster than on the cooperative grid
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
@@ -228,6 +244,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
          cudaHostAlloc((void**)&ws->hml_copy, sizeof(int32_t) * std::max<size_t>(nm, 1), cudaHostAllocDefault) == cudaSuccess;
     if (ok) *ws->hd_energy = 0.0;
   }
+  if (ok) ok = dmalloc(&ws->small_acc, 3 * 256) && dmalloc(&ws->small_ticket, 1) && small_all_prepare(ws) == NNP_OK;
   if (ok) ok = (tc_workspace_create(ws) == NNP_OK);
   if (!ok || cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); nnp_workspace_destroy(ws); return NNP_ERR_CUDA; }
   *out = ws;
@@ -311,6 +328,7 @@ extern "C" int nnp_workspace_set_bin_reuse(nnp_workspace* ws, int32_t every_n, d
 extern "C" int nnp_workspace_set_small_path(nnp_workspace* ws, int32_t on) {
   if (!ws) return NNP_ERR_INVALID_ARG;
   ws->small_path = on ? 1 : 0;
+  ws->small_all = (on == 1) ? 0 : 1;   // 1: the front end only (five launches); any other non-zero value (default 2): one kernel
   return NNP_OK;
 }
 
@@ -353,6 +371,12 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   int nl = 0;
   float box_a[9];
   ws->tile_done = nullptr;
+  // small periodic ML region, everything in ONE kernel: no memset, no other launch
+  if (ws->len_scale == 1.0 && small_all_applicable(ws, box, pbc, n_ml)) {
+    ws->launches = launch_small_all(ws, d_pos, d_Z, box, d_ml, n_atoms, n_ml, d_energy, d_forces);
+    if (cudaGetLastError() != cudaSuccess) return NNP_ERR_CUDA;
+    return NNP_OK;
+  }
   // rows of non-ML atoms are +0.0f; with no index subset every row is written by k_force_out
   if (n_atoms > 0 && (d_ml || n_ml <= 0)) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
   if (ws->len_scale != 1.0) {   // unit conversion (GROMACS: nm -> Angstrom), see nnp_workspace_set_units

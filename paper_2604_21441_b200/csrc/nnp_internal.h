@@ -122,6 +122,7 @@ struct nnp_model {
   void* dev_blob;            // single allocation holding all fp32 weights
   size_t blob_bytes;
   void* tc;                  // tensor-core weight images (mlp_tc.cu), or nullptr
+  nnp::NetTable* d_nets;     // DEVICE copy of nets[] (the single-kernel small-system path reads the tables from global memory)
 };
 
 struct nnp_workspace {
@@ -136,6 +137,10 @@ struct nnp_workspace {
   int mlp_mode;
   int dense_k;               // 1: materialise every column block (no structural-zero compaction)
   int small_path;            // 1 (default): small periodic ML regions take the single-kernel front end (small.cu)
+  int small_all;             // 1 (default): ... and, where applicable, the whole evaluation as ONE kernel (k_small_all)
+  unsigned long long* small_acc;   // [256 * 3] force accumulators of k_small_all (zero between evaluations)
+  unsigned int* small_ticket;
+  size_t small_all_smem;
   int64_t max_rows;          // padded AEV rows
   int max_tiles;
   // last evaluation
@@ -226,6 +231,10 @@ bool box_is_triclinic(const float* box);
 bool neighbor_box_ok(const nnp_workspace* ws, const float* box);
 int launch_aev_forward(nnp_workspace* ws, int64_t n_ml);
 bool small_front_applicable(const nnp_workspace* ws, const float* box, int pbc, int64_t n_ml);
+bool small_all_applicable(const nnp_workspace* ws, const float* box, int pbc, int64_t n_ml);
+int launch_small_all(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, const int32_t* d_ml,
+                     int64_t n_atoms, int64_t n_ml, double* d_energy, float* d_forces);
+int small_all_prepare(nnp_workspace* ws);
 int launch_small_front(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z, const float* box, const int32_t* d_ml,
                        int64_t n_atoms, int64_t n_ml);
 int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);

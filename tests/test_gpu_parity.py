@@ -476,6 +476,7 @@ def test_virial_output(k):
     om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
     ref = oracle.evaluate_virial(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nbr_mode=1 if n_ml > 2000 else 0)
     m, ws = make(cfg)
+    ws.set_small_path(1)     # (the one-kernel small-system path has no virial output: keep one path for the bitwise comparison)
     E0, F0 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
     W = torch.zeros(9, dtype=torch.float64, device="cuda")
     ws.set_virial_output(W)
@@ -589,10 +590,10 @@ def test_small_path_and_general_path(k, layout):
     ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, want_aev=True)
     m, ws = make(cfg)
     out = {}
-    for on in (1, 0):
+    for on in (2, 1, 0):     # one kernel (default) / front end + four stage kernels / general cell-list path
         ws.set_small_path(on)
         E, F = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
-        assert ws.launches() == 5 if on else ws.launches() in (7, 8)   # general path: k_prep, or k_bin_cells + k_cell_sort
+        assert ws.launches() == {2: 1, 1: 5}.get(on, ws.launches()) and ws.launches() in (1, 5, 7, 8)
         check_lists(ws, cfg, cfg["pos"], n_ml, ml)
         G = ws.aev(n_ml).astype(np.float64)
         assert np.all(np.abs(G - ref["aev"]) <= 2e-5 * (1 + np.abs(ref["aev"]))), np.abs(G - ref["aev"]).max()
@@ -600,9 +601,13 @@ def test_small_path_and_general_path(k, layout):
         E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
         assert E2 == E and np.array_equal(F2, F)
         out[on] = (E, F)
-    assert abs(out[1][0] - out[0][0]) / n_ml < 1e-6 and np.abs(out[1][1] - out[0][1]).max() < 1e-4
+    for on in (2, 1):
+        assert abs(out[on][0] - out[0][0]) / n_ml < 1e-6 and np.abs(out[on][1] - out[0][1]).max() < 1e-4
+    mm = None if ml is None else np.setdiff1d(np.arange(n), ml)
+    if mm is not None:   # the single kernel writes the other atoms' rows itself: +0.0f
+        assert np.all(out[2][1][mm] == 0.0) and not np.any(np.signbit(out[2][1][mm]))
     # atoms shifted by whole box vectors: same rows
-    ws.set_small_path(1)
+    ws.set_small_path(2)
     shift = np.random.default_rng(3).integers(-2, 3, size=cfg["pos"].shape).astype(np.float32)
     pos2 = (cfg["pos"] + shift * np.array([cfg["box"][0], cfg["box"][4], cfg["box"][8]], dtype=np.float32)).astype(np.float32)
     ref2 = oracle.evaluate(om, pos2, cfg["Z"], cfg["box"], 1, ml)
