@@ -47,6 +47,7 @@ struct SmallFrontSmemT {
   GridInfo g_s;
   GroupInfo grp_s;
   int cnt_s[MAX_S], gs[MAX_S + 1], pshift[MAX_S], tb[MAX_S + 1];
+  int wcnt[SMALL_MAX / 32][MAX_S];            // atoms per (warp of the ordering phase, species)
 };
 
 // The centres of CTA b.  Plain: NW consecutive sorted indices.  ALIGNED (k_small_all): every species group is cut into
@@ -82,7 +83,7 @@ __device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<
   const double L[3] = {(double)a.Lx, (double)a.Ly, (double)a.Lz};
 
   // ---- P0: species slot and local coordinates of atom `tid`; force accumulators cleared (sliced over the grid)
-  if (tid < MAX_S) cnt_s[tid] = 0;
+  int myslot = -1, pfx = 0;
   if (facc) for (int k = blockIdx.x * blockDim.x + tid; k < 3 * n; k += gridDim.x * blockDim.x) facc[k] = 0ull;
   __syncthreads();
   if (tid < n) {
@@ -105,15 +106,35 @@ __device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<
     }
     tmp[tid] = make_float4(loc[0], loc[1], loc[2], 0.f);
     skey[tid] = (uint8_t)slot;
-    atomicAdd(&cnt_s[slot], 1);   // integer count: order free
+    myslot = slot;
+  }
+  // place inside the species group = atoms of the same species with a smaller ML index: per warp by ballot (pfx = the
+  // lanes below), across warps by the per-warp counts
+  if (w < SMALL_MAX / 32) {
+    for (int q = 0; q < S; ++q) {
+      const unsigned mq = __ballot_sync(0xffffffffu, myslot == q);
+      if (myslot == q) pfx = __popc(mq & ((1u << lane) - 1u));
+      if (lane == 0) sm.wcnt[w][q] = __popc(mq);
+    }
+  }
+  __syncthreads();
+  if (tid < MAX_S) {
+    int t = 0;
+    if (tid < S) for (int ww = 0; ww < SMALL_MAX / 32; ++ww) t += sm.wcnt[ww][tid];
+    cnt_s[tid] = t;
   }
   __syncthreads();
   // ---- P1: groups, tiles, column map, the one-cell grid
-  if (tid == 0) {
-    int run = 0;
-    for (int q = 0; q <= MAX_S; ++q) { if (q <= S) gs[q] = run; if (q < S) run += cnt_s[q]; }
-    for (int q = S + 1; q <= MAX_S; ++q) gs[q] = run;
-    d_groups(gs, S, n, a.max_tiles, a.dense_k, &grp_s, pshift, tb, a.flags);
+  if (w == 0) {   // groups, tiles and the column set by one warp (d_groups_warp); the grid by a thread of the next warp
+    if (lane == 0) {
+      int run = 0;
+      for (int q = 0; q <= MAX_S; ++q) { if (q <= S) gs[q] = run; if (q < S) run += cnt_s[q]; }
+      for (int q = S + 1; q <= MAX_S; ++q) gs[q] = run;
+    }
+    __syncwarp();
+    d_groups_warp(gs, S, n, a.max_tiles, a.dense_k, &grp_s, pshift, tb, a.flags);
+  }
+  if (tid == 32) {
     g_s.nc[0] = g_s.nc[1] = g_s.nc[2] = 1; g_s.ncell = 1; g_s.pbc = 1; g_s.tric = 0;
     for (int k = 0; k < 9; ++k) { g_s.ev[k] = 0.f; g_s.ev_d[k] = 0.0; }
     for (int k = 0; k < 6; ++k) g_s.H_d[k] = (k < 3) ? L[k] : 0.0;
@@ -138,8 +159,8 @@ __device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<
   // ---- P2: order by (slot, ML index): rank by counting
   if (tid < n) {
     const int slot = skey[tid];
-    int rank = gs[slot];
-    for (int b = 0; b < tid; ++b) rank += (skey[b] == slot) ? 1 : 0;
+    int rank = gs[slot] + pfx;
+    for (int ww = 0; ww < w; ++ww) rank += sm.wcnt[ww][slot];
     float4 v = tmp[tid];
     v.w = __int_as_float(tid | (slot << 28));
     sp[rank] = v;
