@@ -12,7 +12,7 @@
 
 namespace nnp {
 
-__global__ void __launch_bounds__(AEV_FWD_WARPS * 32, 10)
+__global__ void __launch_bounds__(AEV_FWD_WARPS * 32, 20)
 k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
               const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,

@@ -6,8 +6,8 @@
 
 namespace nnp {
 
-constexpr int AEV_WARPS = 8;      // warps (centres) per block of the backward kernel
-constexpr int AEV_FWD_WARPS = 4;  // ... of the forward kernel (measured: 4 -> 71.8 us, 8 -> 73.6 us; backward 8 -> 96 us, 4 -> 99 us)
+constexpr int AEV_WARPS = 4;      // warps (centres) per block of the backward kernel (measured, 80 registers: 8 -> 86.6 us, 4 -> 84.2 us, 2 -> 85.5 us)
+constexpr int AEV_FWD_WARPS = 2;  // ... of the forward kernel (measured, 48 registers: 8 -> 73.6 us, 4 -> 67.3 us, 2 -> 66.5 us)
 
 __device__ __forceinline__ float ex2f(float x) {
   float y;

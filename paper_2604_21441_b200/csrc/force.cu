@@ -13,9 +13,9 @@
 namespace nnp {
 
 template <bool VIRIAL>
-// 3 blocks per SM: 80 registers.  (At 4 blocks / 64 registers the packed-arithmetic version spills ~250 bytes per thread
+// 6 blocks of 4 warps per SM: 80 registers.  (At 4 blocks / 64 registers the packed-arithmetic version spills ~250 bytes per thread
 // inside the triplet loop -- local-memory loads are long-scoreboard stalls: 95 us against 86 us.)
-__global__ void __launch_bounds__(AEV_WARPS * 32, 3)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 6)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
