@@ -269,53 +269,57 @@ __device__ __forceinline__ float celu_grad_s(float a, float alpha) { return a > 
 template <bool MAPK, bool MAPN, class Epi>
 __device__ __forceinline__ void dense_rows(const float* __restrict__ Bp, int sk, int K, int N, const float* __restrict__ in,
                                        const int* __restrict__ blkmap, float* __restrict__ part, int n0, Epi epi) {
-  // thread <-> (n, g): the SA_KSPLIT thread groups of 256 take alternate 32-wide k blocks; groups > 0 hand their partial
-  // sums over through shared memory (part[g - 1][n][8]).  Per k block the 32 weights are loaded first (all in flight: the
-  // weights come from L2, ~600 cycles away), then the 256 FMAs run from registers and broadcast shared loads.
-  const int nl = threadIdx.x & 255, n = n0 + nl, grp_id = threadIdx.x >> 8;
-  float acc[SA_R];
+  // Phase A: thread <-> (four consecutive n, k group): the 8 thread groups of 64 take four k of every 32-wide k block each,
+  // weights as 128-bit loads (four neurons per load: a quarter of the load instructions of a thread-per-neuron mapping --
+  // on ONE SM the phase is bound by load instructions, not by FMAs), two k blocks (8 loads) in flight per thread.
+  // Phase B: the partial sums meet in shared memory (part[k group][n][row]); thread <-> n adds the 8 groups in order.
+  static_assert(SA_R == 2 && SA_THREADS == 512, "dense_rows mapping");
+  const int n4 = threadIdx.x & 63, kg = threadIdx.x >> 6;
+  const int n = n0 + 4 * n4;
+  float acc[4][SA_R];
 #pragma unroll
-  for (int r = 0; r < SA_R; ++r) acc[r] = 0.f;
+  for (int j = 0; j < 4; ++j)
+#pragma unroll
+    for (int r = 0; r < SA_R; ++r) acc[j][r] = 0.f;
   if (n < N) {
     const int ncol = MAPN ? blkmap[n >> 5] * BLK + (n & 31) : n;
-    for (int k0 = 32 * grp_id; k0 < K; k0 += 32 * SA_KSPLIT) {     // K is a multiple of 32 (hidden widths, compact AEV blocks)
-      const int kb = MAPK ? blkmap[k0 >> 5] * BLK : k0;
-      const float* bp = Bp + (size_t)kb * sk + ncol;
-      float wv[32];
+    for (int k0 = 0; k0 < K; k0 += 64) {     // K is a multiple of 32 (hidden widths, compact AEV blocks)
+      float4 wv[8];
 #pragma unroll
-      for (int kk = 0; kk < 32; ++kk) wv[kk] = __ldg(bp + (size_t)kk * sk);
+      for (int u = 0; u < 8; ++u) {
+        const int k = k0 + 32 * (u >> 2) + 4 * kg + (u & 3);
+        const int kr = MAPK ? blkmap[min(k, K - 1) >> 5] * BLK + (k & 31) : k;
+        wv[u] = k < K ? __ldg(reinterpret_cast<const float4*>(Bp + (size_t)kr * sk + ncol)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
 #pragma unroll
-      for (int kk = 0; kk < 32; ++kk) {
-        float x[SA_R];
-        if (SA_R == 2) { const float2 v = *reinterpret_cast<const float2*>(in + (k0 + kk) * SA_R); x[0] = v.x; x[SA_R - 1] = v.y; }
-        else {
-#pragma unroll
-          for (int r = 0; r < SA_R; r += 4) {
-            const float4 v = *reinterpret_cast<const float4*>(in + (k0 + kk) * SA_R + r);
-            x[r] = v.x; x[r + 1] = v.y; x[r + 2] = v.z; x[r + 3] = v.w;
-          }
-        }
-#pragma unroll
-        for (int r = 0; r < SA_R; ++r) acc[r] = fmaf(wv[kk], x[r], acc[r]);
+      for (int u = 0; u < 8; ++u) {
+        const int k = min(k0 + 32 * (u >> 2) + 4 * kg + (u & 3), K - 1);
+        const float2 x = *reinterpret_cast<const float2*>(in + k * SA_R);
+        acc[0][0] = fmaf(wv[u].x, x.x, acc[0][0]); acc[0][1] = fmaf(wv[u].x, x.y, acc[0][1]);
+        acc[1][0] = fmaf(wv[u].y, x.x, acc[1][0]); acc[1][1] = fmaf(wv[u].y, x.y, acc[1][1]);
+        acc[2][0] = fmaf(wv[u].z, x.x, acc[2][0]); acc[2][1] = fmaf(wv[u].z, x.y, acc[2][1]);
+        acc[3][0] = fmaf(wv[u].w, x.x, acc[3][0]); acc[3][1] = fmaf(wv[u].w, x.y, acc[3][1]);
       }
     }
-    if (grp_id > 0) {
 #pragma unroll
-      for (int r = 0; r < SA_R; ++r) part[((size_t)(grp_id - 1) * 256 + nl) * SA_R + r] = acc[r];
-    }
+    for (int j = 0; j < 4; ++j)
+      *reinterpret_cast<float2*>(part + ((size_t)kg * 256 + 4 * n4 + j) * SA_R) = make_float2(acc[j][0], acc[j][1]);
   }
   __syncthreads();
-  if (grp_id == 0 && n < N) {
+  const int nl = threadIdx.x, nn = n0 + nl;
+  if (nl < 256 && nn < N) {
+    float o[SA_R] = {0.f, 0.f};
 #pragma unroll
-    for (int gq = 1; gq < SA_KSPLIT; ++gq)
-#pragma unroll
-      for (int r = 0; r < SA_R; ++r) acc[r] += part[((size_t)(gq - 1) * 256 + nl) * SA_R + r];
-    epi(n, acc);
+    for (int g8 = 0; g8 < 8; ++g8) {
+      const float2 v = *reinterpret_cast<const float2*>(part + ((size_t)g8 * 256 + nl) * SA_R);
+      o[0] += v.x; o[1] += v.y;
+    }
+    epi(nn, o);
   }
 }
 
 // forward + backward of the network of species s for the CTA's rows (centres ip_first .. ip_first + n_rows - 1).
-// mb = shared-memory floats: x[Kc][8], h1..h3[HP][8], d3..d1[HP][8], red[warps][8], part[SA_KSPLIT - 1][256][8]
+// mb = shared-memory floats: x[Kc][R], h1..h3[HP][R], d3..d1[HP][R], red[warps][R], part[8][256][R]  (R = SA_R rows)
 __device__ __forceinline__ void small_mlp(const SmallAllArgs& a, const GroupInfo& grp, int s, int ip_first, int n_rows, float* mb) {
   const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
   const int Kc = grp.Kc;
@@ -327,7 +331,7 @@ __device__ __forceinline__ void small_mlp(const SmallAllArgs& a, const GroupInfo
   float* d2 = d3 + HP * SA_R;
   float* d1 = d2 + HP * SA_R;
   float* red = d1 + HP * SA_R;                 // [warps][8]
-  float* part = red + (SA_THREADS / 32) * SA_R;   // [SA_KSPLIT - 1][256][8]
+  float* part = red + (SA_THREADS / 32) * SA_R;   // [8 k groups][256][SA_R]
   const float escale = 1.0f / (float)a.n_members;
   {
     int rowof[SA_R];
@@ -485,7 +489,7 @@ __global__ void __launch_bounds__(SA_THREADS, 1) k_small_all(const __grid_consta
 
 size_t small_all_smem(const nnp_model* m) {
   const size_t front = (sizeof(SmallFrontSmemT<SA_R>) + 15) & ~(size_t)15;
-  const size_t mlp = ((size_t)m->Kfull * SA_R + 6 * (size_t)HP * SA_R + (SA_THREADS / 32) * SA_R + (size_t)(SA_KSPLIT - 1) * 256 * SA_R) * sizeof(float);
+  const size_t mlp = ((size_t)m->Kfull * SA_R + 6 * (size_t)HP * SA_R + (SA_THREADS / 32) * SA_R + (size_t)8 * 256 * SA_R) * sizeof(float);
   return front + std::max(mlp, sizeof(SmallBwdSmem));
 }
 
