@@ -145,7 +145,7 @@ int nnp_workspace_set_small_path(nnp_workspace*, int32_t on);
  * nnp_status() (outputs of that step unspecified, the next evaluation rebuilds).  skin in the caller's length unit.
  * Periodic boxes (orthorhombic or triclinic) on the cell-list path; with an external pair list set only the binning is
  * reused (the list is the engine's own buffered list); open boundaries and the small-system front end keep rebuilding every
- * step.  The first call with every_n > 1 allocates the wide rows (768 bytes per ML atom).  The step counter lives on the
+ * step.  The first call with every_n > 1 allocates the wide rows (256 entries = 1 KB per ML atom; liquid water at skin 1 A: about 105 entries; a row that does not fit raises NNP_ERR_CAPACITY).  The step counter lives on the
  * host: a CUDA graph captures whichever kind of step it was recorded on. */
 int nnp_workspace_set_bin_reuse(nnp_workspace*, int32_t every_n, double skin);
 

@@ -168,8 +168,8 @@ __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const Grid
       for (int h = 0; h < 2; ++h) {
         const int s = 2 * b + h;
         float acc = 0.f;
-        if (s < c.S) {
-          const int q0 = e.segR[s], q1 = e.segR[s + 1];
+        const int q0 = (s < c.S) ? e.segR[s] : 0, q1 = (s < c.S) ? e.segR[s + 1] : 0;
+        if (q1 > q0) {   // (warp-uniform; a species without neighbours -- most of the slots in water -- costs nothing)
           const int qa = (q0 + 1) & ~1, qb = q1 & ~1;
           float2 acc2 = make_float2(0.f, 0.f);
           for (int pp = (qa >> 1) + half; pp < (qb >> 1); pp += 2) {
@@ -187,8 +187,8 @@ __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const Grid
             const float x = rp[0] - shf;
             acc = fmaf(rp[2], ex2f(-x * x), acc);
           }
+          acc += __shfl_xor_sync(0xffffffffu, acc, 16);
         }
-        acc += __shfl_xor_sync(0xffffffffu, acc, 16);
         if (half == h) out = acc;
       }
       row[cp * BLK + lane] = out;

@@ -307,7 +307,7 @@ extern "C" int nnp_workspace_set_pair_list(nnp_workspace* ws, const int32_t* d_p
 extern "C" int nnp_workspace_set_bin_reuse(nnp_workspace* ws, int32_t every_n, double skin) {
   if (!ws || (every_n > 1 && !(skin > 0.0))) return NNP_ERR_INVALID_ARG;
   if (every_n > 1 && !ws->wideR) {   // first use: the wide rows of the row reuse (allocated here, never inside nnp_eval)
-    ws->wcap = 192;
+    ws->wcap = 256;
     const size_t nm = (size_t)std::max<int64_t>(ws->max_ml, 1);
     if (cudaMalloc((void**)&ws->wideR, nm * ws->wcap * sizeof(uint32_t)) != cudaSuccess ||
         cudaMalloc((void**)&ws->cntW, nm * sizeof(int)) != cudaSuccess ||
