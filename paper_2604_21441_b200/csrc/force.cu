@@ -13,9 +13,11 @@
 namespace nnp {
 
 template <bool VIRIAL>
-// 6 blocks of 4 warps per SM: 80 registers.  (At 4 blocks / 64 registers the packed-arithmetic version spills ~250 bytes per thread
-// inside the triplet loop -- local-memory loads are long-scoreboard stalls: 95 us against 86 us.)
-__global__ void __launch_bounds__(AEV_WARPS * 32, 6)
+// 7 blocks of 4 warps per SM: 72 registers, 32 bytes of spills outside the triplet loop.  Alone the kernel gains little over
+// 6 blocks / 80 registers (84.2 -> 83.5 us), but the step gains 5 us (253.4 -> 248.4 us, same box, alternating runs): while the
+// MLP's second wave holds 40 SMs, the extra warps on the other 108 hide more of the gather latency.  (8 blocks / 64
+// registers spill ~250 bytes per thread inside the triplet loop -- local-memory loads are long-scoreboard stalls: 95 us.)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 7)
 k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __restrict__ grp,
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
