@@ -109,6 +109,132 @@ __device__ __forceinline__ void decode_same(int t, int n, float inv_n, int& j, i
   if (k >= n) k -= n;
 }
 
+// Radial block b of a centre: species 2b (columns 0-15) and 2b+1 (columns 16-31); lane & 15 <-> shift.  The two
+// half-warps take alternate PAIRS of neighbours of the species' segment (one 128-bit load, packed arithmetic); the at
+// most two entries of a segment that do not fill an aligned pair are taken one by one.
+__device__ __forceinline__ float fwd_radial_block(const AevConst& c, const FwdEnv& e, int b, int lane) {
+  const int m = lane & 15, half = lane >> 4;
+  const float shf = c.ShfR[m] * sqrtf(c.etaR_l2e);
+  const float2 nshf2 = make_float2(-shf, -shf);
+  const float* radf = reinterpret_cast<const float*>(e.rad);
+  float out = 0.f;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int s = 2 * b + h;
+    float acc = 0.f;
+    const int q0 = (s < c.S) ? e.segR[s] : 0, q1 = (s < c.S) ? e.segR[s + 1] : 0;
+    if (q1 > q0) {   // (warp-uniform; a species without neighbours -- most of the slots in water -- costs nothing)
+      const int qa = (q0 + 1) & ~1, qb = q1 & ~1;
+      float2 acc2 = make_float2(0.f, 0.f);
+      for (int pp = (qa >> 1) + half; pp < (qb >> 1); pp += 2) {
+        const float4 v = e.rad[pp];
+        const float2 x = __fadd2_rn(make_float2(v.x, v.y), nshf2);
+        const float2 t = __fmul2_rn(x, x);
+        acc2 = __ffma2_rn(make_float2(v.z, v.w), make_float2(ex2f(-t.x), ex2f(-t.y)), acc2);
+      }
+      acc = acc2.x + acc2.y;
+      int ql = -1;
+      if (half == 0 && (q0 & 1) && q0 < q1) ql = q0;
+      if (half == 1 && (q1 & 1) && q1 - 1 >= qa) ql = q1 - 1;
+      if (ql >= 0) {
+        const float* rp = radf + ((ql >> 1) << 2) + (ql & 1);
+        const float x = rp[0] - shf;
+        acc = fmaf(rp[2], ex2f(-x * x), acc);
+      }
+      acc += __shfl_xor_sync(0xffffffffu, acc, 16);
+    }
+    if (half == h) out = acc;
+  }
+  return out;
+}
+
+// Phase 1 of the angular part for the chunk of FWD_TCH triplets at c0: lane <-> triplet c0 + lane; the 12 factors go to
+// fac[0..3][lane] (F2_a) and fac[4..11][lane] (B_z^zeta).  bp1 = first block that reaches into the chunk (advanced here).
+__device__ __forceinline__ void fwd_factors(const AevConst& c, const FwdEnv& e, float (*fac)[FWD_TP], int npb, int c0, int lane,
+                                            int& bp1) {
+      const int tp = c0 + lane;
+  while (e.boff[bp1 + 1] <= c0) ++bp1;             // first block that reaches into this chunk (warp-uniform)
+  int b = bp1;
+  for (int bb = bp1 + 1; bb < npb && e.boff[bb] < c0 + FWD_TCH; ++bb) if (tp >= e.boff[bb]) b = bb;
+  const int2 ent = e.btab[b];
+  const int t = tp - e.boff[b], T = ent.y >> 16;
+  const int a1 = ent.x & 255, a2 = (ent.x >> 16) & 255;
+  const bool live = t < T;
+  int j = a1, k = a1;
+  if (live) {
+    // same species: round-robin pairing over the n1 neighbours (decode_same); else the n1 x n2 grid, k fastest
+    const bool same = (ent.y & 256) != 0;
+    const int n = same ? ((ent.x >> 8) & 255) : ((ent.x >> 24) & 255);
+    const int r = (int)(((float)t + 0.5f) * e.binv[b]);
+    const int rem = t - r * n;
+    int ks = rem + r + 1;
+    if (ks >= n) ks -= n;
+    j = a1 + (same ? rem : r);
+    k = same ? a1 + ks : a2 + rem;
+  }
+  const float4 uj = e.ua[j], uk = e.ua[k];
+  const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
+  const float cc = c.cTheta * u;
+  const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.f));
+  const float Rbar = 0.5f * (uj.w + uk.w);
+  const float ff2 = live ? 2.0f * e.fA[j] * e.fA[k] : 0.f;
+#pragma unroll
+  for (int a = 0; a < NSHFA; a += 2) {
+    const float2 x = __fadd2_rn(make_float2(Rbar, Rbar), make_float2(-c.ShfA[a], -c.ShfA[a + 1]));
+    const float2 y = __fmul2_rn(x, x);
+    const float2 F = __fmul2_rn(make_float2(ex2f(-c.etaA_l2e * y.x), ex2f(-c.etaA_l2e * y.y)), make_float2(ff2, ff2));
+    fac[a][lane] = F.x; fac[a + 1][lane] = F.y;
+  }
+  if (c.zeta_is_32) {
+    const float2 cc2 = make_float2(cc, cc), ss2 = make_float2(ss, ss), h2 = make_float2(0.5f, 0.5f);
+#pragma unroll
+    for (int z = 0; z < NSHFZ; z += 2) {
+      const float2 cd = __ffma2_rn(cc2, make_float2(c.cosZ[z], c.cosZ[z + 1]), __fmul2_rn(ss2, make_float2(c.sinZ[z], c.sinZ[z + 1])));
+      const float2 B = __ffma2_rn(h2, cd, h2);      // (1 + cos(theta - ShfZ)) / 2; B^32 >= 0 whatever the rounding of B
+      const float2 B2 = __fmul2_rn(B, B), B4 = __fmul2_rn(B2, B2), B8 = __fmul2_rn(B4, B4), B16 = __fmul2_rn(B8, B8);
+      const float2 B32 = __fmul2_rn(B16, B16);
+      fac[4 + z][lane] = B32.x; fac[5 + z][lane] = B32.y;
+    }
+  } else {
+#pragma unroll
+    for (int z = 0; z < NSHFZ; ++z) {
+      const float B = fmaf(0.5f, fmaf(cc, c.cosZ[z], ss * c.sinZ[z]), 0.5f);
+      float Bz, Bm;
+      bpow(c, fmaxf(B, 0.f), Bz, Bm);
+      fac[4 + z][lane] = Bz;
+    }
+  }
+}
+
+// Species-pair block table of a centre (lane b <-> b-th pair of species present, i1 <= i2): e.btab / e.binv / e.boff.
+__device__ __forceinline__ void fwd_block_table(const AevConst& c, const GroupInfo* __restrict__ grp, FwdEnv& e, int np, int npb,
+                                                int lane) {
+  int run = 0;
+  for (int b0 = 0; b0 < npb; b0 += 32) {
+    const int b = b0 + lane;
+    int T = 0;
+    int2 ent = make_int2(0, 0);
+    float inv = 0.f;
+    if (b < npb) {
+      int p = b, i1 = 0;
+      while (p >= np - i1) { p -= np - i1; ++i1; }
+      const int s1 = grp->pres[i1], s2 = grp->pres[i1 + p];
+      const int a1 = e.segA[s1], n1 = e.segA[s1 + 1] - a1, a2 = e.segA[s2], n2 = e.segA[s2 + 1] - a2;
+      const bool same = (s1 == s2);
+      T = same ? (n1 * (n1 - 1)) / 2 : n1 * n2;
+      const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)];
+      ent = make_int2(a1 | (n1 << 8) | (a2 << 16) | (n2 << 24), (cp & 255) | ((same ? 1 : 0) << 8) | (T << 16));
+      inv = 1.0f / (float)max(same ? n1 : n2, 1);
+    }
+    int inc = (T + 3) & ~3;
+    const int own = inc;
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    if (b < npb) { e.btab[b] = ent; e.binv[b] = inv; e.boff[b] = run + inc - own; }
+    run += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  if (lane == 0) e.boff[npb] = run;
+}
+
 // AEV row of centre ip (sorted index) from its neighbour rows rowR / rowA; all 32 lanes of the warp call this with the
 // warp's FwdEnv staging.  (spos, g, grp and the rows may live in shared memory: small.cu.)
 __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const GridInfo* __restrict__ g,
@@ -121,77 +247,16 @@ __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const Grid
   const int Kc = grp->Kc;
   float* __restrict__ row = aev + (size_t)(ip + grp->pad_shift[si]) * Kc;
 
-  // ---- species-pair block table of this centre (lane b <-> b-th pair of species present, i1 <= i2)
   const int np = grp->npres;
   const int npb = np * (np + 1) / 2;
-  {
-    int run = 0;
-    for (int b0 = 0; b0 < npb; b0 += 32) {
-      const int b = b0 + lane;
-      int T = 0;
-      int2 ent = make_int2(0, 0);
-      float inv = 0.f;
-      if (b < npb) {
-        int p = b, i1 = 0;
-        while (p >= np - i1) { p -= np - i1; ++i1; }
-        const int s1 = grp->pres[i1], s2 = grp->pres[i1 + p];
-        const int a1 = e.segA[s1], n1 = e.segA[s1 + 1] - a1, a2 = e.segA[s2], n2 = e.segA[s2 + 1] - a2;
-        const bool same = (s1 == s2);
-        T = same ? (n1 * (n1 - 1)) / 2 : n1 * n2;
-        const int cp = grp->cpos[c.nRB + s1 * c.S - (s1 * (s1 - 1)) / 2 + (s2 - s1)];
-        ent = make_int2(a1 | (n1 << 8) | (a2 << 16) | (n2 << 24), (cp & 255) | ((same ? 1 : 0) << 8) | (T << 16));
-        inv = 1.0f / (float)max(same ? n1 : n2, 1);
-      }
-      int inc = (T + 3) & ~3;
-      const int own = inc;
-      for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-      if (b < npb) { e.btab[b] = ent; e.binv[b] = inv; e.boff[b] = run + inc - own; }
-      run += __shfl_sync(0xffffffffu, inc, 31);
-    }
-    if (lane == 0) e.boff[npb] = run;
-  }
+  fwd_block_table(c, grp, e, np, npb, lane);
 
-  // ---- radial: block b holds species 2b (columns 0-15) and 2b+1 (columns 16-31); lane & 15 <-> shift.  The two
-  // half-warps take alternate PAIRS of neighbours of the species' segment (one 128-bit load, packed arithmetic); the
-  // at most two entries of a segment that do not fill an aligned pair are taken one by one.
+  // ---- radial
   {
-    const int m = lane & 15, half = lane >> 4;
-    const float rscale = sqrtf(c.etaR_l2e);
-    const float shf = c.ShfR[m] * rscale;
-    const float2 nshf2 = make_float2(-shf, -shf);
-    const float* radf = reinterpret_cast<const float*>(e.rad);
     for (int b = 0; b < c.nRB; ++b) {
       const int cp = grp->cpos[b];
       if (cp < 0) continue;
-      float out = 0.f;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int s = 2 * b + h;
-        float acc = 0.f;
-        const int q0 = (s < c.S) ? e.segR[s] : 0, q1 = (s < c.S) ? e.segR[s + 1] : 0;
-        if (q1 > q0) {   // (warp-uniform; a species without neighbours -- most of the slots in water -- costs nothing)
-          const int qa = (q0 + 1) & ~1, qb = q1 & ~1;
-          float2 acc2 = make_float2(0.f, 0.f);
-          for (int pp = (qa >> 1) + half; pp < (qb >> 1); pp += 2) {
-            const float4 v = e.rad[pp];
-            const float2 x = __fadd2_rn(make_float2(v.x, v.y), nshf2);
-            const float2 t = __fmul2_rn(x, x);
-            acc2 = __ffma2_rn(make_float2(v.z, v.w), make_float2(ex2f(-t.x), ex2f(-t.y)), acc2);
-          }
-          acc = acc2.x + acc2.y;
-          int ql = -1;
-          if (half == 0 && (q0 & 1) && q0 < q1) ql = q0;
-          if (half == 1 && (q1 & 1) && q1 - 1 >= qa) ql = q1 - 1;
-          if (ql >= 0) {
-            const float* rp = radf + ((ql >> 1) << 2) + (ql & 1);
-            const float x = rp[0] - shf;
-            acc = fmaf(rp[2], ex2f(-x * x), acc);
-          }
-          acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-        }
-        if (half == h) out = acc;
-      }
-      row[cp * BLK + lane] = out;
+      row[cp * BLK + lane] = fwd_radial_block(c, e, b, lane);
     }
   }
   // in dense-K mode the angular blocks of absent species pairs are zero-filled (same lane, same address as any later
@@ -209,61 +274,7 @@ __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const Grid
   int bcur = 0;   // block the phase-2 accumulator belongs to
   int bp1 = 0;    // first block of the chunk phase 1 is working on
   for (int c0 = 0; c0 < Ttot; c0 += FWD_TCH) {
-    // phase 1: lane <-> triplet c0 + lane
-    {
-      const int tp = c0 + lane;
-      while (e.boff[bp1 + 1] <= c0) ++bp1;             // first block that reaches into this chunk (warp-uniform)
-      int b = bp1;
-      for (int bb = bp1 + 1; bb < npb && e.boff[bb] < c0 + FWD_TCH; ++bb) if (tp >= e.boff[bb]) b = bb;
-      const int2 ent = e.btab[b];
-      const int t = tp - e.boff[b], T = ent.y >> 16;
-      const int a1 = ent.x & 255, a2 = (ent.x >> 16) & 255;
-      const bool live = t < T;
-      int j = a1, k = a1;
-      if (live) {
-        // same species: round-robin pairing over the n1 neighbours (decode_same); else the n1 x n2 grid, k fastest
-        const bool same = (ent.y & 256) != 0;
-        const int n = same ? ((ent.x >> 8) & 255) : ((ent.x >> 24) & 255);
-        const int r = (int)(((float)t + 0.5f) * e.binv[b]);
-        const int rem = t - r * n;
-        int ks = rem + r + 1;
-        if (ks >= n) ks -= n;
-        j = a1 + (same ? rem : r);
-        k = same ? a1 + ks : a2 + rem;
-      }
-      const float4 uj = e.ua[j], uk = e.ua[k];
-      const float u = fmaf(uj.x, uk.x, fmaf(uj.y, uk.y, uj.z * uk.z));
-      const float cc = c.cTheta * u;
-      const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.f));
-      const float Rbar = 0.5f * (uj.w + uk.w);
-      const float ff2 = live ? 2.0f * e.fA[j] * e.fA[k] : 0.f;
-#pragma unroll
-      for (int a = 0; a < NSHFA; a += 2) {
-        const float2 x = __fadd2_rn(make_float2(Rbar, Rbar), make_float2(-c.ShfA[a], -c.ShfA[a + 1]));
-        const float2 y = __fmul2_rn(x, x);
-        const float2 F = __fmul2_rn(make_float2(ex2f(-c.etaA_l2e * y.x), ex2f(-c.etaA_l2e * y.y)), make_float2(ff2, ff2));
-        e.fac[a][lane] = F.x; e.fac[a + 1][lane] = F.y;
-      }
-      if (c.zeta_is_32) {
-        const float2 cc2 = make_float2(cc, cc), ss2 = make_float2(ss, ss), h2 = make_float2(0.5f, 0.5f);
-#pragma unroll
-        for (int z = 0; z < NSHFZ; z += 2) {
-          const float2 cd = __ffma2_rn(cc2, make_float2(c.cosZ[z], c.cosZ[z + 1]), __fmul2_rn(ss2, make_float2(c.sinZ[z], c.sinZ[z + 1])));
-          const float2 B = __ffma2_rn(h2, cd, h2);      // (1 + cos(theta - ShfZ)) / 2; B^32 >= 0 whatever the rounding of B
-          const float2 B2 = __fmul2_rn(B, B), B4 = __fmul2_rn(B2, B2), B8 = __fmul2_rn(B4, B4), B16 = __fmul2_rn(B8, B8);
-          const float2 B32 = __fmul2_rn(B16, B16);
-          e.fac[4 + z][lane] = B32.x; e.fac[5 + z][lane] = B32.y;
-        }
-      } else {
-#pragma unroll
-        for (int z = 0; z < NSHFZ; ++z) {
-          const float B = fmaf(0.5f, fmaf(cc, c.cosZ[z], ss * c.sinZ[z]), 0.5f);
-          float Bz, Bm;
-          bpow(c, fmaxf(B, 0.f), Bz, Bm);
-          e.fac[4 + z][lane] = Bz;
-        }
-      }
-    }
+    fwd_factors(c, e, e.fac, npb, c0, lane, bp1);
     __syncwarp();
     // phase 2: lane <-> sub-feature (a, z): acc += F2_a[t] * B_z[t]; block boundaries are multiples of 4
     {
@@ -292,6 +303,92 @@ __device__ __forceinline__ void aev_forward_centre(const AevConst& c, const Grid
   for (; bcur < npb; ++bcur) {   // the last block and the empty ones behind it
     row[(e.btab[bcur].y & 255) * BLK + lane] = acc2.x + acc2.y;
     acc2 = make_float2(0.f, 0.f);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- a team of warps per centre
+// The single-kernel evaluation of small systems (small.cu, k_small_all) has two centres per CTA and sixteen warps: one
+// warp per centre leaves the rest idle while it walks through ~2000 dependent-latency-bound instructions (measured:
+// 7.3 us of a 37 us evaluation).  Here TW warps share one centre: the leader stages the environment and the block table;
+// the radial blocks and the chunks of 32 triplets are then dealt out over the team; every warp adds its chunks' sums
+// into accumulators of its own (team.acc[warp]), and the blocks are finished by adding the warps' accumulators in warp
+// order -- fixed orders throughout, so the row is bitwise reproducible (it differs from the one-warp row by rounding).
+template <int TW>
+struct alignas(16) FwdTeam {
+  float fac[TW][12][FWD_TP];         // phase-1 factors, one staging per warp (rows read with 128-bit loads)
+  float acc[TW][FWD_MAXB][32];       // per warp: sub-feature sums of the blocks its chunks touched
+};
+
+__device__ __forceinline__ void team_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// All TW warps of the team call this (tw = warp within the team, 0 = leader, which alone needs the rows and counts);
+// bar = a named barrier of the CTA that belongs to this team.
+template <int TW>
+__device__ __forceinline__ void aev_forward_team(const AevConst& c, const GridInfo* __restrict__ g,
+                                                 const GroupInfo* __restrict__ grp, const float4* __restrict__ spos,
+                                                 const uint32_t* __restrict__ rowR, const uint8_t* __restrict__ rowA, int nR,
+                                                 int nA, int ip, float* __restrict__ aev, int lane, int tw, int bar, FwdEnv& e,
+                                                 FwdTeam<TW>& tm) {
+  const float4 ci = spos[ip];
+  const int si = (__float_as_int(ci.w) >> 28) & 7;
+  const int Kc = grp->Kc;
+  float* __restrict__ row = aev + (size_t)(ip + grp->pad_shift[si]) * Kc;
+  const int np = grp->npres;
+  const int npb = np * (np + 1) / 2;
+  if (tw == 0) {
+    fwd_load_env(c, g, grp, spos, rowR, rowA, nR, nA, ci, lane, e);
+    fwd_block_table(c, grp, e, np, npb, lane);
+    // dense-K: the angular blocks of absent species pairs are zero (before the barrier: the blocks present are stored after it)
+    if (grp->nblk == c.nblk_full && np < c.S)
+      for (int b = c.nRB; b < c.nblk_full; ++b) row[grp->cpos[b] * BLK + lane] = 0.f;
+  }
+  team_bar(bar, TW * 32);
+  // ---- radial blocks: from the last warp downwards (the first warps have the most chunks)
+  {
+    int idx = 0;
+    for (int b = 0; b < c.nRB; ++b) {
+      const int cp = grp->cpos[b];
+      if (cp < 0) continue;
+      if (TW - 1 - (idx % TW) == tw) row[cp * BLK + lane] = fwd_radial_block(c, e, b, lane);
+      ++idx;
+    }
+  }
+  // ---- angular: chunk i of 32 triplets goes to warp i mod TW
+  for (int b = 0; b < npb; ++b) tm.acc[tw][b][lane] = 0.f;
+  const int Ttot = e.boff[npb];
+  const int fa = lane >> 3, fz = lane & 7;
+  const float* __restrict__ f2row = tm.fac[tw][fa];
+  const float* __restrict__ bzrow = tm.fac[tw][4 + fz];
+  int bp1 = 0, bcur = 0;
+  for (int c0 = FWD_TCH * tw; c0 < Ttot; c0 += FWD_TCH * TW) {
+    fwd_factors(c, e, tm.fac[tw], npb, c0, lane, bp1);
+    __syncwarp();
+    int q = c0;
+    const int qend = min(c0 + FWD_TCH, Ttot);
+    while (q < qend) {
+      while (e.boff[bcur + 1] <= q) ++bcur;
+      const int bend = min(e.boff[bcur + 1], qend);
+      const float4* fp = reinterpret_cast<const float4*>(f2row + (q - c0));
+      const float4* bp = reinterpret_cast<const float4*>(bzrow + (q - c0));
+      const int n4 = (bend - q) >> 2;
+      float2 acc2 = make_float2(0.f, 0.f);
+#pragma unroll 2
+      for (int i = 0; i < n4; ++i) {
+        const float4 f = fp[i], bz = bp[i];
+        acc2 = __ffma2_rn(make_float2(f.x, f.y), make_float2(bz.x, bz.y), acc2);
+        acc2 = __ffma2_rn(make_float2(f.z, f.w), make_float2(bz.z, bz.w), acc2);
+      }
+      tm.acc[tw][bcur][lane] += acc2.x + acc2.y;
+      q = bend;
+    }
+    __syncwarp();
+  }
+  team_bar(bar, TW * 32);
+  for (int b = tw; b < npb; b += TW) {
+    float v = 0.f;
+#pragma unroll
+    for (int w = 0; w < TW; ++w) v += tm.acc[w][b][lane];
+    row[(e.btab[b].y & 255) * BLK + lane] = v;
   }
 }
 

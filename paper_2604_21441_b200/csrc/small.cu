@@ -67,8 +67,11 @@ __device__ __forceinline__ void small_centres(const int* gs, int S, int n, int& 
 
 // K0-K3 of the block's centres (whole block; no early exit: the single-kernel evaluation goes on afterwards).  facc =
 // the accumulator array cleared here (sliced over the grid), or nullptr.
-template <int NW, bool ALIGNED>
-__device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<NW>& sm, unsigned long long* facc) {
+// TW > 1 (k_small_all): a team of TW warps per centre for the AEV row (aev_forward.cuh aev_forward_team): warp c < NW leads
+// centre c, warps NW + (TW - 1) c .. are its helpers; team = the teams' staging.
+template <int NW, bool ALIGNED, int TW = 1>
+__device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<NW>& sm, unsigned long long* facc,
+                                            FwdTeam<TW>* team = nullptr) {
   FwdEnv* env = sm.env;
   float4* sp = sm.sp;
   uint32_t (*rowR_s)[RCAP_MAX] = sm.rowR_s;
@@ -172,8 +175,12 @@ __device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<
   // ---- P3: neighbour rows of centre ip: all-pairs sweep, 32 candidates at a time (minimum image per pair)
   int ip_first, n_rows;
   small_centres<NW, ALIGNED>(gs, S, n, ip_first, n_rows);
-  const int ip = ip_first + w;
-  if (w < n_rows) {   // (k_small_all runs with more warps than centres: the others wait at the next barrier)
+  const int cidx = (TW == 1 || w < NW) ? w : (w - NW) / (TW > 1 ? TW - 1 : 1);   // centre this warp works for
+  const int tw = (TW == 1 || w < NW) ? 0 : 1 + (w - NW) % (TW > 1 ? TW - 1 : 1);
+  const int ip = ip_first + cidx;
+  if (TW > 1 && tw > 0) {
+    if (cidx < n_rows) aev_forward_team<TW>(a.c, &g_s, &grp_s, sp, nullptr, nullptr, 0, 0, ip, a.aev, lane, tw, 1 + cidx, env[cidx], team[cidx]);
+  } else if (w < n_rows) {   // (k_small_front: warp <-> centre; warps beyond the centres wait at the next barrier)
   const float4 pi = sp[ip];
   const int a_i = __float_as_int(pi.w) & 0x0fffffff;
   const int o_i = a.ml ? a.ml[a_i] : a_i;
@@ -218,7 +225,8 @@ __device__ __forceinline__ void small_front(const SmallArgs& a, SmallFrontSmemT<
   if (bad) atomicOr(a.flags, bad);
   __syncwarp();
   // ---- P4: this centre's AEV row, from the shared-memory copies of positions, rows, grid and groups
-  aev_forward_centre(a.c, &g_s, &grp_s, sp, rowR_s[w], rowA_s[w], nR, nA, ip, a.aev, lane, env[w]);
+  if (TW > 1) aev_forward_team<TW>(a.c, &g_s, &grp_s, sp, rowR_s[w], rowA_s[w], nR, nA, ip, a.aev, lane, 0, 1 + w, env[w], team[w]);
+  else aev_forward_centre(a.c, &g_s, &grp_s, sp, rowR_s[w], rowA_s[w], nR, nA, ip, a.aev, lane, env[w]);
   }
 }
 
@@ -247,6 +255,7 @@ constexpr int SA_R = 2;             // rows (centres) per CTA: the MLP phase is 
 constexpr int SA_KSPLIT = 2;        // thread groups of 256 sharing the k loop of the MLP phase
 static_assert(SA_R == 2 || SA_R % 4 == 0, "row vector loads");
 constexpr int SA_THREADS = 256 * SA_KSPLIT;
+constexpr int SA_TW = SA_THREADS / 32 / SA_R;   // warps per centre in the front end's AEV phase (a team: aev_forward.cuh)
 
 struct SmallAllArgs {
   SmallArgs f;
@@ -440,7 +449,8 @@ __global__ void __launch_bounds__(SA_THREADS, 1) k_small_all(const __grid_consta
   // after every CTA's ticket -- i.e. after all of this)
   if (a.zero_forces)
     for (int k = blockIdx.x * blockDim.x + tid; k < 3 * a.f.n_atoms; k += gridDim.x * blockDim.x) a.forces[k] = 0.f;
-  small_front<SA_R, true>(a.f, sm, nullptr);
+  // (the teams' staging shares the MLP staging: the front end is over before the MLP phase starts)
+  small_front<SA_R, true, SA_TW>(a.f, sm, nullptr, reinterpret_cast<FwdTeam<SA_TW>*>(mb));
   __syncthreads();
   int ip_first, n_rows;
   small_centres<SA_R, true>(sm.gs, a.f.c.S, n, ip_first, n_rows);
@@ -490,7 +500,7 @@ __global__ void __launch_bounds__(SA_THREADS, 1) k_small_all(const __grid_consta
 size_t small_all_smem(const nnp_model* m) {
   const size_t front = (sizeof(SmallFrontSmemT<SA_R>) + 15) & ~(size_t)15;
   const size_t mlp = ((size_t)m->Kfull * SA_R + 6 * (size_t)HP * SA_R + (SA_THREADS / 32) * SA_R + (size_t)8 * 256 * SA_R) * sizeof(float);
-  return front + std::max(mlp, sizeof(SmallBwdSmem));
+  return front + std::max(std::max(mlp, sizeof(SmallBwdSmem)), SA_R * sizeof(FwdTeam<SA_TW>));
 }
 
 // the single-kernel evaluation takes what the front end takes, with the tensor-core-shaped networks (four layers,
