@@ -361,4 +361,179 @@ __device__ __forceinline__ void fill_pairoff(const AevConst& c, const GroupInfo*
   }
 }
 
+// ---------------------------------------------------------------------------------------------- a team of warps per centre
+// k_small_all (small.cu) has sixteen warps for two centres; one warp per centre walks the pair rounds and the radial
+// passes one after the other (measured 5.6 us of a 33 us evaluation).  Here TW warps share the centre: the leader stages
+// the environment; the iterations of the pair rounds (two rounds each) are dealt out over the warps from warp 0 upwards,
+// the radial passes (32 neighbours each) over the warps from the last one downwards; every warp keeps the angular shares it
+// produced in an array of its own (PaccW[warp]); after a team barrier the radial warps add the shares of their neighbours
+// in warp order and scatter.  Orders are fixed (and the scatter is integer): bitwise reproducible; the result differs
+// from the one-warp version by rounding (another summation order of the angular shares).
+template <int TW>
+struct BwdTeam {
+  float PaccW[TW][ACAP_MAX][3];
+};
+
+template <int TW>
+__device__ __forceinline__ void aev_backward_team(const AevConst& c, const GridInfo* __restrict__ g,
+                                                  const GroupInfo* __restrict__ grp, const float4* __restrict__ spos,
+                                                  const uint32_t* __restrict__ rowR, const uint8_t* __restrict__ rowA, int nR,
+                                                  int nA, int ip, const float4* gb, int gs,
+                                                  unsigned long long* __restrict__ facc, int lane, int tw, int bar, BwdEnv& e,
+                                                  BwdTeam<TW>& tm, const int* pairoff) {
+  if (tw == 0) {
+    const float4 ci = spos[ip];
+    bwd_load_env(c, g, spos, rowR, rowA, nR, nA, ci, lane, e);
+  }
+  float (*Pacc)[3] = tm.PaccW[tw];
+  for (int j = lane; j < nA; j += 32) { Pacc[j][0] = 0.f; Pacc[j][1] = 0.f; Pacc[j][2] = 0.f; }
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(TW * 32) : "memory");
+
+  // ---- angular shares of this warp's iterations -> PaccW[tw]  (nA <= ACAP_MAX = 32: lanes hold the neighbours)
+  {
+    const int n = nA;
+    const float zm1 = c.zeta - 1.0f;
+    int it = 0;   // running iteration number over the passes: iteration i belongs to warp i mod TW
+    auto rr_pass = [&](int base, int ns) {
+      const int W = (ns <= 8) ? 8 : 16;
+      const int NG = 32 / W, grp_id = lane / W, jl = lane & (W - 1);
+      const bool act = jl < ns;
+      const int nrounds = ns >> 1;
+      float px = 0.f, py = 0.f, pz = 0.f;
+      float4 uj = make_float4(0.f, 0.f, 1.f, 1.f);
+      float fj = 0.f, dfj = 0.f;
+      int sj = 0;
+      if (act) { uj = e.ua[base + jl]; fj = e.fA[base + jl]; dfj = e.dfA[base + jl]; sj = e.slotA[base + jl]; }
+      bool any = false;
+      for (int m0 = 1; m0 <= nrounds; m0 += NG, ++it) {
+        if (it % TW != tw) continue;
+        any = true;
+        const int m = m0 + grp_id;
+        const bool last_half = ((ns & 1) == 0) && (m == nrounds);   // even ns: the round m = ns/2 holds each pair twice
+        const bool on = act && m <= nrounds && (!last_half || jl < nrounds);
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        if (on) {
+          int k = jl + m;
+          if (k >= ns) k -= ns;
+          k += base;
+          const PairShares o = pair_shares(c, zm1, gb + pairoff[sj * MAX_S + e.slotA[k]] * gs, gs, uj, fj, dfj, e.ua[k], e.fA[k],
+                                           e.dfA[k]);
+          px += o.jx; py += o.jy; pz += o.jz;
+          qx = o.kx; qy = o.ky; qz = o.kz;
+        }
+        int src = jl - m;
+        if (src < 0) src += ns;
+        const int srcl = (grp_id * W + src) & 31;
+        const float rx = __shfl_sync(0xffffffffu, qx, srcl);
+        const float ry = __shfl_sync(0xffffffffu, qy, srcl);
+        const float rz = __shfl_sync(0xffffffffu, qz, srcl);
+        if (act && m <= nrounds && (!last_half || jl >= nrounds)) { px += rx; py += ry; pz += rz; }
+      }
+      if (any) {   // (warp-uniform)
+        for (int o = W; o < 32; o <<= 1) {
+          px += __shfl_xor_sync(0xffffffffu, px, o);
+          py += __shfl_xor_sync(0xffffffffu, py, o);
+          pz += __shfl_xor_sync(0xffffffffu, pz, o);
+        }
+        if (act && grp_id == 0) { Pacc[base + jl][0] += px; Pacc[base + jl][1] += py; Pacc[base + jl][2] += pz; }
+        __syncwarp();
+      }
+    };
+    if (n <= 16) {
+      rr_pass(0, n);
+    } else {
+      rr_pass(0, 16);
+      rr_pass(16, n - 16);
+      // cross pairs A x B
+      const int g2 = lane >> 4, jl = lane & 15, nb = n - 16;
+      const float4 uj = e.ua[jl];
+      const float fj = e.fA[jl], dfj = e.dfA[jl];
+      const int sj = e.slotA[jl];
+      float px = 0.f, py = 0.f, pz = 0.f;
+      bool any = false;
+      for (int r0 = 0; r0 < nb; r0 += 2, ++it) {
+        if (it % TW != tw) continue;
+        any = true;
+        const int r = r0 + g2, k = 16 + r;
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        if (r < nb) {
+          const PairShares o = pair_shares(c, zm1, gb + pairoff[sj * MAX_S + e.slotA[k]] * gs, gs, uj, fj, dfj, e.ua[k], e.fA[k],
+                                           e.dfA[k]);
+          px += o.jx; py += o.jy; pz += o.jz;
+          qx = o.kx; qy = o.ky; qz = o.kz;
+        }
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) {   // k's share: sum over the 16 lanes of the group
+          qx += __shfl_xor_sync(0xffffffffu, qx, o);
+          qy += __shfl_xor_sync(0xffffffffu, qy, o);
+          qz += __shfl_xor_sync(0xffffffffu, qz, o);
+        }
+        if (jl == 0 && r < nb) { Pacc[k][0] += qx; Pacc[k][1] += qy; Pacc[k][2] += qz; }
+      }
+      if (any) {
+        px += __shfl_xor_sync(0xffffffffu, px, 16);
+        py += __shfl_xor_sync(0xffffffffu, py, 16);
+        pz += __shfl_xor_sync(0xffffffffu, pz, 16);
+        __syncwarp();
+        if (g2 == 0) { Pacc[jl][0] += px; Pacc[jl][1] += py; Pacc[jl][2] += pz; }
+      }
+    }
+  }
+
+  // ---- radial coefficients of this warp's pass (lane <-> radial neighbour), before the barrier: they need no shares
+  const int q = 32 * (TW - 1 - tw) + lane;
+  const bool mine = q < nR;
+  float px = 0.f, py = 0.f, pz = 0.f;
+  if (mine) {
+    const float4 uq = e.u[q];
+    const int s = e.slotR[q];
+    const float4* gr = gb + (size_t)(grp->cpos[s >> 1] * (BLK / 4) + (s & 1) * 4) * gs;
+    float fc, dfc;
+    cutoff(fminf(uq.w, c.Rcr), c.inv_Rcr, fc, dfc);
+    const float f = c.cR * fc, df = c.cR * dfc;
+    const float2 R2 = make_float2(uq.w, uq.w), hf2 = make_float2(-2.0f * c.etaR * f, -2.0f * c.etaR * f), df2 = make_float2(df, df);
+    float2 coef2 = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      const float4 gv = gr[v * gs];
+#pragma unroll
+      for (int t = 0; t < 4; t += 2) {
+        const float2 x = __fadd2_rn(R2, make_float2(-c.ShfR[4 * v + t], -c.ShfR[4 * v + t + 1]));
+        const float2 y = __fmul2_rn(x, x);
+        const float2 ex = make_float2(ex2f(-c.etaR_l2e * y.x), ex2f(-c.etaR_l2e * y.y));
+        const float2 gg = (t == 0) ? make_float2(gv.x, gv.y) : make_float2(gv.z, gv.w);
+        coef2 = __ffma2_rn(__fmul2_rn(gg, ex), __ffma2_rn(x, hf2, df2), coef2);
+      }
+    }
+    const float coef = coef2.x + coef2.y;
+    px = coef * uq.x; py = coef * uq.y; pz = coef * uq.z;
+  }
+  asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(TW * 32) : "memory");
+  if (32 * (TW - 1 - tw) >= nR) return;   // (warp-uniform: no radial pass for this warp)
+
+  // ---- assembly: angular shares in warp order, fixed point, scatter
+  long long ox = 0, oy = 0, oz = 0;
+  if (mine) {
+    const int ia = e.ainv[q];
+    if (ia != 255) {
+      float ax = 0.f, ay = 0.f, az = 0.f;
+#pragma unroll
+      for (int w = 0; w < TW; ++w) { ax += tm.PaccW[w][ia][0]; ay += tm.PaccW[w][ia][1]; az += tm.PaccW[w][ia][2]; }
+      px += ax; py += ay; pz += az;
+    }
+    const long long fx = to_fix(px), fy = to_fix(py), fz = to_fix(pz);
+    ox = fx; oy = fy; oz = fz;
+    const int jp = (int)(rowR[q] & JMASK);
+    atomicAdd(&facc[3 * (size_t)jp + 0], (unsigned long long)(-fx));
+    atomicAdd(&facc[3 * (size_t)jp + 1], (unsigned long long)(-fy));
+    atomicAdd(&facc[3 * (size_t)jp + 2], (unsigned long long)(-fz));
+  }
+  for (int o = 16; o > 0; o >>= 1) { ox += shfl_xor_ll(ox, o); oy += shfl_xor_ll(oy, o); oz += shfl_xor_ll(oz, o); }
+  if (lane == 0) {
+    atomicAdd(&facc[3 * (size_t)ip + 0], (unsigned long long)ox);
+    atomicAdd(&facc[3 * (size_t)ip + 1], (unsigned long long)oy);
+    atomicAdd(&facc[3 * (size_t)ip + 2], (unsigned long long)oz);
+  }
+}
+
 }  // namespace nnp

@@ -433,7 +433,7 @@ __device__ __forceinline__ void small_mlp(const SmallAllArgs& a, const GroupInfo
 
 struct SmallBwdSmem {
   BwdEnv env[SA_R];
-  float Pacc[SA_R][ACAP_MAX][3];
+  BwdTeam<SA_TW> team[SA_R];
   int pairoff[MAX_S * MAX_S];
 };
 
@@ -459,14 +459,17 @@ __global__ void __launch_bounds__(SA_THREADS, 1) k_small_all(const __grid_consta
   SmallBwdSmem& sb = *reinterpret_cast<SmallBwdSmem*>(mb);
   fill_pairoff(a.f.c, &sm.grp_s, sb.pairoff);
   __syncthreads();
-  const int ip = ip_first + w;
-  if (w < n_rows) {
+  // a team of SA_TW warps per centre, as in the front end: warp c < SA_R leads centre c
+  const int cidx = (w < SA_R) ? w : (w - SA_R) / (SA_TW - 1), tw = (w < SA_R) ? 0 : 1 + (w - SA_R) % (SA_TW - 1);
+  const int ip = ip_first + cidx;
+  if (cidx < n_rows) {
     const int si = (__float_as_int(sm.sp[ip].w) >> 28) & 7;
     const int Kc = sm.grp_s.Kc;
     const float4* gb = reinterpret_cast<const float4*>(a.daev + daev_off((size_t)(ip + sm.grp_s.pad_shift[si]), 0, Kc));
-    // (rows from global memory: the front end's shared copies hold them too, but only until the next centre of a warp)
-    aev_backward_centre<false>(a.f.c, &sm.g_s, &sm.grp_s, sm.sp, a.f.nbrR + (size_t)ip * a.f.rcap, a.f.nbrA + (size_t)ip * a.f.acap,
-                               a.f.cntR[ip], a.f.cntA[ip], ip, gb, TILE_M, a.acc, nullptr, lane, sb.env[w], sb.Pacc[w], sb.pairoff);
+    // (rows from global memory: the MLP staging has taken the place of the front end's shared copies)
+    aev_backward_team<SA_TW>(a.f.c, &sm.g_s, &sm.grp_s, sm.sp, a.f.nbrR + (size_t)ip * a.f.rcap, a.f.nbrA + (size_t)ip * a.f.acap,
+                             a.f.cntR[ip], a.f.cntA[ip], ip, gb, TILE_M, a.acc, lane, tw, 1 + cidx, sb.env[cidx], sb.team[cidx],
+                             sb.pairoff);
   }
   // ---- output by the last CTA to get here
   __threadfence();
