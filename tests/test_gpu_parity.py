@@ -616,6 +616,39 @@ def test_small_path_and_general_path(k, layout):
     check_EF(E3, F3, ref2, n_ml, rows=ml)
 
 
+@pytest.mark.parametrize("n_sub", [1, 2, 3, 5, 17, 33, 100, 255, 256])
+def test_small_path_subset_sizes(n_sub):
+    """The one-kernel path deals a centre's triplet chunks, pair rounds and radial passes over a team of eight warps and the
+    species groups over CTAs in chunks of two: ML subsets of odd sizes (one atom, groups of one, the 256-atom limit), half of
+    them a compact ball (full rows, up to ~20 angular neighbours) and half scattered atoms (empty and one-entry rows), must
+    give the oracle's rows, E and F, and what the general path gives."""
+    cfg = gen.get_config(4)
+    n = cfg["pos"].shape[0]
+    rng = np.random.default_rng(1000 + n_sub)
+    L = np.array([cfg["box"][0], cfg["box"][4], cfg["box"][8]], dtype=np.float64)
+    if n_sub % 2:   # the n_sub atoms nearest to a random atom (minimum image)
+        d = cfg["pos64"] - cfg["pos64"][rng.integers(n)]
+        d -= L * np.rint(d / L)
+        ml = np.sort(np.argsort((d * d).sum(1), kind="stable")[:n_sub]).astype(np.int32)
+    else:
+        ml = np.sort(rng.choice(n, size=n_sub, replace=False)).astype(np.int32)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    m, ws = make(cfg, max_atoms=n)
+    out = {}
+    for on in (2, 0):
+        ws.set_small_path(on)
+        E, F = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+        if on == 2:
+            assert ws.launches() == 1
+        check_lists(ws, cfg, cfg["pos"], n_sub, ml)
+        check_EF(E, F, ref, n_sub, rows=ml)
+        E2, F2 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+        assert E2 == E and np.array_equal(F2, F)
+        out[on] = (E, F)
+    assert abs(out[2][0] - out[0][0]) / n_sub < 1e-6 and np.abs(out[2][1] - out[0][1]).max() < 1e-4
+
+
 # ------------------------------------------------------------------ triclinic boxes (SURVEY.md section 8.f item 4, reading #35)
 @pytest.mark.parametrize("shear", [(0.3, -0.2, 0.4), (-0.5, 0.5, -0.5), (0.0, 0.0, 0.25)])
 def test_triclinic_box(shear):
