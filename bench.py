@@ -296,15 +296,17 @@ def run_ours(args, rank, world, local_rank):
     hpos = [torch.from_numpy(P[t]).pin_memory() for t in range(N_POS_SETS)]
     hZ = torch.from_numpy(cfg["Z"]).pin_memory()
     hF = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    npos, nZ, nF = [h.numpy() for h in hpos], hZ.numpy(), hF.numpy()   # numpy views of the pinned buffers
+    nbox = np.ascontiguousarray(box, dtype=np.float32)
     for t in range(3):
-        ws.eval_host(hpos[t].numpy(), hZ.numpy(), box, 1, None, hF.numpy())
+        ws.eval_host(npos[t], nZ, nbox, 1, None, nF)
     e2e_s = 0.0
     barrier()
     for k in range(args.steps):
         flush.zero_()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        ws.eval_host(hpos[k % N_POS_SETS].numpy(), hZ.numpy(), box, 1, None, hF.numpy())
+        ws.eval_host(npos[k % N_POS_SETS], nZ, nbox, 1, None, nF)
         e2e_s += time.perf_counter() - t0
     barrier()
 

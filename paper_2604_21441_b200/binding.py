@@ -283,6 +283,13 @@ class Model:
         self.close()
 
 
+def _as(a, dtype):
+    """`a` itself when it already is a C-contiguous array of `dtype` (no new object: see Workspace._ptr), else a converted copy."""
+    if type(a) is np.ndarray and a.dtype == dtype and a.flags.c_contiguous:
+        return a
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
 class Workspace:
     def __init__(self, model, max_atoms, max_ml_atoms=None, stream=None):
         import torch
@@ -293,6 +300,9 @@ class Workspace:
         rc, h = nnp_workspace_create(model.handle, self.max_atoms, self.max_ml, self.stream.cuda_stream)
         _check(rc, "nnp_workspace_create")
         self.handle = h
+        self._pcache = {}                              # id(array) -> (array, address): see _ptr
+        self._E = np.zeros(1, dtype=np.float64)        # energy word of eval_host
+        self._E_ptr = self._E.ctypes.data
 
     def set_mlp_mode(self, mode):
         _check(nnp_workspace_set_mlp_mode(self.handle, mode), "nnp_workspace_set_mlp_mode")
@@ -366,20 +376,32 @@ class Workspace:
 
     def eval_host(self, pos, Z, box, pbc=1, ml_index=None, forces_out=None):
         """numpy in / numpy out through nnp_eval_host (copies + synchronisation inside the library)."""
-        pos = np.ascontiguousarray(pos, dtype=np.float32)
-        Z = np.ascontiguousarray(Z, dtype=np.int32)
-        b = np.ascontiguousarray(box, dtype=np.float32).reshape(9)
+        pos = _as(pos, np.float32)
+        Z = _as(Z, np.int32)
+        b = _as(box, np.float32)
         n = pos.shape[0]
-        ml = None if ml_index is None else np.ascontiguousarray(ml_index, dtype=np.int32)
-        E = np.zeros(1, dtype=np.float64)
+        ml = None if ml_index is None else _as(ml_index, np.int32)
         F = np.empty((n, 3), dtype=np.float32) if forces_out is None else forces_out
-        rc = nnp_eval_host(self.handle, n, pos.ctypes.data, Z.ctypes.data, b.ctypes.data, pbc,
-                           None if ml is None else ml.ctypes.data, 0 if ml is None else len(ml), E.ctypes.data,
-                           F.ctypes.data)
+        rc = nnp_eval_host(self.handle, n, self._ptr(pos), self._ptr(Z), self._ptr(b), pbc,
+                           None if ml is None else self._ptr(ml), 0 if ml is None else len(ml), self._E_ptr,
+                           self._ptr(F))
         _check(rc, "nnp_eval_host")
         self._last = None
         self._n_ml = n if ml is None else len(ml)
-        return float(E[0]), F
+        return float(self._E[0]), F
+
+    def _ptr(self, a):
+        """Address of a numpy array's buffer.  `a.ctypes.data` costs ~2.5 us a call -- five of them were 12 us of a 290 us
+        step -- so the address of an array OBJECT seen before is remembered (the entry holds a reference: the id cannot be
+        reused, and numpy refuses to reallocate a referenced array's buffer); at most 64 entries."""
+        ent = self._pcache.get(id(a))
+        if ent is not None and ent[0] is a:
+            return ent[1]
+        p = a.ctypes.data
+        if len(self._pcache) >= 64:
+            self._pcache.clear()
+        self._pcache[id(a)] = (a, p)
+        return p
 
     def status(self):
         return nnp_status(self.handle)
