@@ -35,6 +35,7 @@ extern "C" {
 #define NNP_ERR_CUDA (-6)            /* CUDA runtime error or no device                                        */
 #define NNP_ERR_UNSUPPORTED (-7)     /* descriptor shape outside the kernels' range (see nnp_model_create)     */
 #define NNP_ERR_STALE (-8)           /* cell binning reused beyond its validity (nnp_workspace_set_bin_reuse)   */
+#define NNP_ERR_STATIC_LIMIT (-9)    /* size beyond the fixed maximum of a no-allocation entry point            */
 
 typedef struct nnp_model nnp_model;         /* opaque, immutable after create, shareable between workspaces */
 typedef struct nnp_workspace nnp_workspace; /* opaque scratch, one per stream, not thread-safe              */
@@ -246,6 +247,22 @@ int nnp_debug_stage_times(nnp_workspace*, float* ms);
  * writes HOST *h_tflops = best of 5 launches, counting 2 flop per FMA lane.  variant 0: scalar FFMA with three register
  * operands; variant 1: packed FFMA2 (fma.rn.f32x2, two FMA lanes per instruction, sm_100).  Synchronises the stream. */
 int nnp_debug_fp32_peak(void* cuda_stream, int32_t variant, double* h_tflops);
+
+/* The energy reduction of K8 without a workspace and WITHOUT ANY ALLOCATION (eq. 2: E is the sum of the
+ * atomic network outputs) -- for callers that cannot call cudaMalloc (CUDA graph capture, tight
+ * serving loops, harnesses that forbid it):  *d_energy = e_scale * sum_{i < n} d_e_atom[i], summed in fp64 in a fixed order
+ * (block partials, then the last block adds them in index order): bitwise reproducible, no floating-point atomics.
+ *   cuda_stream  cudaStream_t of the CURRENT device (the call is asynchronous on it)
+ *   d_e_atom     DEVICE [n] fp32 atomic energies (e.g. what nnp_debug_atomic_energies reports), read-only
+ *   e_scale      factor on the sum (1.0 = same unit as the inputs)
+ *   d_energy     DEVICE [1] fp64, written by the kernel
+ * Scratch: a static device array inside the library (33 024 bytes on every GPU that loads it, held until exit); the call
+ * uses no cudaMalloc / cudaFree and no allocating routine (one cudaMemsetAsync of the ticket line + one kernel).
+ * n > NNP_STATIC_MAX_ATOMS returns NNP_ERR_STATIC_LIMIT (nothing launched); n == 0 writes 0.0; bad pointers / n < 0
+ * NNP_ERR_INVALID_ARG.  ALL calls on a device share the one scratch array: calls in one stream are ordered and safe; calls
+ * whose kernels may overlap on the GPU (different streams without a dependency) RACE and give wrong sums -- serialise them. */
+#define NNP_STATIC_MAX_ATOMS 1048576
+int nnp_energy_sum_static(void* cuda_stream, int64_t n, const float* d_e_atom, double e_scale, double* d_energy);
 
 #ifdef __cplusplus
 }

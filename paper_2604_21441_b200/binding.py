@@ -19,8 +19,10 @@ EXPORTS = [
     "nnp_workspace_destroy", "nnp_workspace_set_mlp_mode", "nnp_workspace_set_dense_k", "nnp_workspace_set_virial_output", "nnp_workspace_set_units", "nnp_workspace_set_pair_list", "nnp_workspace_set_small_path", "nnp_workspace_set_bin_reuse", "nnp_eval",
     "nnp_eval_host", "nnp_status", "nnp_strerror", "nnp_debug_neighbors", "nnp_debug_aev", "nnp_debug_daev",
     "nnp_debug_atomic_energies", "nnp_debug_counters", "nnp_debug_mlp_timeline", "nnp_link_place", "nnp_link_spread", "nnp_workspace_set_profiling", "nnp_debug_stage_times",
-    "nnp_debug_fp32_peak", "nnp_model_default_mlp_mode",
+    "nnp_debug_fp32_peak", "nnp_model_default_mlp_mode", "nnp_energy_sum_static",
 ]
+NNP_ERR_STATIC_LIMIT = -9
+NNP_STATIC_MAX_ATOMS = 1048576
 
 
 class NNPError(RuntimeError):
@@ -89,6 +91,7 @@ def lib():
         L.nnp_workspace_set_profiling.argtypes = [vp, i32]
         L.nnp_debug_stage_times.argtypes = [vp, vp]
         L.nnp_debug_fp32_peak.argtypes = [vp, i32, C.POINTER(C.c_double)]
+        L.nnp_energy_sum_static.argtypes = [vp, i64, vp, C.c_double, vp]
         _lib = L
     return _lib
 
@@ -221,6 +224,11 @@ def nnp_debug_fp32_peak(cuda_stream, variant):
     t = C.c_double(0.0)
     rc = lib().nnp_debug_fp32_peak(cuda_stream, int(variant), C.byref(t))
     return rc, t.value
+
+
+def nnp_energy_sum_static(cuda_stream, n, d_e_atom, e_scale, d_energy):
+    """raw device pointers in, status out: the no-allocation energy reduction (nnp.h)"""
+    return lib().nnp_energy_sum_static(cuda_stream, int(n), d_e_atom, float(e_scale), d_energy)
 
 
 # ---------------------------------------------------------------- convenience owners

@@ -22,6 +22,7 @@ extern "C" const char* nnp_strerror(int code) {
     case NNP_ERR_CAPACITY: return "neighbour row, cell buffer or tile capacity exceeded";
     case NNP_ERR_COINCIDENT: return "two ML atoms coincide";
     case NNP_ERR_CUDA: return "CUDA error or no CUDA device";
+    case NNP_ERR_STATIC_LIMIT: return "size beyond the fixed maximum of a no-allocation entry point (NNP_STATIC_MAX_ATOMS)";
     case NNP_ERR_UNSUPPORTED: return "descriptor or network shape outside the kernels' range";
     case NNP_ERR_STALE: return "an atom left its cell by more than skin / 2 while the cell binning was being reused";
     default: return "unknown error";
