@@ -18,8 +18,10 @@ k_aev_forward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __res
               const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
               float* __restrict__ aev) {
   __shared__ FwdEnv env[AEV_FWD_WARPS];
+  TL_SCOPE(0);
   pdl_trigger();
   pdl_wait();
+  TL_WAITED(0);
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int ip = blockIdx.x * AEV_FWD_WARPS + w;
   if (ip >= n_ml) return;
@@ -37,3 +39,5 @@ int launch_aev_forward(nnp_workspace* ws, int64_t n_ml) {
 }
 
 }  // namespace nnp
+
+TL_EXPORT(nnp_debug_step_timeline_aev)

@@ -27,6 +27,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   __shared__ int timed_out;
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
   __shared__ int pairoff[MAX_S * MAX_S];   // (s1, s2) -> first float4 piece of the pair's dE/dAEV block
+  TL_SCOPE(0);
   pdl_trigger();
   if (!tile_done) pdl_wait();   // with per-tile flags the MLP kernel is NOT awaited as a whole (see below)
   if (threadIdx.x == 0) timed_out = 0;
@@ -58,6 +59,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
     }
   }
   __syncthreads();
+  TL_WAITED(0);   // (here: the block's tile flags are up)
   if (timed_out) return;
   const int ip = blockIdx.x * AEV_WARPS + w;
   if (ip >= n_ml) return;
@@ -85,8 +87,10 @@ k_force_out(const float4* __restrict__ spos, const unsigned long long* __restric
   __shared__ double wsum[8];
   __shared__ long long vsum[8][9];
   __shared__ bool last;
+  TL_SCOPE(1);
   pdl_trigger();
   pdl_wait();
+  TL_WAITED(1);
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
   double e = 0.0;
@@ -168,3 +172,5 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
 }
 
 }  // namespace nnp
+
+TL_EXPORT(nnp_debug_step_timeline_force)

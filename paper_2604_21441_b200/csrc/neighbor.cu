@@ -346,6 +346,7 @@ struct BinArgs {
 };
 
 __global__ void __launch_bounds__(BIN_THREADS) k_bin_cells(const __grid_constant__ BinArgs a) {
+  TL_SCOPE(0);
   __shared__ int spres;
   pdl_trigger();
   const GridInfo* g = &a.hg;
@@ -383,8 +384,10 @@ __global__ void __launch_bounds__(256) k_cell_sort(const __grid_constant__ SortA
   __shared__ int cnt8[8][MAX_S], bst8[8][MAX_S];
   __shared__ int gs[MAX_S + 1], pre_s[MAX_S], pshift[MAX_S], tb[MAX_S + 1];
   __shared__ GroupInfo grp_s;
+  TL_SCOPE(1);
   pdl_trigger();
   pdl_wait();
+  TL_WAITED(1);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int S = a.S, ncell = a.ncell;
   const int c0 = blockIdx.x * 8, cell = c0 + warp;
@@ -536,8 +539,10 @@ __global__ void __launch_bounds__(256, 4) k_neighbors(AevConst c, const GridInfo
   __shared__ int cenStart[MAX_S], cenOff[MAX_S + 1];
   __shared__ int wsum[8];
   __shared__ unsigned short surv[8][SURV_CAP];
+  TL_SCOPE(2);
   pdl_trigger();
   pdl_wait();
+  TL_WAITED(2);
   const int cell = blockIdx.x, ncell = g->ncell;
   if (cell >= ncell) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1132,3 +1137,5 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
 }
 
 }  // namespace nnp
+
+TL_EXPORT(nnp_debug_step_timeline_neighbor)

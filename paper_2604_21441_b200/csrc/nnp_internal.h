@@ -208,6 +208,38 @@ namespace nnp {
 // scheduling of kernel n+1 overlap the tail of kernel n.  k_aev_backward alone does not wait for the whole MLP
 // kernel but per tile (force.cu).  Stage profiling (events between the kernels) switches the attribute off.
 #ifdef __CUDACC__
+// Step timeline: where the kernels of ONE evaluation sit in time when they run as the PDL chain (ncu serialises them, stage
+// profiling too).  Profiling scaffolding, compiled in only with -DNNP_STEP_TIMELINE (NNP_EXTRA_NVCC_FLAGS of build.py; read by
+// `python -m paper_2604_21441_b200.step_timeline`): thread 0 of every block records %globaltimer into the slot of its kernel --
+// {first block in, first block past griddepcontrol.wait, last block out, last block in, mark: first, mark: last}.  One array per
+// translation unit (no relocatable device code), each with an export of its own.  The product build carries none of this.
+#ifdef NNP_STEP_TIMELINE
+static __device__ unsigned long long g_step_tl[4][6];
+__device__ __forceinline__ unsigned long long tl_now() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+struct TlScope {
+  int k;
+  __device__ __forceinline__ explicit TlScope(int k_) : k(k_) {
+    if (threadIdx.x == 0) { const unsigned long long t = tl_now(); atomicMin(&g_step_tl[k][0], t); atomicMax(&g_step_tl[k][3], t); }
+  }
+  __device__ __forceinline__ ~TlScope() { if (threadIdx.x == 0) atomicMax(&g_step_tl[k][2], tl_now()); }
+};
+#define TL_SCOPE(k) TlScope tl_scope_(k)
+#define TL_WAITED(k) do { if (threadIdx.x == 0) atomicMin(&g_step_tl[k][1], tl_now()); } while (0)
+#define TL_MARK(k) do { if (threadIdx.x == 0) { const unsigned long long t_ = tl_now(); atomicMin(&g_step_tl[k][4], t_); atomicMax(&g_step_tl[k][5], t_); } } while (0)
+// host: copy the unit's slots out (h[24]) and re-arm them (minima to ~0, maxima to 0)
+#define TL_EXPORT(name)                                                                                            \
+  extern "C" int name(unsigned long long* h) {                                                                     \
+    if (cudaMemcpyFromSymbol(h, nnp::g_step_tl, sizeof(nnp::g_step_tl)) != cudaSuccess) return NNP_ERR_CUDA;                  \
+    unsigned long long z[4][6];                                                                                    \
+    for (int k = 0; k < 4; ++k) { z[k][0] = z[k][1] = z[k][4] = ~0ull; z[k][2] = z[k][3] = z[k][5] = 0ull; }        \
+    return cudaMemcpyToSymbol(nnp::g_step_tl, z, sizeof(z)) == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;                      \
+  }
+#else
+#define TL_SCOPE(k) do { } while (0)
+#define TL_WAITED(k) do { } while (0)
+#define TL_MARK(k) do { } while (0)
+#define TL_EXPORT(name)
+#endif
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 template <class... KArgs, class... Args>
