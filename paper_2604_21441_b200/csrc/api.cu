@@ -219,6 +219,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
     ws->prep_cluster = prep_cluster_size();
     ws->small_path = 1;
     ws->small_all = 1;
+    ws->pack_done = 0;
     ws->prep_cluster_max = 8192;   // measured: 24 000 atoms run 4 us slower in one cluster than on the cooperative grid
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;

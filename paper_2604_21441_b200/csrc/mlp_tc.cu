@@ -925,22 +925,40 @@ static void ensemble_guard_after(cudaStream_t st) {
   if (cudaEventRecord(g_ens_event, st) == cudaSuccess) g_ens_recorded = true; else cudaGetLastError();
 }
 
+// k_tc_pack_w1 needs the groups of this evaluation (k_cell_sort / k_prep / k_small_front) and must be through before the MLP
+// kernel starts.  Directly in front of the MLP kernel it sits on the critical path (step timeline: the AEV kernel ends, the
+// pack kernel's wait returns 1.1 us later, it runs 1 us, and only then do the MLP CTAs come in: 2.6 us); the cell-list path
+// therefore launches it right after k_cell_sort, where it is a 1 us link in front of k_neighbors instead and its L2
+// prefetch has the whole neighbour + AEV stage to land.  Returns the number of launches (0: no tensor-core MLP this time).
+int launch_tc_pack(nnp_workspace* ws) {
+  const nnp_model* m = ws->model;
+  TcModel* tm = static_cast<TcModel*>(m->tc);
+  TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
+  if (!tm || !tw || ws->mlp_mode == NNP_MLP_FP32_SIMT) return 0;
+  TcPackAll pall;
+  for (int mem = 0; mem < MAX_MEMBERS; ++mem)
+    for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
+  const bool pdl = !ws->profiling;
+  launch_pdl(pdl, ws->stream, k_tc_pack_w1, dim3(32, m->aev.S, m->n_members), dim3(256), 0, tm->d_nets, ws->groups, pall,
+             tm->d_tabs, pdl ? m->Kfull : 0, tw->key, tw->done, ws->max_tiles);
+  ws->pack_done = 1;
+  return 1;
+}
+
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
-  if (n_ml <= 0) return 0;
+  if (n_ml <= 0) { ws->pack_done = 0; return 0; }
   const nnp_model* m = ws->model;
   TcModel* tm = static_cast<TcModel*>(m->tc);
   TcWorkspace* tw = static_cast<TcWorkspace*>(ws->tc_ws);
   if (!tm || !tw) return launch_mlp_simt(ws, n_ml);
   ws->tile_done = tw->done; ws->tile_done_target = m->n_members;
-  TcPackAll pall;
-  for (int mem = 0; mem < MAX_MEMBERS; ++mem)
-    for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
+  int nl = 0;
+  if (!ws->pack_done) nl += launch_tc_pack(ws);
+  ws->pack_done = 0;
   const bool ens = m->n_members > 1;
   if (ens) ensemble_guard_before(ws->stream);
   // (a wait on another stream's event in front of the launch: no programmatic overlap with the predecessor then)
   const bool pdl = !ws->profiling;
-  launch_pdl(pdl, ws->stream, k_tc_pack_w1, dim3(32, m->aev.S, m->n_members), dim3(256), 0, tm->d_nets, ws->groups, pall,
-             tm->d_tabs, pdl ? m->Kfull : 0, tw->key, tw->done, ws->max_tiles);
   // one persistent CTA per SM over the (member, tile) work items (all CTAs are co-resident: 1 CTA/SM by shared memory)
   const int grid = (int)std::min<int64_t>((int64_t)ws->max_tiles * m->n_members, tw->num_sms);
   const float escale = 1.0f / (float)m->n_members;   // E = mean over the ensemble members
@@ -951,7 +969,7 @@ int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml) {
     launch_pdl(pdl, ws->stream, k_mlp_tc<3>, dim3(grid), dim3(TC_THREADS), tw->smem_bytes[0], tm->d_nets, tm->d_tabs,
                tw->d_pall, ws->groups, ws->tiles, ws->aev, ws->daev, ws->e_atom, tw->key, tw->done, m->n_members, escale, tw->cscr);
   if (ens) ensemble_guard_after(ws->stream);
-  return 2;
+  return nl + 1;
 }
 
 }  // namespace nnp

@@ -1090,6 +1090,9 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     launch_pdl(!ws->profiling, st, k_cell_sort, dim3((unsigned)((a.hg.ncell + 7) / 8)), dim3(256), 0, q);
     fast_bin = true;
     extra = 1;
+    // the MLP's layer-1 image check and operand prefetch: off the AEV -> MLP edge (mlp_tc.cu launch_tc_pack); stage
+    // profiling keeps it with the MLP stage
+    if (n_ml > 0 && !ws->profiling && !ws->ext_pairs) extra += launch_tc_pack(ws);
   } else if (ws->prep_cluster > 0 && n_ml <= ws->prep_cluster_max) {   // small systems: barrier latency dominates, a few SMs suffice
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(ws->prep_cluster); cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = 0; cfg.stream = st;

@@ -141,6 +141,7 @@ struct nnp_workspace {
   unsigned long long* small_acc;   // [256 * 3] force accumulators of k_small_all (zero between evaluations)
   unsigned int* small_ticket;
   size_t small_all_smem;
+  int pack_done;             // launch_tc_pack has run for this evaluation already (the cell-list path runs it early)
   int64_t max_rows;          // padded AEV rows
   int max_tiles;
   // last evaluation
@@ -271,6 +272,8 @@ int launch_small_front(nnp_workspace* ws, const float* d_pos, const int32_t* d_Z
                        int64_t n_atoms, int64_t n_ml);
 int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
+// the layer-1 image check / repack + L2 prefetch of the MLP operands, ahead of the MLP kernel (see launch_tc_pack)
+int launch_tc_pack(nnp_workspace* ws);
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
                        float* d_forces);
 int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][n_species] */);
