@@ -939,8 +939,11 @@ int launch_tc_pack(nnp_workspace* ws) {
   for (int mem = 0; mem < MAX_MEMBERS; ++mem)
     for (int s = 0; s < MAX_S; ++s) { pall.m[mem].w1[s] = tw->w1img[mem][s]; pall.m[mem].w1t[s] = tw->w1timg[mem][s]; }
   const bool pdl = !ws->profiling;
+  // the operand prefetch pays for one network per element at compact K (~2 MB: step 249.2 -> 247.5 us); with eight members
+  // (16 MB) or dense K (first-layer images of 1 MB each) it costs more in front of k_neighbors than it saves: +6 / +4 us
+  const bool prefetch = pdl && m->n_members == 1 && !ws->dense_k;
   launch_pdl(pdl, ws->stream, k_tc_pack_w1, dim3(32, m->aev.S, m->n_members), dim3(256), 0, tm->d_nets, ws->groups, pall,
-             tm->d_tabs, pdl ? m->Kfull : 0, tw->key, tw->done, ws->max_tiles);
+             tm->d_tabs, prefetch ? m->Kfull : 0, tw->key, tw->done, ws->max_tiles);
   ws->pack_done = 1;
   return 1;
 }
