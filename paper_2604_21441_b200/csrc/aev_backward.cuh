@@ -381,6 +381,11 @@ __device__ __forceinline__ void aev_backward_team(const AevConst& c, const GridI
                                                   int nA, int ip, const float4* gb, int gs,
                                                   unsigned long long* __restrict__ facc, int lane, int tw, int bar, BwdEnv& e,
                                                   BwdTeam<TW>& tm, const int* pairoff) {
+  if (nA > 32) {   // beyond liquid densities: the lanes-hold-neighbours rounds below stop at 32 -- the leader alone takes the
+                   // centre through the one-warp version and its general pair loop (warp-uniform branch, before any barrier)
+    if (tw == 0) aev_backward_centre<false>(c, g, grp, spos, rowR, rowA, nR, nA, ip, gb, gs, facc, nullptr, lane, e, tm.PaccW[0], pairoff);
+    return;
+  }
   if (tw == 0) {
     const float4 ci = spos[ip];
     bwd_load_env(c, g, spos, rowR, rowA, nR, nA, ci, lane, e);
@@ -389,7 +394,7 @@ __device__ __forceinline__ void aev_backward_team(const AevConst& c, const GridI
   for (int j = lane; j < nA; j += 32) { Pacc[j][0] = 0.f; Pacc[j][1] = 0.f; Pacc[j][2] = 0.f; }
   asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(TW * 32) : "memory");
 
-  // ---- angular shares of this warp's iterations -> PaccW[tw]  (nA <= ACAP_MAX = 32: lanes hold the neighbours)
+  // ---- angular shares of this warp's iterations -> PaccW[tw]  (nA <= 32 here: lanes hold the neighbours)
   {
     const int n = nA;
     const float zm1 = c.zeta - 1.0f;

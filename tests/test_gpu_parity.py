@@ -264,6 +264,34 @@ def test_dense_blob_many_angular_neighbours():
     check_EF(Eg, Fg, ref, 40)
 
 
+def test_dense_blob_periodic_small_path():
+    """The same blob in a periodic 24 A box: <= 256 atoms, so the one-kernel path takes it, whose team of warps handles at
+    most 32 angular neighbours per centre and must hand centres beyond that to the general pair loop."""
+    rng = np.random.default_rng(5)
+    pts = []
+    while len(pts) < 40:
+        p = rng.uniform(-2.8, 2.8, 3)
+        if np.linalg.norm(p) <= 2.8 and all(np.linalg.norm(p - q) >= 0.75 for q in pts):
+            pts.append(p)
+    pos = (np.array(pts) + 12.0).astype(np.float32)
+    Z = rng.choice([1, 6, 7, 8], size=40).astype(np.int32)
+    cfg = gen.get_config(4)
+    box = np.diag([24.0, 24.0, 24.0]).astype(np.float32).reshape(9)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    sub = dict(cfg, pos=pos, Z=Z, ml_index=None, box=box)
+    m, ws = make(sub)
+    ref = oracle.evaluate(om, pos, Z, box, 1, None)
+    for on in (2, 1, 0):
+        ws.set_small_path(on)
+        Eg, Fg = run_gpu(ws, pos, Z, box, 1)
+        if on == 2:
+            assert ws.launches() == 1
+        sA, _ = ws.neighbors(1, 40)
+        assert np.diff(sA).max() > 32, np.diff(sA).max()
+        check_lists(ws, sub, pos, 40, None, pbc=1)
+        check_EF(Eg, Fg, ref, 40)
+
+
 def test_one_layer_network_golden_monomer():
     """All-ones one-layer network on a water monomer: E = 7.1130060875."""
     import json, os
