@@ -183,7 +183,9 @@ int nnp_eval(nnp_workspace*, int64_t n_atoms, const float* d_pos, const int32_t*
 /* Same evaluation with HOST buffers: copies inputs to workspace-owned device buffers, runs nnp_eval,
  * copies energy and forces back and synchronises the stream.  h_ml_index may be NULL.  This is the
  * end-to-end entry point a host MD engine (GROMACS nnpot) would call.  Per call: ONE host-to-device
- * copy (positions) and ONE device-to-host copy (forces); the energy arrives through a mapped pinned word the output
+ * copy (positions) and ONE device-to-host copy (forces) -- none for the forces when h_forces is pinned (device-mapped) host
+ * memory, all atoms are ML atoms and the cell-list path runs: the output kernel then writes them in the caller's order
+ * straight into h_forces (coalesced stores over PCIe); the energy arrives through a mapped pinned word the output
  * kernel writes; atomic numbers and the ML index are compared with the copy of the previous call and uploaded only when
  * they changed (a change also ends any binning reuse: the next evaluation bins afresh). */
 int nnp_eval_host(nnp_workspace*, int64_t n_atoms, const float* h_pos, const int32_t* h_Z, const float box[9],

@@ -376,6 +376,7 @@ struct SortArgs {
   GroupInfo* groups; TileInfo* tiles;
   const float4* cellbuf; const int* cell_count; const int* present;
   int* bstart; float4* spos; int* scell; int* flags;
+  int* inv;   // [n_ml] ML-local index -> sorted index (k_force_out writes the forces in the caller's order through it)
   int S, ncell, n_ml, max_tiles, dense_k;
 };
 
@@ -462,7 +463,7 @@ __global__ void __launch_bounds__(256) k_cell_sort(const __grid_constant__ SortA
     for (int u = 0; u < PER; ++u) {
       if (u * 32 + lane < n) {
         const int dst = bst8[warp][(key[u] >> 28) & 7] + rank[u];
-        if (dst < a.n_ml) { a.spos[dst] = e[u]; a.scell[dst] = cell; }
+        if (dst < a.n_ml) { a.spos[dst] = e[u]; a.scell[dst] = cell; a.inv[key[u] & 0x0fffffff] = dst; }
       }
     }
   }
@@ -1067,6 +1068,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
       return 2;
     }
   } else {
+  ws->inv_valid = 0;   // (set again below when k_cell_sort writes the inverse order)
   if (reuse_ok) {
     ws->reuse_left = ws->reuse_every - 1; ws->reuse_n_atoms = n_atoms; ws->reuse_n_ml = n_ml;
     ws->reuse_ml = d_ml; ws->reuse_Z = d_Z;
@@ -1085,11 +1087,12 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     SortArgs q;
     q.groups = ws->groups; q.tiles = ws->tiles;
     q.cellbuf = ws->cellbuf; q.cell_count = ws->cell_count; q.present = ws->present;
-    q.bstart = ws->bstart; q.spos = ws->spos; q.scell = ws->scell; q.flags = ws->flags;
+    q.bstart = ws->bstart; q.spos = ws->spos; q.scell = ws->scell; q.flags = ws->flags; q.inv = ws->inv;
     q.S = m->aev.S; q.ncell = a.hg.ncell; q.n_ml = (int)n_ml; q.max_tiles = ws->max_tiles; q.dense_k = ws->dense_k;
     launch_pdl(!ws->profiling, st, k_cell_sort, dim3((unsigned)((a.hg.ncell + 7) / 8)), dim3(256), 0, q);
     fast_bin = true;
     extra = 1;
+    ws->inv_valid = 1;
     // the MLP's layer-1 image check and operand prefetch: off the AEV -> MLP edge (mlp_tc.cu launch_tc_pack); stage
     // profiling keeps it with the MLP stage
     if (n_ml > 0 && !ws->profiling && !ws->ext_pairs) extra += launch_tc_pack(ws);

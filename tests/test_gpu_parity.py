@@ -205,6 +205,30 @@ def test_bitwise_reproducible_and_host_entry():
     assert ws.launches() > 0
 
 
+def test_host_entry_pinned_force_buffer():
+    """A pinned force buffer is written by the output kernel itself, in the caller's order (no device-to-host copy): same
+    bits as the copy path and the device entry point, on the cell-list path (cfg 1) and with an ML subset (copy path)."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    m, ws = make(cfg)
+    E1, F1 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"])
+    hF = torch.full((n, 3), float("nan"), dtype=torch.float32).pin_memory()
+    nF = hF.numpy()
+    for rep in range(2):
+        E2, F2 = ws.eval_host(cfg["pos"], cfg["Z"], cfg["box"], 1, None, nF)
+        assert ws.status() == 0
+        assert F2 is nF and E2 == E1 and np.array_equal(nF.astype(np.float64), F1)
+        nF[:] = np.nan
+    E3, F3 = ws.eval_host(cfg["pos"], cfg["Z"], cfg["box"])          # pageable buffer: the copy path
+    assert E3 == E1 and np.array_equal(F3.astype(np.float64), F1)
+    ml = np.arange(0, n, 3, dtype=np.int32)                             # index subset: scattered rows, copy path
+    m2, ws2 = make(dict(cfg, ml_index=ml), max_atoms=n)
+    E4, F4 = run_gpu(ws2, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    E5, F5 = ws2.eval_host(cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nF)
+    assert E5 == E4 and np.array_equal(nF.astype(np.float64), F4)
+
+
 def test_nonzero_biases_and_padding_rows():
     """Non-zero biases make MLP(0) != 0: padded tile rows must not leak into E."""
     cfg = _small_cfg(bias_scale=0.3)
