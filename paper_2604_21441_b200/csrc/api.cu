@@ -220,7 +220,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
     ws->small_path = 1;
     ws->small_all = 1;
     ws->pack_done = 0;
-    ws->inv_valid = 0; ws->forces_alias = nullptr; ws->forces_in_alias = 0; ws->alias_host = nullptr; ws->alias_dev = nullptr;
+    ws->inv_valid = 0; ws->forces_alias = nullptr; ws->forces_in_alias = 0;
     ws->prep_cluster_max = 8192;   // measured: 24 000 atoms run 4 us slower in one cluster than on the cooperative grid
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
@@ -420,9 +420,27 @@ extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_
     return NNP_ERR_INVALID_ARG;
   if (h_ml && (n_ml < 0 || n_ml > ws->max_ml)) return NNP_ERR_INVALID_ARG;
   cudaStream_t st = ws->stream;
-  // (positions: read in place from a pinned buffer by the binning kernel was measured too -- e2e 271 -> 286 us: the three
-  // 4-byte loads per atom do not stream over PCIe; the copy stays)
-  CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
+  // Pinned (device-mapped) host buffers can be used by the kernels in place.  (Asked on every call -- ~1 us each: an
+  // address may have been freed and handed out again as pageable memory since the last one.)
+  auto device_alias = [](const void* h) -> void* {
+    cudaPointerAttributes at;
+    if (h && cudaPointerGetAttributes(&at, h) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) return at.devicePointer;
+    cudaGetLastError();
+    return nullptr;
+  };
+  float* const f_alias = n_atoms > 0 ? static_cast<float*>(device_alias(h_forces)) : nullptr;
+  // A small ML region inside a large system (ONE kernel, k_small_all; 14-107 ML atoms among
+  // thousands): the kernel reads the few ML positions it needs from the caller's pinned buffer and writes the force rows
+  // (zeros but for the ML atoms) into the caller's pinned buffer itself, instead of two copies of the whole arrays (cfg 4,
+  // 64 of 9064 atoms: 69.1 -> 64.7 us per call).  Not below 2048 atoms (a 96-atom box: 55.7 -> 57.8 us, the PCIe round
+  // trip inside the kernel costs more than two 1 KB copies), and not for the cell-list path's positions (read in place
+  // by the binning kernel: e2e 271 -> 286 us at 24 000 atoms -- three 4-byte loads per atom do not stream over PCIe); its
+  // forces go in place where the output kernel writes them coalesced (below).
+  const bool small_direct = ws->len_scale == 1.0 && f_alias && n_atoms >= 2048 &&
+                            small_all_applicable(ws, box, pbc, h_ml ? n_ml : n_atoms);
+  const float* const p_alias = small_direct ? static_cast<const float*>(device_alias(h_pos)) : nullptr;
+  const bool in_place = small_direct && p_alias;
+  if (!in_place) CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
   // atomic numbers and the ML index rarely change between MD steps: they are compared with the host copy of the last
   // call and uploaded only when different (the comparison also makes binning reuse safe for this entry point: the
   // device buffers are always the same, so pointer identity alone would say "same atoms" -- a change bins afresh)
@@ -438,23 +456,15 @@ extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_
     ws->hml_n = h_ml ? n_ml : -1; ws->hml_valid = 1;
   }
   if (!z_same || !ml_same) ws->reuse_left = 0;
-  // A pinned (device-mapped) force buffer of the caller is written by the output kernel itself where that kernel writes in
-  // the caller's order (coalesced: force.cu k_force_out): no device-to-host copy then.  The pointer query is remembered.
-  if (h_forces != ws->alias_host) {
-    cudaPointerAttributes at;
-    ws->alias_host = h_forces; ws->alias_dev = nullptr;
-    if (cudaPointerGetAttributes(&at, h_forces) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
-      ws->alias_dev = static_cast<float*>(at.devicePointer);
-    else
-      cudaGetLastError();
-  }
-  ws->forces_alias = (!h_ml && n_atoms > 0) ? ws->alias_dev : nullptr;
+  // A pinned force buffer of the caller is written by the output kernel itself where that kernel writes in the caller's
+  // order (coalesced: force.cu k_force_out): no device-to-host copy then.
+  ws->forces_alias = !h_ml ? f_alias : nullptr;
   ws->forces_in_alias = 0;
-  int rc = nnp_eval(ws, n_atoms, ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml, ws->hd_energy_dev,
-                    ws->hd_forces);
+  int rc = nnp_eval(ws, n_atoms, in_place ? p_alias : ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml,
+                    ws->hd_energy_dev, in_place ? f_alias : ws->hd_forces);
   ws->forces_alias = nullptr;
   if (rc) return rc;
-  if (!ws->forces_in_alias)
+  if (!ws->forces_in_alias && !in_place)
     CU_OK(cudaMemcpyAsync(h_forces, ws->hd_forces, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyDeviceToHost, st));
   CU_OK(cudaStreamSynchronize(st));
   *h_energy = *ws->hd_energy;   // mapped pinned word, written by the output kernel (or the memset of an empty subset)

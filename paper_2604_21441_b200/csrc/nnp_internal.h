@@ -144,7 +144,6 @@ struct nnp_workspace {
   int* inv;                  // [max_ml] ML-local index -> sorted index (written by k_cell_sort)
   int inv_valid;             // inv matches the current sorted order
   float* forces_alias;       // nnp_eval_host: device alias of the caller's pinned force buffer, or NULL
-  const float* alias_host; float* alias_dev;   // the last host force buffer seen and its device alias (NULL: not pinned)
   int forces_in_alias;       // the last evaluation wrote its forces straight through forces_alias
   int pack_done;             // launch_tc_pack has run for this evaluation already (the cell-list path runs it early)
   int64_t max_rows;          // padded AEV rows

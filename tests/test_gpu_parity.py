@@ -229,6 +229,28 @@ def test_host_entry_pinned_force_buffer():
     assert E5 == E4 and np.array_equal(nF.astype(np.float64), F4)
 
 
+def test_host_entry_small_region_in_place():
+    """cfg 4 (64 ML atoms of 9064) through nnp_eval_host with pinned buffers: the one-kernel path reads the positions from
+    and writes the forces into the caller's buffers (no copies); same bits as the device entry point, rows of the other
+    atoms +0.0f, twice in a row (the second call must clear what the first one left)."""
+    torch = _torch()
+    cfg = gen.get_config(4)
+    n = cfg["pos"].shape[0]
+    ml = cfg["ml_index"]
+    m, ws = make(cfg)
+    E1, F1 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert ws.launches() == 1
+    hP = torch.from_numpy(np.ascontiguousarray(cfg["pos"], np.float32)).pin_memory().numpy()
+    hF = torch.full((n, 3), float("nan"), dtype=torch.float32).pin_memory().numpy()
+    for rep in range(2):
+        E2, F2 = ws.eval_host(hP, cfg["Z"], cfg["box"], 1, ml, hF)
+        assert ws.status() == 0 and ws.launches() == 1
+        assert E2 == E1 and np.array_equal(hF.astype(np.float64), F1)
+        mm = np.setdiff1d(np.arange(n), ml)
+        assert np.all(hF[mm] == 0.0) and not np.any(np.signbit(hF[mm]))
+        hF[:] = np.nan
+
+
 def test_nonzero_biases_and_padding_rows():
     """Non-zero biases make MLP(0) != 0: padded tile rows must not leak into E."""
     cfg = _small_cfg(bias_scale=0.3)
