@@ -411,6 +411,38 @@ def test_error_reporting():
     check_EF(Eg, Fg, ref, cfg["pos"].shape[0])
 
 
+def test_capacity_overflow_is_reported_and_recovered_from():
+    """150 atoms within 2.9 A of one point: every radial row (capacity 128), every angular row (48) and -- in a periodic box
+    with a cell grid -- one cell's append buffer (96) overflow.  Every path must report NNP_ERR_CAPACITY (-4) instead of
+    wrong numbers, and the workspace must evaluate correctly afterwards (the cell-list path by its general binning)."""
+    rng = np.random.default_rng(11)
+    pts = []
+    while len(pts) < 150:
+        p = rng.uniform(-2.9, 2.9, 3)
+        if np.linalg.norm(p) <= 2.9 and all(np.linalg.norm(p - q) >= 0.7 for q in pts):
+            pts.append(p)
+    cfg = gen.get_config(4)
+    box = np.diag([24.0, 24.0, 24.0]).astype(np.float32).reshape(9)
+    pos = (np.array(pts) + 12.0).astype(np.float32)
+    Z = rng.choice([1, 6, 7, 8], size=150).astype(np.int32)
+    m, ws = make(dict(cfg, pos=pos, Z=Z, ml_index=None, box=box))
+    torch = _torch()
+    dpos, dZ = torch.from_numpy(pos).cuda(), torch.from_numpy(Z).cuda()
+    for on, pbc in ((2, 1), (1, 1), (0, 1), (0, 0)):   # one kernel / small front end / cell list / open boundaries
+        ws.set_small_path(on)
+        ws.eval(dpos, dZ, box, pbc)
+        assert ws.status() == -4, (on, pbc)
+    # afterwards: the 40-atom blob of the tests above, on every path, against the oracle
+    pos40, Z40 = pos[:40].copy(), Z[:40].copy()
+    pos40 = (12.0 + (pos40 - 12.0) * 1.6).astype(np.float32)   # spread out: no row overflows any more
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    for on, pbc in ((2, 1), (1, 1), (0, 1), (0, 0)):
+        ws.set_small_path(on)
+        ref = oracle.evaluate(om, pos40, Z40, box, pbc, None)
+        Eg, Fg = run_gpu(ws, pos40, Z40, box, pbc)
+        check_EF(Eg, Fg, ref, 40)
+
+
 # ------------------------------------------------------------------ link atoms (PAPER.md lines 77-82, eq. 4)
 @pytest.mark.parametrize("pbc", [0, 1])
 def test_link_atoms_place_eval_spread(pbc):
@@ -930,6 +962,45 @@ def test_bin_reuse_over_md_like_steps():
     m2, ws2 = make(cfg)
     E2, F2 = run_gpu(ws2, P[3], cfg["Z"], cfg["box"])
     assert E1 == E2 and np.array_equal(F1, F2)
+
+
+def test_host_entry_pinned_buffers_with_reuse_and_changing_sizes():
+    """The output kernel writes a pinned force buffer in the caller's order through the inverse map of the LAST cell sort:
+    reuse steps (no sort) must still use the right map, and a later call with fewer atoms on the same workspace a new one.
+    Device entry point on a second workspace = the reference bits."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    P = gen.perturbed_positions(cfg["pos64"], cfg["perturb_seed"], 7, sigma=0.05)
+    m, ws = make(cfg)
+    m2, ws2 = make(cfg)
+    ws.set_bin_reuse(5, 1.0)
+    ws2.set_bin_reuse(5, 1.0)
+    hP = torch.empty((n, 3), dtype=torch.float32).pin_memory().numpy()
+    hF = torch.empty((n, 3), dtype=torch.float32).pin_memory().numpy()
+    dZ = torch.from_numpy(cfg["Z"]).cuda()
+    dpos = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    for t in range(7):
+        hP[:] = P[t]
+        hF[:] = np.nan
+        E, F = ws.eval_host(hP, cfg["Z"], cfg["box"], 1, None, hF)
+        assert ws.status() == 0 and ws.launches() == (8 if t % 5 == 0 else 7)
+        dpos.copy_(torch.from_numpy(P[t]))
+        E2, F2 = ws2.eval(dpos, dZ, cfg["box"], 1)
+        torch.cuda.synchronize()
+        assert ws2.status() == 0
+        assert E == float(E2.cpu()[0]) and np.array_equal(hF, F2.cpu().numpy()), t
+    # fewer atoms (the first 800 waters; same box: a thinner liquid) on the same workspace and the same pinned buffers
+    ws.set_bin_reuse(0)
+    k = 2400
+    pos_k, Z_k = np.ascontiguousarray(P[0][:k]), np.ascontiguousarray(cfg["Z"][:k])
+    hP[:k] = pos_k
+    hF[:] = np.nan
+    E, F = ws.eval_host(hP[:k], Z_k, cfg["box"], 1, None, hF[:k])
+    assert ws.status() == 0
+    m3, ws3 = make(dict(cfg, pos=pos_k, Z=Z_k))
+    E3, F3 = run_gpu(ws3, pos_k, Z_k, cfg["box"])
+    assert E == E3 and np.array_equal(hF[:k].astype(np.float64), F3) and np.all(np.isnan(hF[k:]))
 
 
 def test_bin_reuse_triclinic():
