@@ -379,7 +379,7 @@ def run_ours(args, rank, world, local_rank):
         "ns_per_day_2fs": 0.1728 * args.steps / total_s,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 12 * n, "d2h_bytes_per_step": 12 * n + 8,
                 "ms_per_step": 1e3 * e2e_s / args.steps,
-                "note": "nnp_eval_host: positions H2D (copy), forces written by the output kernel straight into the pinned host buffer, energy through a mapped pinned word; Z is uploaded only when it changed"},
+                "note": "nnp_eval_host: positions read from the pinned host buffer by the binning kernel, forces written by the output kernel straight into the pinned host buffer, energy through a mapped pinned word; Z is uploaded only when it changed"},
         "gpu_launches": int(launches_per_step * args.steps),
         "clocks": clk, "roofline": roof, "stages": stages, "cpu_baseline": cpu,
         "vs_cpu_baseline": (value / cpu["value"]) if cpu else None, "fp32_peak_tflops": fp32,

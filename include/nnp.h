@@ -185,7 +185,8 @@ int nnp_eval(nnp_workspace*, int64_t n_atoms, const float* d_pos, const int32_t*
  * end-to-end entry point a host MD engine (GROMACS nnpot) would call.  Per call: ONE host-to-device
  * copy (positions) and ONE device-to-host copy (forces) -- none for the forces when h_forces is pinned (device-mapped) host
  * memory, all atoms are ML atoms and the cell-list path runs: the output kernel then writes them in the caller's order
- * straight into h_forces (coalesced stores over PCIe).  A small ML region inside a system of >= 2048 atoms (the one-kernel
+ * straight into h_forces (coalesced stores over PCIe), and pinned positions are uploaded by the binning kernel itself
+ * (each block streams the 3 KB of its atoms) instead of by a copy in front of it.  A small ML region inside a system of >= 2048 atoms (the one-kernel
  * path) with pinned h_pos and h_forces runs without either copy: the kernel uses both buffers in place.  The energy
  * arrives through a mapped pinned word the output kernel writes; atomic numbers and the ML index are compared with the copy of the previous call and uploaded only when
  * they changed (a change also ends any binning reuse: the next evaluation bins afresh). */

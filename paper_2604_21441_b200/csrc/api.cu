@@ -221,6 +221,7 @@ extern "C" int nnp_workspace_create(const nnp_model* m, int64_t max_atoms, int64
     ws->small_all = 1;
     ws->pack_done = 0;
     ws->inv_valid = 0; ws->forces_alias = nullptr; ws->forces_in_alias = 0;
+    ws->pos_src_host = nullptr; ws->pos_src_dev = nullptr; ws->pos_src_bytes = 0;
     ws->prep_cluster_max = 8192;   // measured: 24 000 atoms run 4 us slower in one cluster than on the cooperative grid
   }
   ws->max_tiles = (int)(max_ml / TILE_M) + m->aev.S + 1;
@@ -356,6 +357,12 @@ static int check_box(const float* box, int pbc) {
   return NNP_OK;
 }
 
+void nnp::flush_pos_upload(nnp_workspace* ws) {
+  if (!ws->pos_src_host) return;
+  cudaMemcpyAsync(ws->hd_pos, ws->pos_src_host, ws->pos_src_bytes, cudaMemcpyHostToDevice, ws->stream);
+  ws->pos_src_host = nullptr; ws->pos_src_dev = nullptr;
+}
+
 extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, const int32_t* d_Z, const float box[9],
                         int32_t pbc, const int32_t* d_ml, int64_t n_ml, double* d_energy, float* d_forces) {
   if (!ws || n_atoms < 0 || !d_energy || (n_atoms > 0 && (!d_pos || !d_Z || !d_forces))) return NNP_ERR_INVALID_ARG;
@@ -376,11 +383,13 @@ extern "C" int nnp_eval(nnp_workspace* ws, int64_t n_atoms, const float* d_pos, 
   ws->tile_done = nullptr;
   // small periodic ML region, everything in ONE kernel: no memset, no other launch
   if (ws->len_scale == 1.0 && small_all_applicable(ws, box, pbc, n_ml)) {
+    flush_pos_upload(ws);
     ws->inv_valid = 0;   // (another sorted order from here on)
     ws->launches = launch_small_all(ws, d_pos, d_Z, box, d_ml, n_atoms, n_ml, d_energy, d_forces);
     if (cudaGetLastError() != cudaSuccess) return NNP_ERR_CUDA;
     return NNP_OK;
   }
+  if (ws->len_scale != 1.0 || d_ml || n_ml <= 0 || small_front_applicable(ws, box, pbc, n_ml)) flush_pos_upload(ws);
   // rows of non-ML atoms are +0.0f; with no index subset every row is written by k_force_out
   if (n_atoms > 0 && (d_ml || n_ml <= 0)) cudaMemsetAsync(d_forces, 0, sizeof(float) * 3 * (size_t)n_atoms, ws->stream);
   if (ws->len_scale != 1.0) {   // unit conversion (GROMACS: nm -> Angstrom), see nnp_workspace_set_units
@@ -440,7 +449,14 @@ extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_
                             small_all_applicable(ws, box, pbc, h_ml ? n_ml : n_atoms);
   const float* const p_alias = small_direct ? static_cast<const float*>(device_alias(h_pos)) : nullptr;
   const bool in_place = small_direct && p_alias;
-  if (!in_place) CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
+  ws->pos_src_host = nullptr; ws->pos_src_dev = nullptr;
+  if (!in_place) {
+    // cell-list path with all atoms ML atoms and pinned positions: the upload is left to the binning kernel (pending here,
+    // flush_pos_upload turns it into this copy on every other path)
+    const float* up = (!h_ml && n_atoms >= 2048 && f_alias) ? static_cast<const float*>(device_alias(h_pos)) : nullptr;
+    if (up) { ws->pos_src_host = h_pos; ws->pos_src_dev = up; ws->pos_src_bytes = sizeof(float) * 3 * (size_t)n_atoms; }
+    else CU_OK(cudaMemcpyAsync(ws->hd_pos, h_pos, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyHostToDevice, st));
+  }
   // atomic numbers and the ML index rarely change between MD steps: they are compared with the host copy of the last
   // call and uploaded only when different (the comparison also makes binning reuse safe for this entry point: the
   // device buffers are always the same, so pointer identity alone would say "same atoms" -- a change bins afresh)
@@ -463,6 +479,7 @@ extern "C" int nnp_eval_host(nnp_workspace* ws, int64_t n_atoms, const float* h_
   int rc = nnp_eval(ws, n_atoms, in_place ? p_alias : ws->hd_pos, ws->hd_Z, box, pbc, h_ml ? ws->hd_ml : nullptr, n_ml,
                     ws->hd_energy_dev, in_place ? f_alias : ws->hd_forces);
   ws->forces_alias = nullptr;
+  ws->pos_src_host = nullptr; ws->pos_src_dev = nullptr;   // (an evaluation that failed before its first launch)
   if (rc) return rc;
   if (!ws->forces_in_alias && !in_place)
     CU_OK(cudaMemcpyAsync(h_forces, ws->hd_forces, sizeof(float) * 3 * (size_t)n_atoms, cudaMemcpyDeviceToHost, st));

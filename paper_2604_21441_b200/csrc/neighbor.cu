@@ -343,6 +343,7 @@ struct BinArgs {
   float4* cellbuf; int* cellfill; int* cell_count; int* present;
   unsigned long long* facc; int* flags;
   int n_atoms, n_ml;
+  const float* pos_src; float* pos_dst;   // nnp_eval_host: the caller's pinned positions, to be staged into pos (= pos_dst) here
 };
 
 __global__ void __launch_bounds__(BIN_THREADS) k_bin_cells(const __grid_constant__ BinArgs a) {
@@ -352,6 +353,17 @@ __global__ void __launch_bounds__(BIN_THREADS) k_bin_cells(const __grid_constant
   const GridInfo* g = &a.hg;
   if (threadIdx.x == 0) spres = 0;
   if (blockIdx.x == 0 && threadIdx.x == 0) *a.grid = a.hg;
+  if (a.pos_src) {
+    // the host entry point's upload, done here: the block streams the 768 floats of ITS atoms from the caller's pinned
+    // buffer (whole 128-byte lines over PCIe) into the device copy every later reader uses, and goes on with them
+    // (all atoms are ML atoms in this mode: atom i = thread i).  Saves the copy's launch and its ~10 us ahead of this kernel.
+    const size_t base = (size_t)blockIdx.x * (3 * BIN_THREADS), lim = 3 * (size_t)a.n_atoms;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const size_t idx = base + threadIdx.x + BIN_THREADS * k;
+      if (idx < lim) a.pos_dst[idx] = a.pos_src[idx];
+    }
+  }
   __syncthreads();
   const int i = blockIdx.x * BIN_THREADS + threadIdx.x;
   int bit = 0;
@@ -1051,6 +1063,7 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
   const bool tric_box = pbc && box_is_triclinic(box);
   const bool fast = a.host_grid && a.hg.nc[0] >= 3 && a.hg.nc[1] >= 3 && a.hg.nc[2] >= 3 && !ws->ext_pairs && !ws->slow_prep &&
                     a.hg.ncell <= ws->max_cells && a.hg.ncell <= FAST_MAX_CELLS;
+  if (same || !fast) flush_pos_upload(ws);   // (k_bin_cells stages a pending upload itself)
   int extra = 0;   // kernels launched beyond the first
   bool fast_bin = false;   // this evaluation binned with k_bin_cells (k_neighbors clears its counters)
   if (same) {
@@ -1083,6 +1096,11 @@ int launch_neighbor_stage(nnp_workspace* ws, const float* d_pos, const int32_t* 
     b.cellbuf = ws->cellbuf; b.cellfill = ws->cellfill; b.cell_count = ws->cell_count; b.present = ws->present;
     b.facc = ws->facc; b.flags = ws->flags;
     b.n_atoms = (int)n_atoms; b.n_ml = (int)n_ml;
+    b.pos_src = nullptr; b.pos_dst = nullptr;
+    if (ws->pos_src_dev && !d_ml && d_pos == ws->hd_pos) {   // (the pending upload of nnp_eval_host: staged by the kernel)
+      b.pos_src = ws->pos_src_dev; b.pos_dst = ws->hd_pos;
+      ws->pos_src_host = nullptr; ws->pos_src_dev = nullptr;
+    }
     k_bin_cells<<<(unsigned)((n_ml + BIN_THREADS - 1) / BIN_THREADS), BIN_THREADS, 0, st>>>(b);
     SortArgs q;
     q.groups = ws->groups; q.tiles = ws->tiles;

@@ -144,6 +144,9 @@ struct nnp_workspace {
   int* inv;                  // [max_ml] ML-local index -> sorted index (written by k_cell_sort)
   int inv_valid;             // inv matches the current sorted order
   float* forces_alias;       // nnp_eval_host: device alias of the caller's pinned force buffer, or NULL
+  // nnp_eval_host with pinned positions: the upload into hd_pos is still pending when nnp_eval starts -- the binning
+  // kernel of the cell-list path does it itself (coalesced, block by block), every other path asks for the copy first
+  const float* pos_src_host; const float* pos_src_dev; size_t pos_src_bytes;
   int forces_in_alias;       // the last evaluation wrote its forces straight through forces_alias
   int pack_done;             // launch_tc_pack has run for this evaluation already (the cell-list path runs it early)
   int64_t max_rows;          // padded AEV rows
@@ -278,6 +281,8 @@ int launch_mlp_simt(nnp_workspace* ws, int64_t n_ml);
 int launch_mlp_tc(nnp_workspace* ws, int64_t n_ml);
 // the layer-1 image check / repack + L2 prefetch of the MLP operands, ahead of the MLP kernel (see launch_tc_pack)
 int launch_tc_pack(nnp_workspace* ws);
+// the pending position upload of nnp_eval_host, as a copy (no-op when there is none)
+void flush_pos_upload(nnp_workspace* ws);
 int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const int32_t* d_ml, double* d_energy,
                        float* d_forces);
 int tc_model_create(nnp_model* m, const nnp_mlp_desc* nets /* [n_members][n_species] */);
