@@ -1003,6 +1003,39 @@ def test_host_entry_pinned_buffers_with_reuse_and_changing_sizes():
     assert E == E3 and np.array_equal(hF[:k].astype(np.float64), F3) and np.all(np.isnan(hF[k:]))
 
 
+def test_host_entry_pinned_buffers_on_the_other_paths():
+    """Pinned host buffers where the binning kernel does NOT do the upload itself and the output kernel does not write in
+    place: open boundaries (general binning), unit conversion (positions are scaled first), an external pair list.  The
+    pending upload must become a copy on each of them: same bits as the device entry point."""
+    torch = _torch()
+    cfg = gen.get_config(1)
+    n = cfg["pos"].shape[0]
+    hP = torch.from_numpy(np.ascontiguousarray(cfg["pos"], np.float32)).pin_memory().numpy()
+    hF = torch.empty((n, 3), dtype=torch.float32).pin_memory().numpy()
+    m, ws = make(cfg)
+    # open boundaries
+    E0, F0 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 0)
+    hF[:] = np.nan
+    E1, _ = ws.eval_host(hP, cfg["Z"], cfg["box"], 0, None, hF)
+    assert ws.status() == 0 and E1 == E0 and np.array_equal(hF.astype(np.float64), F0)
+    # nm / kJ/mol
+    ws.set_units(10.0, 96.485)
+    pos_nm = (cfg["pos"] / 10.0).astype(np.float32)
+    box_nm = (cfg["box"] / 10.0).astype(np.float32)
+    E0, F0 = run_gpu(ws, pos_nm, cfg["Z"], box_nm, 1)
+    hP[:] = pos_nm
+    hF[:] = np.nan
+    E1, _ = ws.eval_host(hP, cfg["Z"], box_nm, 1, None, hF)
+    assert ws.status() == 0 and E1 == E0 and np.array_equal(hF.astype(np.float64), F0)
+    ws.set_units(1.0, 1.0)
+    # periodic again, the in-place path, after the others
+    hP[:] = cfg["pos"]
+    E0, F0 = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1)
+    hF[:] = np.nan
+    E1, _ = ws.eval_host(hP, cfg["Z"], cfg["box"], 1, None, hF)
+    assert ws.status() == 0 and E1 == E0 and np.array_equal(hF.astype(np.float64), F0)
+
+
 def test_bin_reuse_triclinic():
     torch = _torch()
     cfg = gen.get_config(1)
