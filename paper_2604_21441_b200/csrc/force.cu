@@ -12,6 +12,17 @@
 
 namespace nnp {
 
+#ifndef BWD_ROUNDS
+#define BWD_ROUNDS 2
+#endif
+constexpr int BWD_CENTRES = AEV_WARPS * BWD_ROUNDS;   // centres of a LONG block: BWD_ROUNDS per warp, one after the other
+// Block shapes.  A block's start-up (launch, pair table, flag poll, two barriers: ~1.5 us) is a tenth of a centre's time, so
+// the first BWD_LONG_PCT % of the centres go to long blocks that pay it once for BWD_ROUNDS centres per warp; the rest -- the
+// end of the grid -- stays one centre per warp, because long blocks at the end stretch the drain.  cfg 2, kernel alone /
+// whole step (us): one round everywhere 83.7 / 247.2; two rounds everywhere 79.9 / 248.6 (the drain eats the gain);
+// two rounds for 80 %, one for the rest 77.7 / 241.0; 70 %: 76.9 / 241.5; 90 %: 77.3 / 241.5; three rounds for 75 %: 77.0 /
+// 241.4; four for 60 %: 76.5 / 241.3.  (The same for k_aev_forward, whose blocks have no such start-up: 66.2 -> 67.8 us.)
+
 template <bool VIRIAL>
 // 7 blocks of 4 warps per SM: 72 registers, 32 bytes of spills outside the triplet loop.  Alone the kernel gains little over
 // 6 blocks / 80 registers (84.2 -> 83.5 us), but the step gains 5 us (253.4 -> 248.4 us, same box, alternating runs): while the
@@ -22,7 +33,7 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
                const float4* __restrict__ spos, const uint32_t* __restrict__ nbrR, const uint8_t* __restrict__ nbrA,
                const int* __restrict__ cntR, const int* __restrict__ cntA, int n_ml, int rcap, int acap,
                const float* daev, unsigned long long* __restrict__ facc, long long* __restrict__ wcentre,
-               const int* tile_done, int done_target, int* __restrict__ flags) {
+               const int* tile_done, int done_target, int* __restrict__ flags, int nb_long) {
   __shared__ BwdEnv env[AEV_WARPS];
   __shared__ int timed_out;
   __shared__ float Pacc[AEV_WARPS][ACAP_MAX][3];
@@ -40,8 +51,11 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   // whole kernel.  Thread t looks after centre t and polls only where the tile changes (the rows of a block are
   // contiguous: one poller per block almost always -- thousands of polling warps saturate the L2 slice that holds
   // the flags and slow the MLP's weight stream down).  dE/dAEV is read through ordinary (coherent) loads.
-  if (tile_done && threadIdx.x < AEV_WARPS) {
-    const int ipw = blockIdx.x * AEV_WARPS + threadIdx.x;
+  // the first nb_long blocks take BWD_ROUNDS centres per warp, the others (the end of the grid: a short drain) one
+  const int rounds = (int)blockIdx.x < nb_long ? BWD_ROUNDS : 1;
+  const int ip0 = (int)blockIdx.x < nb_long ? (int)blockIdx.x * BWD_CENTRES : nb_long * BWD_CENTRES + ((int)blockIdx.x - nb_long) * AEV_WARPS;
+  if (tile_done && threadIdx.x < rounds * AEV_WARPS) {
+    const int ipw = ip0 + threadIdx.x;
     if (ipw < n_ml) {
       const int tw = (ipw + grp->pad_shift[(__float_as_int(spos[ipw].w) >> 28) & 7]) / TILE_M;
       bool poll = true;
@@ -61,7 +75,9 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   __syncthreads();
   TL_WAITED(0);   // (here: the block's tile flags are up)
   if (timed_out) return;
-  const int ip = blockIdx.x * AEV_WARPS + w;
+#pragma unroll 1
+  for (int r = 0; r < rounds; ++r) {
+  const int ip = ip0 + r * AEV_WARPS + w;
   if (ip >= n_ml) return;
   const float4 ci = spos[ip];
   const int si = (__float_as_int(ci.w) >> 28) & 7;
@@ -73,6 +89,8 @@ k_aev_backward(AevConst c, const GridInfo* __restrict__ g, const GroupInfo* __re
   const float4* gb = reinterpret_cast<const float4*>(daev + daev_off((size_t)(ip + grp->pad_shift[si]), 0, Kc));
   aev_backward_centre<VIRIAL>(c, g, grp, spos, nbrR + (size_t)ip * rcap, nbrA + (size_t)ip * acap, cntR[ip], cntA[ip], ip, gb, TILE_M,
                               facc, wcentre, lane, env[w], Pacc[w], pairoff);
+  __syncwarp();
+  }
 }
 
 // K8b: facc (sorted order, fixed point; = sum_j (p_aj - p_ja) = +F) -> forces in the caller's atom order, and
@@ -172,18 +190,24 @@ int launch_force_stage(nnp_workspace* ws, int64_t n_atoms, int64_t n_ml, const i
   int nl = 0;
   // (rows of non-ML atoms are +0.0f: nnp_eval clears the force array before the first kernel when a subset is given)
   if (n_ml > 0) {
-    const int nb = (int)((n_ml + AEV_WARPS - 1) / AEV_WARPS);
+#ifndef BWD_LONG_PCT
+#define BWD_LONG_PCT 80
+#endif
+    // (only where one-round blocks would run several waves anyway -- 7 blocks x 148 SMs hold 4144 centres: at 3000 atoms long
+    // blocks turned one wave into two rounds, 89 -> 94 us per evaluation)
+    const int nb_long = n_ml >= 8192 ? (int)(n_ml * BWD_LONG_PCT / 100 / BWD_CENTRES) : 0;
+    const int nb = nb_long + (int)((n_ml - (int64_t)nb_long * BWD_CENTRES + AEV_WARPS - 1) / AEV_WARPS);
     // after the tcgen05 MLP kernel the launch is a programmatic dependent launch: blocks start on the SMs the
     // persistent MLP CTAs have left and wait per tile (see the kernel); stage profiling keeps the stages apart
     const int* done = ws->profiling ? nullptr : ws->tile_done;
     if (ws->d_virial)
       launch_pdl(done != nullptr, ws->stream, k_aev_backward<true>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
                  ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
-                 ws->facc, ws->wcentre, done, ws->tile_done_target, ws->flags);
+                 ws->facc, ws->wcentre, done, ws->tile_done_target, ws->flags, nb_long);
     else
       launch_pdl(done != nullptr, ws->stream, k_aev_backward<false>, dim3(nb), dim3(AEV_WARPS * 32), 0, m->aev, ws->grid,
                  ws->groups, ws->spos, ws->nbrR, ws->nbrA, ws->cntR, ws->cntA, (int)n_ml, ws->rcap, ws->acap, ws->daev,
-                 ws->facc, nullptr, done, ws->tile_done_target, ws->flags);
+                 ws->facc, nullptr, done, ws->tile_done_target, ws->flags, nb_long);
     prof_mark(ws, 4);
     // forces in the caller's order through the inverse map, straight into the caller's pinned host buffer (nnp_eval_host
     // sets forces_alias), where there is such a map and no index subset
