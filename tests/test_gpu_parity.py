@@ -155,6 +155,29 @@ def test_config2_full_size():
     check_EF(Eg2, Fg2, ref, n)
 
 
+@pytest.mark.parametrize("n_sub", [8191, 8193, 8205])
+def test_backward_block_shapes_around_the_threshold(n_sub):
+    """k_aev_backward gives long blocks (two centres per warp) to the first 80 % of the grid from 8192 ML atoms on and
+    one-centre blocks to the rest: ML subsets of cfg 2 just below / above the threshold, sizes that are no multiple of a
+    block, with and without virial output (the other instantiation) -- E, F, virial against the oracle."""
+    cfg = gen.get_config(2)
+    n = cfg["pos"].shape[0]
+    ml = np.sort(np.random.default_rng(n_sub).choice(n, size=n_sub, replace=False)).astype(np.int32)
+    om = oracle.Model(cfg["aev"], cfg["nets"], cfg["celu_alpha"])
+    ref = oracle.evaluate(om, cfg["pos"], cfg["Z"], cfg["box"], 1, ml, nbr_mode=1)
+    m, ws = make(dict(cfg, ml_index=ml), max_atoms=n)
+    Eg, Fg = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    check_EF(Eg, Fg, ref, n_sub, rows=ml)
+    mm = np.setdiff1d(np.arange(n), ml)
+    assert np.all(Fg[mm] == 0.0)
+    torch = _torch()
+    W = torch.zeros(9, dtype=torch.float64, device="cuda")
+    ws.set_virial_output(W)
+    Ev, Fv = run_gpu(ws, cfg["pos"], cfg["Z"], cfg["box"], 1, ml)
+    assert Ev == Eg and np.array_equal(Fv, Fg)          # the virial instantiation: same forces, bit for bit
+    ws.set_virial_output(None)
+
+
 def test_config3_sampled():
     """cfg 3 (96 000 atoms): lists bit-exact; E/F checked on every atom with the oracle's cell-list mode."""
     cfg = gen.get_config(3)
